@@ -1,0 +1,300 @@
+"""Pins for the CPU oracle (oracle/) against what the paper and mathematics fix.
+
+None of these compares the oracle with itself or with the CUDA path: each one
+ties an oracle function to a closed form, a library routine on a special case,
+an invariant, or brute force written independently here (SURVEY.md 8(c) table
+"What pins the oracle").
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate, special
+
+import oracle
+import workloads
+
+RNG = np.random.default_rng(7)
+
+
+def rel(a, b):
+    return np.linalg.norm(np.ravel(a) - np.ravel(b)) / np.linalg.norm(np.ravel(b))
+
+
+def dirichlet_np(u, n):
+    """Closed-form sum_j exp(i 2 pi j u / n)/n over j=-floor(n/2)..ceil(n/2)-1, real part."""
+    u = np.asarray(u, dtype=np.float64)
+    den = n * np.sin(np.pi * u / n)
+    num = np.sin(np.pi * u) * (np.cos(np.pi * u / n) if n % 2 == 0 else 1.0)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        out = num / den
+    out[np.abs(den) < 1e-12] = 1.0
+    return out
+
+
+# ---------------------------------------------------------------- C1 delta ----
+@pytest.mark.parametrize("n_det", [33, 48])        # odd and even detector counts
+def test_c1_delta_pixel_is_dirichlet_kernel(n_det):
+    """delta at (iy0,ix0) => S[a,s] = D_n(t_s - X0 cos - Y0 sin): pins centre,
+    sign, orientation, angle direction and scale of the whole (linear) operator."""
+    N, n_angles = 32, 20
+    for (iy0, ix0) in [(16, 16), (3, 29), (20, 7)]:
+        S = oracle.forward(workloads.delta_image(N, iy0, ix0), n_angles, n_det)
+        th = np.pi * np.arange(n_angles) / n_angles
+        tau = (ix0 - N // 2) * np.cos(th) + (iy0 - N // 2) * np.sin(th)
+        t = np.arange(n_det) - n_det // 2
+        ref = dirichlet_np(t[None, :] - tau[:, None], n_det)
+        assert np.abs(S - ref).max() < 1e-12
+
+
+def test_c1b_dirichlet_closed_form_function_matches_direct_sum():
+    """odirichlet_forward (closed form) == odirect_forward (double sum) on noise."""
+    x = RNG.standard_normal((16, 16))
+    for n_det in (23, 24):
+        assert np.abs(oracle.forward(x, 9, n_det) - oracle.dirichlet_forward(x, 9, n_det)).max() < 1e-11
+
+
+# --------------------------------------------------- C2 axis-aligned slices ----
+def test_c2_axis_rows_are_column_and_row_sums():
+    N, n_angles, n_det = 24, 8, 31          # n_det >= N, even n_angles
+    x = RNG.standard_normal((N, N))
+    S = oracle.forward(x, n_angles, n_det)
+    cd, c = n_det // 2, N // 2
+    col = np.zeros(n_det); col[cd - c + np.arange(N)] = x.sum(axis=0)
+    row = np.zeros(n_det); row[cd - c + np.arange(N)] = x.sum(axis=1)
+    assert np.abs(S[0] - col).max() < 1e-12              # theta = 0: t = X
+    assert np.abs(S[n_angles // 2] - row).max() < 1e-12  # theta = pi/2: t = Y
+
+
+def test_c2b_fourier_slice_against_numpy_fft2():
+    """n_det == N: the theta=0 radial line of ndft2 is the ky=0 row of fft2(x),
+    the theta=pi/2 line the kx=0 column, up to the centring phase."""
+    N = 16
+    x = RNG.standard_normal((N, N))
+    F = oracle.ndft2(x, 2, N)                     # angles 0 and pi/2
+    X2 = np.fft.fft2(x)
+    c = N // 2
+    j = np.arange(N) - c
+    phase = np.exp(2j * np.pi * j * c / N)        # image origin at pixel c
+    assert np.abs(F[0] - X2[0, j % N] * phase).max() < 1e-11
+    assert np.abs(F[1] - X2[j % N, 0] * phase).max() < 1e-11
+
+
+def test_ndft2_on_cartesian_points_equals_fft2_everywhere():
+    """Brute-force check of the 2-D phase: for n_det = N and theta in {0, pi/2} done
+    above; here a complex image and the conjugate-transpose pair."""
+    N = 8
+    x = RNG.standard_normal((N, N)) + 1j * RNG.standard_normal((N, N))
+    n_angles, n_det = 5, 9
+    F = oracle.ndft2(x, n_angles, n_det)
+    # brute force, written independently with a dense matrix
+    c, cd = N // 2, n_det // 2
+    iy, ix = np.mgrid[0:N, 0:N]
+    A = np.empty((n_angles * n_det, N * N), dtype=complex)
+    for a in range(n_angles):
+        th = math.pi * a / n_angles
+        for k in range(n_det):
+            w = 2 * math.pi * (k - cd) / n_det
+            A[a * n_det + k] = np.exp(-1j * w * ((ix - c) * math.cos(th) + (iy - c) * math.sin(th))).ravel()
+    assert np.abs(F.ravel() - A @ x.ravel()).max() < 1e-11
+    P = RNG.standard_normal((n_angles, n_det)) + 1j * RNG.standard_normal((n_angles, n_det))
+    z = oracle.ndft1(P, N)
+    assert np.abs(z.ravel() - A.conj().T @ P.ravel()).max() < 1e-11
+
+
+# ------------------------------------------------------------ C3 Gaussian ----
+def test_c3_gaussian_blob_matches_continuous_radon():
+    N, n_angles, n_det, s = 64, 12, 91, 3.5
+    x0, y0 = 5.25, -7.5
+    S = oracle.forward(workloads.gaussian_blob(N, x0, y0, s), n_angles, n_det)
+    th = np.pi * np.arange(n_angles) / n_angles
+    tau0 = x0 * np.cos(th) + y0 * np.sin(th)
+    t = np.arange(n_det) - n_det // 2
+    ref = math.sqrt(2 * math.pi) * s * np.exp(-(t[None, :] - tau0[:, None]) ** 2 / (2 * s * s))
+    assert rel(S, ref) < 1e-10
+    L = oracle.ray_forward(workloads.gaussian_blob(N, x0, y0, s), n_angles, n_det)
+    assert rel(L, ref) < 2e-2
+
+
+# ---------------------------------------------------- C4 disk chord length ----
+def test_c4_disk_chord_length_converges_like_one_over_r():
+    errs_d, errs_r = [], []
+    radii = [6.0, 12.0, 24.0]
+    for r in radii:
+        N = 64
+        n_angles, n_det = 8, 91
+        x0, y0 = 2.5, -1.25
+        img = workloads.single_disk(N, x0, y0, r, 0.8)
+        th = np.pi * np.arange(n_angles) / n_angles
+        tau0 = x0 * np.cos(th) + y0 * np.sin(th)
+        t = np.arange(n_det) - n_det // 2
+        chord = 2 * 0.8 * np.sqrt(np.maximum(r * r - (t[None, :] - tau0[:, None]) ** 2, 0.0))
+        errs_d.append(rel(oracle.forward(img, n_angles, n_det), chord))
+        errs_r.append(rel(oracle.ray_forward(img, n_angles, n_det), chord))
+    for errs in (errs_d, errs_r):
+        for r, e in zip(radii, errs):
+            assert e < 0.5 / r, (r, e)
+        assert errs[2] < 0.6 * errs[0]      # shrinks with radius
+
+
+# ------------------------------------------------------- C5 / C6 / C9 ----
+def test_c5_mass_conservation():
+    x = workloads.make_image(1).astype(np.float64)
+    S = oracle.forward(x, 30, 91)
+    assert np.abs(S.sum(axis=1) - x.sum()).max() < 1e-9 * abs(x.sum())
+
+
+@pytest.mark.parametrize("n_det", [21, 22])
+def test_c6_adjoint_identity(n_det):
+    N, n_angles = 12, 7
+    x = RNG.standard_normal((N, N)); y = RNG.standard_normal((n_angles, n_det))
+    lhs = np.vdot(oracle.forward(x, n_angles, n_det), y)
+    rhs = np.vdot(x, oracle.adjoint(y, N))
+    assert abs(lhs - rhs) < 1e-12 * max(abs(lhs), 1.0)
+
+
+def test_c7_dense_matrix_brute_force_and_transpose():
+    """Build A from the Dirichlet closed form (independent of the C double sum) at
+    N=8; forward == A x, adjoint == A^T y."""
+    N, n_angles, n_det = 8, 6, 11
+    c, cd = N // 2, n_det // 2
+    iy, ix = np.mgrid[0:N, 0:N]
+    A = np.empty((n_angles * n_det, N * N))
+    for a in range(n_angles):
+        th = math.pi * a / n_angles
+        tau = ((ix - c) * math.cos(th) + (iy - c) * math.sin(th)).ravel()
+        for s in range(n_det):
+            A[a * n_det + s] = dirichlet_np((s - cd) - tau, n_det)
+    x = RNG.standard_normal((N, N)); y = RNG.standard_normal((n_angles, n_det))
+    assert np.abs(oracle.forward(x, n_angles, n_det).ravel() - A @ x.ravel()).max() < 1e-12
+    assert np.abs(oracle.adjoint(y, N).ravel() - A.T @ y.ravel()).max() < 1e-12
+
+
+def test_c9_invariances_linearity_shift_and_pi_symmetry():
+    N, n_det = 16, 25
+    x1 = RNG.standard_normal((N, N)); x2 = RNG.standard_normal((N, N))
+    f = lambda x, na=6: oracle.forward(x, na, n_det)
+    assert np.abs(f(2.0 * x1 - 0.5 * x2) - (2.0 * f(x1) - 0.5 * f(x2))).max() < 1e-11
+    # theta -> theta + pi flips the detector: plan with 2*n_angles over [0, 2 pi)
+    S = oracle.forward(x1, 12, n_det)[::2]         # angles 0, pi/3 ... -> need [0,2pi): use 2pi*a/12
+    # angles pi*a/12 for a=0..11 cover [0,pi); emulate theta+pi by rotating the image 180 deg
+    xr = np.zeros_like(x1); xr[1:, 1:] = x1[1:, 1:][::-1, ::-1]   # (X,Y)->(-X,-Y) about c=N/2
+    x1m = x1.copy(); x1m[0, :] = 0; x1m[:, 0] = 0
+    Sa = oracle.forward(x1m, 5, n_det); Sb = oracle.forward(xr, 5, n_det)
+    assert np.abs(Sa - Sb[:, ::-1]).max() < 1e-11   # S_rot[a, s] = S[a, -s] (odd n_det: c_d symmetric)
+
+
+def test_subset_evaluation_is_exact():
+    x = workloads.make_image(1).astype(np.float64)
+    full = oracle.forward(x, 10, 91)
+    idx = RNG.choice(10 * 91, 50, replace=False)
+    assert np.abs(oracle.forward(x, 10, 91, idx=idx) - full.ravel()[idx]).max() < 1e-12
+    y = RNG.standard_normal((10, 91))
+    fa = oracle.adjoint(y, 64)
+    pix = RNG.choice(64 * 64, 40, replace=False)
+    assert np.abs(oracle.adjoint(y, 64, pix=pix) - fa.ravel()[pix]).max() < 1e-12
+
+
+# ------------------------------------------------ O-ray orientation pin ----
+def test_oray_orientation_matches_odirect_on_offcentre_disk():
+    N, n_angles, n_det = 64, 16, 91
+    img = workloads.single_disk(N, 14.0, -9.0, 7.0, 1.0)
+    S = oracle.forward(img, n_angles, n_det); L = oracle.ray_forward(img, n_angles, n_det)
+    assert rel(L, S) < 0.08
+    # peak position follows tau0 = x0 cos + y0 sin for every angle (orientation, centre)
+    th = np.pi * np.arange(n_angles) / n_angles
+    tau0 = 14.0 * np.cos(th) - 9.0 * np.sin(th)
+    for Z in (S, L):
+        com = (Z * (np.arange(n_det) - n_det // 2)[None, :]).sum(1) / Z.sum(1)
+        assert np.abs(com - tau0).max() < 0.05
+
+
+# ------------------------------------------------------ Kaiser-Bessel pins ----
+def test_kb_i0_against_scipy_and_kernel_special_values():
+    for z in (0.0, 0.3, 2.0, 13.8551, 30.0):
+        assert abs(oracle.kb_i0(z) - special.i0(z)) < 1e-13 * special.i0(z)
+    beta = oracle.kb_beta(6, 2.0)
+    assert abs(beta - math.pi * math.sqrt(9 * 2.25 - 0.8)) < 1e-14      # 13.8551...
+    assert abs(beta - 13.8551) < 1e-4
+    assert abs(oracle.kb_phi(0.0) - 1.0) < 1e-15
+    assert abs(oracle.kb_phi(3.0) - 1.0 / special.i0(beta)) < 1e-18
+    assert oracle.kb_phi(3.0000001) == 0.0
+    u = np.linspace(-3, 3, 41)
+    assert np.abs(oracle.kb_phi(u) - oracle.kb_phi(-u)).max() == 0.0
+
+
+def test_kb_fourier_transform_closed_form_against_quadrature():
+    """phihat(xi) closed form == numerical integral of phi(u) cos(2 pi xi u)."""
+    beta = oracle.kb_beta()
+    for xi in (0.0, 0.1, 0.25, 0.5, 0.74, 0.9):       # incl. beyond sqrt: beta/(pi W) = 0.735
+        num, _ = integrate.quad(lambda u: float(oracle.kb_phi(u)) * math.cos(2 * math.pi * xi * u),
+                                -3, 3, epsabs=1e-13, epsrel=1e-13, limit=200)
+        assert abs(num - float(oracle.kb_phihat(xi))) < 1e-10
+
+
+# -------------------------------------------------------------- O-grid pins ----
+def test_ogrid_interp_of_plane_wave_is_deapodised_exponential():
+    """Inverse gridding (eq :87) of G_r[k] = exp(-i 2 pi k.X/G) returns
+    phihat(X/G) phihat(Y/G) exp(-i 2 pi kappa.X/G) up to the aliasing error of the
+    kernel (W=6, sigma=2: ~1e-5 relative for |X| <= G/4): ties tap selection,
+    kernel, centred layout and the de-apodisation formula together."""
+    G, n_angles, n_det = 64, 7, 45
+    k = np.arange(G) - G // 2
+    for (X, Y) in [(0, 0), (5, -3), (-16, 15), (11, 16)]:
+        grid = np.exp(-2j * np.pi * (k[None, :] * X + k[:, None] * Y) / G)
+        P = oracle.grid_interp(grid, n_angles, n_det)
+        th = np.pi * np.arange(n_angles) / n_angles
+        rho = G * (np.arange(n_det) - n_det // 2) / n_det
+        kx = rho[None, :] * np.cos(th)[:, None]; ky = rho[None, :] * np.sin(th)[:, None]
+        hx, hy = float(oracle.kb_phihat(X / G)), float(oracle.kb_phihat(Y / G))
+        ref = hx * hy * np.exp(-2j * np.pi * (kx * X + ky * Y) / G)
+        # Poisson summation: P - ref = sum over aliases phihat(X/G + p), p != 0; for
+        # Kaiser-Bessel W=6, sigma=2, beta=13.855 and |X| <= G/4 that is the method's
+        # design accuracy, ~1e-5 relative (1.03e-5 worst case, corner pixel)
+        err = np.abs(P - ref).max() / abs(hx * hy)
+        assert 1e-8 < err < 3e-5, (X, Y, err)   # 2-D corner: ~2x the 1-D 1.03e-5
+
+
+def test_ogrid_grid_is_transpose_of_interp_and_brute_force():
+    G, n_angles, n_det = 16, 5, 13
+    grid = RNG.standard_normal((G, G)) + 1j * RNG.standard_normal((G, G))
+    P = RNG.standard_normal((n_angles, n_det)) + 1j * RNG.standard_normal((n_angles, n_det))
+    lhs = np.vdot(P, oracle.grid_interp(grid, n_angles, n_det))
+    rhs = np.vdot(oracle.grid_grid(P, G), grid)
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    # brute force with scipy's I0 and an independently written tap loop
+    beta = math.pi * math.sqrt((6 / 2.0) ** 2 * 1.5 ** 2 - 0.8)
+    phi = lambda u: special.i0(beta * math.sqrt(max(1 - (u / 3) ** 2, 0))) / special.i0(beta) if abs(u) <= 3 else 0.0
+    out = np.zeros((n_angles, n_det), dtype=complex)
+    for a in range(n_angles):
+        for kk in range(n_det):
+            rho = G * (kk - n_det // 2) / n_det
+            kx, ky = rho * math.cos(math.pi * a / n_angles), rho * math.sin(math.pi * a / n_angles)
+            for yy in range(math.ceil(ky - 3), math.ceil(ky - 3) + 6):
+                for xx in range(math.ceil(kx - 3), math.ceil(kx - 3) + 6):
+                    out[a, kk] += grid[(yy + G // 2) % G, (xx + G // 2) % G] * phi(xx - kx) * phi(yy - ky)
+    assert np.abs(out - oracle.grid_interp(grid, n_angles, n_det)).max() < 1e-12
+
+
+# ------------------------------ O-alg gated against O-direct (error bound) ----
+def test_fast_algorithm_within_kernel_error_bound_of_exact_operator():
+    """'the exact result within the method's error bound': the fp64 fast algorithm
+    (O-alg) must sit within the KB W=6, sigma=2 aliasing bound of O-direct -- and
+    not far below it (C8: an error << 1e-6 would mean comparing a method with itself)."""
+    x = workloads.make_image(1).astype(np.float64)
+    S = oracle.forward(x, 90, 91)
+    Sf = oracle.fast_forward(x, 90, 91)
+    e = rel(Sf, S)
+    assert 5e-7 < e < 1e-5
+    y = S
+    A = oracle.adjoint(y, 64); Af = oracle.fast_adjoint(y, 64)
+    e = rel(Af, A)
+    assert 5e-7 < e < 1e-5
+    # bare NUFFT on white noise and a corner pixel (gate G2 inputs): <= 1e-4
+    for img in (workloads.white_noise(32, 3), workloads.delta_image(32, 0, 31)):
+        e = rel(oracle.fast_nufft2(img, 16, 45), oracle.ndft2(img.astype(np.float64), 16, 45))
+        assert e < 1e-4
+    # adjointness of the fast pair is exact (W-independent): C6 for O-alg
+    x2 = RNG.standard_normal((64, 64)); y2 = RNG.standard_normal((90, 91))
+    lhs = np.vdot(oracle.fast_forward(x2, 90, 91), y2); rhs = np.vdot(x2, oracle.fast_adjoint(y2, 64))
+    assert abs(lhs - rhs) < 1e-11 * abs(lhs)
