@@ -1,0 +1,167 @@
+/*
+ * radon.h -- C ABI of libradon_b200: the gridding / inverse-gridding (NUFFT)
+ * pair behind the fast Radon transform y = Radon{x} and its adjoint, hand-written
+ * CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Source of the operations: Maia et al., "Compressive Phase Contrast Tomography",
+ * arXiv 1009.1380.  "PAPER.md:NN" cites a line of the reference text.
+ *
+ *   - the solver "requires us to provide a function to perform y = Radon{x}"
+ *     (section I) -> radon_forward; the solver also applies the
+ *     transpose every iteration -> radon_adjoint.
+ *   - "first perform a 2D FFT of x on a regular grid, and then interpolate the
+ *     transform onto a polar grid before 1D inverse Fourier transforms are applied
+ *     to interpolated points along the same radial lines" (section II)
+ *     -> the stages of radon_forward; radon_adjoint runs the transposed stages in
+ *     reverse order.
+ *   - "The gridding operation requires the convolution between irregular samples
+ *     and a kernel calculated at regular sample position and vice versa"
+ *      with the sums printed beside Fig. 5:
+ *       G_i(x_i,y_i) = sum_r G_r(x_r,y_r) K(x_r-x_i, y_r-y_i)
+ *         -> radon_interp_only  (inverse gridding, regular -> polar, a gather)
+ *       G_r(x_r,y_r) = sum_i D G(x_i,y_i) K(x_i-x_r, y_i-y_r)   (D == 1)
+ *         -> radon_grid_only    (gridding, polar -> regular, a scatter)
+ *   - the paper names neither kernel nor oversampling; BASELINE.json north_star
+ *     fixes a Kaiser-Bessel kernel of width W = 6 on a sigma = 2 oversampled grid.
+ *
+ * Conventions (DESIGN.md section 4 lists every reading of the paper):
+ *   image     x[iy*N + ix], fp32, row-major; centred coordinates X = ix - N/2,
+ *             Y = iy - N/2 (integer division).
+ *   sinogram  y[a*n_det + s], fp32, angle-major; theta_a = pi*a/n_angles,
+ *             detector coordinate t = s - n_det/2 = X cos(theta) + Y sin(theta).
+ *   polar     P[a*n_det + k], complex64 stored as interleaved (re, im) floats;
+ *             radial frequency index j = k - n_det/2, sample position on the
+ *             oversampled grid kappa = (G j / n_det)(cos theta_a, sin theta_a).
+ *   grid      g[cy*G + cx], complex64 interleaved, G = sigma*N, CENTRED layout:
+ *             cell (cx, cy) holds frequency (cx - G/2, cy - G/2); indices wrap
+ *             mod G (the DTFT is periodic).
+ *   Operator  S[a,s] = Re{ (1/n) sum_k F[a,k] exp(+i 2 pi j t/n) },
+ *             F[a,k] = sum_pix x exp(-i (2 pi j/n)(X cos + Y sin));
+ *             radon_adjoint is its exact transpose (no density weights, no 1/M).
+ *
+ * Pointers: every d_* argument is a DEVICE pointer owned by the caller (e.g. a
+ * torch tensor's data_ptr()); every h_* argument is a HOST pointer owned by the
+ * caller.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ * Device entry points are asynchronous on `stream`; input and output must not
+ * alias.  A plan owns its tables and workspace, belongs to the CUDA device that
+ * was current at creation, and must not be used from two streams at once.
+ *
+ * Errors: every call returns RADON_OK (0) or a negative code; nothing throws.
+ * There is no CPU fallback and no other backend: on a machine without an sm_100
+ * device radon_plan_create returns RADON_EARCH / RADON_ECUDA.
+ */
+#ifndef RADON_B200_H
+#define RADON_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RADON_OK            0
+#define RADON_EINVAL       -1   /* bad argument (see each call) */
+#define RADON_ENOMEM       -2   /* host or device allocation failed */
+#define RADON_ECUDA        -3   /* a CUDA runtime call failed (radon_last_cuda_error) */
+#define RADON_EARCH        -4   /* current device is not compute capability 10.x */
+#define RADON_EUNSUPPORTED -5   /* valid but not built: W != 6, sigma*N not a power of two */
+
+typedef struct radon_plan radon_plan;   /* opaque, owned by the library */
+
+/* Plan for images N x N, n_angles uniform angles in [0, pi), n_det detector bins,
+ * oversampling sigma (G = sigma*N must be an even integer; this build needs a
+ * power of two, 16 <= G <= 8192) and Kaiser-Bessel width W (this build: 6).
+ * Builds, for the current CUDA device: per-angle fp64 direction table (Fourier
+ * slice geometry), Kaiser-Bessel LUT and de-apodisation vectors,
+ * the conflict-free gather/scatter schedules (the plan-time binning that takes
+ * the place of the paper's load-balanced bins), FFT twiddles and
+ * chirp tables, and the workspace.  EINVAL: N < 8, n_angles < 1, n_det < 2,
+ * n_angles or n_det > 65535, sigma*N not an even integer, W outside [2,12],
+ * out == NULL.  On failure *out is set to NULL. */
+int radon_plan_create(radon_plan **out, int N, int n_angles, int n_det, float sigma, int W);
+
+/* Frees everything the plan owns (synchronises the device first). NULL is OK. */
+int radon_plan_destroy(radon_plan *p);
+
+/* y = Radon{x}.  d_x: N*N fp32.  d_sino: n_angles*n_det fp32. */
+int radon_forward(radon_plan *p, const float *d_x, float *d_sino, void *stream);
+
+/* x~ = Radon^T{y}: exact transpose of radon_forward (PAPER.md:85 with D == 1). */
+int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, void *stream);
+
+/* `batch` contiguous slices sharing the plan (BASELINE.json configs[4]). */
+int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream);
+int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batch, void *stream);
+
+/* Same operators on HOST buffers (pinned or pageable): slices are copied to the
+ * device, transformed and copied back on two internal streams so that the copies
+ * of neighbouring slices overlap the kernels; returns after the last copy has
+ * landed (synchronous).  h_x: batch*N*N fp32, h_sino: batch*n_angles*n_det fp32. */
+int radon_forward_host(radon_plan *p, const float *h_x, float *h_sino, int batch);
+int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x, int batch);
+
+/* Bare NUFFT (type 2): image -> M = n_angles*n_det complex polar samples
+ * F[a,k] (de-apodise + zero-pad, 2-D FFT, inverse gridding).  d_polar: 2*M floats. */
+int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, void *stream);
+/* Its transpose on arbitrary complex polar input; output is the real part
+ * (gridding, 2-D inverse FFT, crop + de-apodise).  d_x: N*N fp32. */
+int radon_nufft1(radon_plan *p, const float *d_polar, float *d_x, void *stream);
+
+/* Inverse gridding alone: d_grid 2*G*G floats (centred layout)
+ * -> d_polar 2*M floats. */
+int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *stream);
+/* Gridding alone (D == 1): d_polar 2*M floats -> d_grid 2*G*G floats;
+ * every cell of d_grid is written exactly once (zeros included), no atomics, and
+ * the result is bit-identical from run to run. */
+int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream);
+
+/* 1-D transforms along the projections alone (last step):
+ * radon_proj_ifft: polar 2*M floats -> sinogram, S = Re{(1/n) sum_k P exp(+i 2 pi j t/n)};
+ * radon_proj_fft:  sinogram -> polar, its transpose Yh = (1/n) sum_s y exp(-i 2 pi j t/n). */
+int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream);
+int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *stream);
+
+/* Any of the out pointers may be NULL.  workspace_bytes = device bytes the plan owns. */
+int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_det,
+                    long long *M, size_t *workspace_bytes);
+
+/* Schedule statistics of a plan (all host data; out pointers may be NULL):
+ * slots = 32 * rounds issued, filled = slots holding a sample, ctas = thread blocks
+ * per launch, for the gather (interp) and the scatter (grid) kernels. */
+int radon_plan_schedule_stats(const radon_plan *p,
+                              long long *gather_slots, long long *gather_filled, int *gather_ctas,
+                              long long *scatter_slots, long long *scatter_filled, int *scatter_ctas);
+
+/* Host-only self-check of the plan-time schedule builder; needs NO GPU.  Builds
+ * the gather and scatter schedules for the geometry and verifies that every
+ * sample is issued exactly once by the gather, that the scatter issues every
+ * (sample, wrap image, output rectangle) incidence exactly once, that no two
+ * samples issued to one warp in the same round have overlapping W x W footprints
+ * (write-conflict freedom without atomics) and that the 16 lanes of every
+ * half-warp start in distinct shared-memory bank pairs.  Returns RADON_OK or
+ * RADON_EINVAL; *n_violations (may be NULL) receives the number of violations. */
+int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W,
+                             long long *n_violations);
+
+/* Host-only statistics of the schedules for a geometry (no GPU, no plan needed):
+ * out[0..9] = gather slots, gather filled, gather CTAs, max gather rounds per CTA,
+ * scatter slots, scatter filled, scatter CTAs, max scatter rounds per warp,
+ * merge jobs, partial rectangles. */
+int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, long long out[10]);
+
+/* Host-only evaluation of the W Kaiser-Bessel tap weights exactly as the kernels compute
+ * them (plan-time polynomial pieces, fp32 Horner): w[l] = phi(delta - W/2 + l), l = 0..W-1,
+ * for the fractional offset delta in [0,1].  Needs no GPU; used by the CPU unit tests. */
+int radon_kb_weights_host(int W, float sigma, float delta, float *w);
+
+/* Number of kernels the library has launched in this process (monotonic). */
+long long radon_kernel_launch_count(void);
+
+const char *radon_strerror(int code);
+/* Text of the last CUDA error seen by this library on the calling thread. */
+const char *radon_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RADON_B200_H */

@@ -10,8 +10,11 @@ Functions (each cites the passage it follows; details in radon_oracle.c):
   (SURVEY.md 8(c) items 1-3).  ``idx`` / ``pix`` evaluate a subset
   of outputs (each output is an independent sum, so a subset is exact).
 * ``ndft2`` / ``ndft1``          bare non-uniform DFT and its conjugate transpose.
-* ``dirichlet_forward``          closed form of the same operator (second,
-  independent implementation used by the pins).
+* ``dirichlet_forward`` / ``dirichlet_forward_subset`` / ``dirichlet_adjoint``
+  closed form of the same operator (periodic-sinc detector response): the second,
+  independent implementation used by the pins, and -- because one output costs N^2
+  (forward) or M (adjoint) terms instead of a whole radial line -- the form used for
+  sampled outputs at BASELINE.json's full sizes.
 * ``ray_forward``                O-ray, ray-sampled line integral (north_star).
 * ``kb_*``, ``grid_interp``, ``grid_grid``  O-grid: the two sums printed with
   Fig. 5 with a directly evaluated Kaiser-Bessel kernel.
@@ -49,6 +52,8 @@ def _load():
         lib.odirect_forward.argtypes = [D, I, I, I, L, LL, D]
         lib.odirect_adjoint.argtypes = [D, I, I, I, L, LL, D]
         lib.odirichlet_forward.argtypes = [D, I, I, I, D]
+        lib.odirichlet_forward_subset.argtypes = [D, I, I, I, L, LL, D]
+        lib.odirichlet_adjoint.argtypes = [D, I, I, I, L, LL, D]
         lib.oray_forward.argtypes = [D, I, I, I, DBL, D]
         lib.okb_i0.argtypes = [DBL]; lib.okb_i0.restype = DBL
         lib.okb_beta.argtypes = [I, DBL]; lib.okb_beta.restype = DBL
@@ -149,6 +154,28 @@ def dirichlet_forward(x, n_angles, n_det):
     S = np.empty((n_angles, n_det))
     lib.odirichlet_forward(_d(x), x.shape[0], n_angles, n_det, _d(S))
     return S
+
+
+def dirichlet_forward_subset(x, n_angles, n_det, idx):
+    """Listed sinogram entries q = a*n_det + s by the closed form (N^2 terms each)."""
+    lib = _load()
+    x = _f64(x)
+    idx, n_idx = _idx(idx)
+    S = np.empty(n_idx)
+    lib.odirichlet_forward_subset(_d(x), x.shape[0], n_angles, n_det, _l(idx), n_idx, _d(S))
+    return S
+
+
+def dirichlet_adjoint(y, N, pix=None):
+    """Transpose by the closed form; listed pixels p = iy*N + ix (None: all), M terms each."""
+    lib = _load()
+    y = _f64(y)
+    n_angles, n_det = y.shape
+    pix, n_pix = _idx(pix)
+    cnt = n_pix if pix is not None else N * N
+    xt = np.empty(cnt)
+    lib.odirichlet_adjoint(_d(y), N, n_angles, n_det, _l(pix), n_pix, _d(xt))
+    return xt if pix is not None else xt.reshape(N, N)
 
 
 def ray_forward(x, n_angles, n_det, h=0.25):

@@ -271,6 +271,52 @@ void odirichlet_forward(const double *x, int N, int n_angles, int n_det, double 
     }
 }
 
+/* Closed-form evaluation of listed outputs only (used at BASELINE.json's full  */
+/* sizes, where the double sum of odirect_forward needs a whole radial line    */
+/* -- n_det * N^2 terms -- per sampled angle): N^2 terms per listed entry.      */
+void odirichlet_forward_subset(const double *x, int N, int n_angles, int n_det,
+                               const long long *idx, long long n_idx, double *S)
+{
+    const int c = N / 2, cd = n_det / 2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long long q = 0; q < n_idx; ++q) {
+        const int a = (int)(idx[q] / n_det), s = (int)(idx[q] % n_det);
+        const double theta = M_PI * (double)a / (double)n_angles;
+        const double ct = cos(theta), st = sin(theta), t = (double)(s - cd);
+        double acc = 0.0;
+        for (int iy = 0; iy < N; ++iy)
+            for (int ix = 0; ix < N; ++ix) {
+                const double v = x[(size_t)iy * N + ix];
+                if (v != 0.0) acc += v * dirichlet(t - ((ix - c) * ct + (iy - c) * st), n_det);
+            }
+        S[q] = acc;
+    }
+}
+
+/* Transpose in closed form: x~[pix] = sum_{a,s} y[a,s] D_n(t_s - tau_a(pix)),  */
+/* M terms per listed pixel (pix == NULL: all pixels).                          */
+void odirichlet_adjoint(const double *y, int N, int n_angles, int n_det,
+                        const long long *pix, long long n_pix, double *xt)
+{
+    const int c = N / 2, cd = n_det / 2;
+    const long long cnt = pix ? n_pix : (long long)N * N;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long long q = 0; q < cnt; ++q) {
+        const long long p = pix ? pix[q] : q;
+        const double X = (double)((int)(p % N) - c), Y = (double)((int)(p / N) - c);
+        double acc = 0.0;
+        for (int a = 0; a < n_angles; ++a) {
+            const double theta = M_PI * (double)a / (double)n_angles;
+            const double tau = X * cos(theta) + Y * sin(theta);
+            for (int s = 0; s < n_det; ++s) {
+                const double v = y[(size_t)a * n_det + s];
+                if (v != 0.0) acc += v * dirichlet((double)(s - cd) - tau, n_det);
+            }
+        }
+        xt[q] = acc;
+    }
+}
+
 /* ------------------------------------------------------------------------- */
 /* O-ray (north_star; SURVEY 8(c) "O-ray"): line integral by ray sampling.    */
 /*   L[a,s] = h sum_q bilinear(x; c + t cos - u_q sin, c + t sin + u_q cos),  */

@@ -1,0 +1,445 @@
+// api.cu -- the C ABI of libradon_b200 (include/radon.h): plan life cycle and the stage
+// sequences of radon_forward / radon_adjoint.  No torch types, no exceptions across the ABI.
+#include "../../include/radon.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "kernels.h"
+
+using namespace radon;
+
+static thread_local std::string g_last_cuda_error;
+
+#define CUDA_TRY(expr)                                                                 \
+    do {                                                                               \
+        cudaError_t e__ = (expr);                                                      \
+        if (e__ != cudaSuccess) {                                                      \
+            g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(e__);   \
+            return RADON_ECUDA;                                                        \
+        }                                                                              \
+    } while (0)
+
+struct Workspace {
+    float2 *T = nullptr;       // G x N intermediate of the 2-D FFT
+    float2 *grid = nullptr;    // G x G oversampled spectrum (centred)
+    float2 *polar = nullptr;   // M polar samples
+    float *img = nullptr;      // N x N   (host-buffer entry points only)
+    float *sino = nullptr;     // M       (host-buffer entry points only)
+};
+
+struct radon_plan {
+    Geometry geo;
+    DevicePlan dev;
+    Workspace ws[2];
+    long long M = 0;
+    size_t device_bytes = 0;
+    long long gather_slots = 0, gather_filled = 0, scatter_slots = 0, scatter_filled = 0;
+    cudaStream_t hstream[2] = {nullptr, nullptr};
+    cudaEvent_t hevent[2] = {nullptr, nullptr};
+};
+
+template <typename T>
+static int dev_alloc(radon_plan *p, T **ptr, size_t count)
+{
+    *ptr = nullptr;
+    if (count == 0) return RADON_OK;
+    cudaError_t e = cudaMalloc((void **)ptr, count * sizeof(T));
+    if (e != cudaSuccess) {
+        g_last_cuda_error = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+        return e == cudaErrorMemoryAllocation ? RADON_ENOMEM : RADON_ECUDA;
+    }
+    p->device_bytes += count * sizeof(T);
+    return RADON_OK;
+}
+
+template <typename T, typename H>
+static int dev_upload(radon_plan *p, T **ptr, const std::vector<H> &host)
+{
+    static_assert(sizeof(T) % sizeof(H) == 0 || sizeof(H) % sizeof(T) == 0, "layout");
+    const size_t bytes = host.size() * sizeof(H);
+    int rc = dev_alloc(p, (unsigned char **)ptr, bytes);
+    if (rc) return rc;
+    if (bytes) CUDA_TRY(cudaMemcpy(*ptr, host.data(), bytes, cudaMemcpyHostToDevice));
+    return RADON_OK;
+}
+
+static int validate(int N, int n_angles, int n_det, float sigma, int W, int *G_out)
+{
+    if (N < 8 || n_angles < 1 || n_det < 2 || n_angles > 65535 || n_det > 65535) return RADON_EINVAL;
+    if (W < 2 || W > 12) return RADON_EINVAL;
+    if (!(sigma > 1.0f) || sigma > 8.0f) return RADON_EINVAL;
+    const double g = (double)sigma * N;
+    const long long G = llround(g);
+    if (fabs(g - (double)G) > 1e-6 || (G & 1)) return RADON_EINVAL;
+    if (W != KW) return RADON_EUNSUPPORTED;
+    if (!fft_length_supported((int)G)) return RADON_EUNSUPPORTED;
+    if (2 * (long long)n_det - 1 > 8192) return RADON_EUNSUPPORTED;
+    *G_out = (int)G;
+    return RADON_OK;
+}
+
+extern "C" int radon_plan_destroy(radon_plan *p)
+{
+    if (!p) return RADON_OK;
+    cudaDeviceSynchronize();
+    DevicePlan &d = p->dev;
+    cudaFree(d.cs); cudaFree(d.lut); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
+    cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
+    cudaFree(d.gather_ctas); cudaFree(d.gather_slots); cudaFree(d.scatter_ctas); cudaFree(d.scatter_slots);
+    cudaFree(d.merge_jobs); cudaFree(d.scratch);
+    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.img); cudaFree(w.sino); }
+    for (int i = 0; i < 2; ++i) {
+        if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
+        if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
+    }
+    delete p;
+    return RADON_OK;
+}
+
+static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float sigma, int W, int G)
+{
+    int devid = 0;
+    CUDA_TRY(cudaGetDevice(&devid));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, devid));
+    if (prop.major != 10) return RADON_EARCH;          // sm_100a only: no other backend
+    if (init_kernel_attributes()) { g_last_cuda_error = "cudaFuncSetAttribute(max dynamic smem)"; return RADON_ECUDA; }
+
+    p->geo.init(N, n_angles, n_det, (double)sigma, W);
+    p->M = (long long)n_angles * n_det;
+    DevicePlan &d = p->dev;
+    d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det;
+    const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
+    d.LP = pow2 ? n_det : std::max(16, next_pow2(2 * n_det - 1));
+
+    int rc;
+    // P1: Fourier-slice directions, fp64
+    if ((rc = dev_upload(p, &d.cs, p->geo.cs))) return rc;
+    // P2: Kaiser-Bessel LUT, de-apodisation
+    std::vector<float> lut, deapod, tw, ca, cb, hf;
+    build_kb_poly(W, sigma, d.kb);
+    build_deapod(N, G, W, sigma, deapod);
+#if RADON_KB_LUT
+    build_kb_lut(W, sigma, lut);
+    if ((rc = dev_upload(p, &d.lut, lut))) return rc;
+#endif
+    if ((rc = dev_upload(p, &d.deapod, deapod))) return rc;
+    build_twiddles(G, tw);
+    if ((rc = dev_upload(p, &d.tw_G, tw))) return rc;
+    build_twiddles(d.LP, tw);
+    if ((rc = dev_upload(p, &d.tw_P, tw))) return rc;
+    build_chirp(n_det, d.LP, ca, cb, hf);
+    if ((rc = dev_upload(p, &d.chirp_a, ca))) return rc;
+    if ((rc = dev_upload(p, &d.chirp_b, cb))) return rc;
+    if (!hf.empty() && (rc = dev_upload(p, &d.chirp_hf, hf))) return rc;
+    // P3: schedules
+    Schedules sch;
+    build_schedules(p->geo, sch);
+    p->gather_slots = (long long)sch.gather_slots.size(); p->gather_filled = sch.gather_filled;
+    p->scatter_slots = (long long)sch.scatter_slots.size(); p->scatter_filled = sch.scatter_filled;
+    d.n_gather_ctas = (int)sch.gather_ctas.size();
+    d.n_scatter_ctas = (int)sch.scatter_ctas.size();
+    d.n_merge_jobs = (int)sch.merge_jobs.size();
+    if ((rc = dev_upload(p, &d.gather_ctas, sch.gather_ctas))) return rc;
+    if ((rc = dev_upload(p, &d.gather_slots, sch.gather_slots))) return rc;
+    if ((rc = dev_upload(p, &d.scatter_ctas, sch.scatter_ctas))) return rc;
+    if ((rc = dev_upload(p, &d.scatter_slots, sch.scatter_slots))) return rc;
+    if ((rc = dev_upload(p, &d.merge_jobs, sch.merge_jobs))) return rc;
+    if ((rc = dev_alloc(p, &d.scratch, (size_t)sch.n_partial_slots * ST_X * ST_Y))) return rc;
+    // workspace (two sets: the host-buffer entry points overlap copies with kernels)
+    for (auto &w : p->ws) {
+        if ((rc = dev_alloc(p, &w.T, (size_t)G * N))) return rc;
+        if ((rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
+        if ((rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
+    }
+    return RADON_OK;
+}
+
+extern "C" int radon_plan_create(radon_plan **out, int N, int n_angles, int n_det, float sigma, int W)
+{
+    if (!out) return RADON_EINVAL;
+    *out = nullptr;
+    int G = 0;
+    int rc = validate(N, n_angles, n_det, sigma, W, &G);
+    if (rc) return rc;
+    radon_plan *p = new (std::nothrow) radon_plan();
+    if (!p) return RADON_ENOMEM;
+    try {
+        rc = plan_create_impl(p, N, n_angles, n_det, sigma, W, G);
+    } catch (const std::bad_alloc &) {
+        rc = RADON_ENOMEM;
+    } catch (...) {
+        rc = RADON_EINVAL;
+    }
+    if (rc) { radon_plan_destroy(p); return rc; }
+    *out = p;
+    return RADON_OK;
+}
+
+static int check_launch()
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        g_last_cuda_error = std::string("kernel launch: ") + cudaGetErrorString(e);
+        return RADON_ECUDA;
+    }
+    return RADON_OK;
+}
+
+// ---- stage sequences ------------------------------------------------------------------
+static int nufft2_ws(radon_plan *p, Workspace &w, const float *d_x, float2 *d_polar, cudaStream_t st)
+{
+    if (launch_fft2d_pass(0, p->dev, d_x, w.T, st)) return RADON_ECUDA;        // F1 + F2 (columns)
+    if (launch_fft2d_pass(1, p->dev, w.T, w.grid, st)) return RADON_ECUDA;     // F2 (rows)
+    if (launch_gather(p->dev, w.grid, d_polar, st)) return RADON_ECUDA;        // F3
+    return check_launch();
+}
+
+static int nufft1_ws(radon_plan *p, Workspace &w, const float2 *d_polar, float *d_x, cudaStream_t st)
+{
+    if (launch_scatter(p->dev, d_polar, w.grid, st)) return RADON_ECUDA;       // A2
+    if (launch_fft2d_pass(2, p->dev, w.grid, w.T, st)) return RADON_ECUDA;     // A3 (rows)
+    if (launch_fft2d_pass(3, p->dev, w.T, d_x, st)) return RADON_ECUDA;        // A3 (columns) + A4
+    return check_launch();
+}
+
+static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_sino, cudaStream_t st)
+{
+    int rc = nufft2_ws(p, w, d_x, w.polar, st);
+    if (rc) return rc;
+    if (launch_proj(true, p->dev, (const float *)w.polar, d_sino, st)) return RADON_ECUDA;   // F4
+    return check_launch();
+}
+
+static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st)
+{
+    if (launch_proj(false, p->dev, d_sino, (float *)w.polar, st)) return RADON_ECUDA;        // A1
+    int rc = check_launch();
+    if (rc) return rc;
+    return nufft1_ws(p, w, w.polar, d_x, st);
+}
+
+extern "C" int radon_forward(radon_plan *p, const float *d_x, float *d_sino, void *stream)
+{
+    if (!p || !d_x || !d_sino) return RADON_EINVAL;
+    return forward_ws(p, p->ws[0], d_x, d_sino, (cudaStream_t)stream);
+}
+
+extern "C" int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, void *stream)
+{
+    if (!p || !d_x || !d_sino) return RADON_EINVAL;
+    return adjoint_ws(p, p->ws[0], d_sino, d_x, (cudaStream_t)stream);
+}
+
+extern "C" int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream)
+{
+    if (!p || !d_x || !d_sino || batch < 0) return RADON_EINVAL;
+    const size_t nx = (size_t)p->dev.N * p->dev.N;
+    for (int b = 0; b < batch; ++b) {
+        int rc = forward_ws(p, p->ws[0], d_x + b * nx, d_sino + (size_t)b * p->M, (cudaStream_t)stream);
+        if (rc) return rc;
+    }
+    return RADON_OK;
+}
+
+extern "C" int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batch, void *stream)
+{
+    if (!p || !d_x || !d_sino || batch < 0) return RADON_EINVAL;
+    const size_t nx = (size_t)p->dev.N * p->dev.N;
+    for (int b = 0; b < batch; ++b) {
+        int rc = adjoint_ws(p, p->ws[0], d_sino + (size_t)b * p->M, d_x + b * nx, (cudaStream_t)stream);
+        if (rc) return rc;
+    }
+    return RADON_OK;
+}
+
+// ---- host-buffer entry points: two streams, copies of slice b+1 overlap kernels of slice b
+static int host_setup(radon_plan *p)
+{
+    for (int i = 0; i < 2; ++i) {
+        if (!p->hstream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
+        if (!p->hevent[i]) CUDA_TRY(cudaEventCreateWithFlags(&p->hevent[i], cudaEventDisableTiming));
+        int rc;
+        if (!p->ws[i].img && (rc = dev_alloc(p, &p->ws[i].img, (size_t)p->dev.N * p->dev.N))) return rc;
+        if (!p->ws[i].sino && (rc = dev_alloc(p, &p->ws[i].sino, (size_t)p->M))) return rc;
+    }
+    return RADON_OK;
+}
+
+static int host_run(radon_plan *p, bool fwd, const float *h_in, float *h_out, int batch)
+{
+    if (!p || !h_in || !h_out || batch < 0) return RADON_EINVAL;
+    int rc = host_setup(p);
+    if (rc) return rc;
+    const size_t nx = (size_t)p->dev.N * p->dev.N, ns = (size_t)p->M;
+    const size_t n_in = fwd ? nx : ns, n_out = fwd ? ns : nx;
+    for (int b = 0; b < batch; ++b) {
+        const int i = b & 1;
+        cudaStream_t st = p->hstream[i];
+        Workspace &w = p->ws[i];
+        float *d_in = fwd ? w.img : w.sino, *d_out = fwd ? w.sino : w.img;
+        CUDA_TRY(cudaMemcpyAsync(d_in, h_in + b * n_in, n_in * sizeof(float), cudaMemcpyHostToDevice, st));
+        rc = fwd ? forward_ws(p, w, d_in, d_out, st) : adjoint_ws(p, w, d_in, d_out, st);
+        if (rc) return rc;
+        CUDA_TRY(cudaMemcpyAsync(h_out + b * n_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
+    CUDA_TRY(cudaStreamSynchronize(p->hstream[0]));
+    CUDA_TRY(cudaStreamSynchronize(p->hstream[1]));
+    return RADON_OK;
+}
+
+extern "C" int radon_forward_host(radon_plan *p, const float *h_x, float *h_sino, int batch)
+{
+    return host_run(p, true, h_x, h_sino, batch);
+}
+
+extern "C" int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x, int batch)
+{
+    return host_run(p, false, h_sino, h_x, batch);
+}
+
+// ---- test / measurement hooks ---------------------------------------------------------
+extern "C" int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, void *stream)
+{
+    if (!p || !d_x || !d_polar) return RADON_EINVAL;
+    return nufft2_ws(p, p->ws[0], d_x, (float2 *)d_polar, (cudaStream_t)stream);
+}
+
+extern "C" int radon_nufft1(radon_plan *p, const float *d_polar, float *d_x, void *stream)
+{
+    if (!p || !d_x || !d_polar) return RADON_EINVAL;
+    return nufft1_ws(p, p->ws[0], (const float2 *)d_polar, d_x, (cudaStream_t)stream);
+}
+
+extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *stream)
+{
+    if (!p || !d_grid || !d_polar) return RADON_EINVAL;
+    if (launch_gather(p->dev, (const float2 *)d_grid, (float2 *)d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
+{
+    if (!p || !d_grid || !d_polar) return RADON_EINVAL;
+    if (launch_scatter(p->dev, (const float2 *)d_polar, (float2 *)d_grid, (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+extern "C" int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream)
+{
+    if (!p || !d_polar || !d_sino) return RADON_EINVAL;
+    if (launch_proj(true, p->dev, d_polar, d_sino, (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+extern "C" int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *stream)
+{
+    if (!p || !d_polar || !d_sino) return RADON_EINVAL;
+    if (launch_proj(false, p->dev, d_sino, d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+extern "C" int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_det,
+                               long long *M, size_t *workspace_bytes)
+{
+    if (!p) return RADON_EINVAL;
+    if (N) *N = p->dev.N;
+    if (G) *G = p->dev.G;
+    if (n_angles) *n_angles = p->dev.n_angles;
+    if (n_det) *n_det = p->dev.n_det;
+    if (M) *M = p->M;
+    if (workspace_bytes) *workspace_bytes = p->device_bytes;
+    return RADON_OK;
+}
+
+extern "C" int radon_plan_schedule_stats(const radon_plan *p,
+                                         long long *gather_slots, long long *gather_filled, int *gather_ctas,
+                                         long long *scatter_slots, long long *scatter_filled, int *scatter_ctas)
+{
+    if (!p) return RADON_EINVAL;
+    if (gather_slots) *gather_slots = p->gather_slots;
+    if (gather_filled) *gather_filled = p->gather_filled;
+    if (gather_ctas) *gather_ctas = p->dev.n_gather_ctas;
+    if (scatter_slots) *scatter_slots = p->scatter_slots;
+    if (scatter_filled) *scatter_filled = p->scatter_filled;
+    if (scatter_ctas) *scatter_ctas = p->dev.n_scatter_ctas;
+    return RADON_OK;
+}
+
+extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W,
+                                        long long *n_violations)
+{
+    if (n_violations) *n_violations = -1;
+    int G = 0;
+    int rc = validate(N, n_angles, n_det, sigma, W, &G);
+    if (rc) return rc;
+    try {
+        Geometry geo;
+        geo.init(N, n_angles, n_det, (double)sigma, W);
+        Schedules sch;
+        build_schedules(geo, sch);
+        const long long bad = check_schedules(geo, sch);
+        if (n_violations) *n_violations = bad;
+        return bad == 0 ? RADON_OK : RADON_EINVAL;
+    } catch (...) {
+        return RADON_ENOMEM;
+    }
+}
+
+extern "C" int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, long long out[10])
+{
+    if (!out) return RADON_EINVAL;
+    int G = 0;
+    int rc = validate(N, n_angles, n_det, sigma, W, &G);
+    if (rc) return rc;
+    try {
+        Geometry geo;
+        geo.init(N, n_angles, n_det, (double)sigma, W);
+        Schedules sch;
+        build_schedules(geo, sch);
+        long long mg = 0, ms = 0;
+        for (const auto &c : sch.gather_ctas) mg = std::max<long long>(mg, c.round_count);
+        for (const auto &c : sch.scatter_ctas)
+            for (const auto &it : c.items) ms = std::max<long long>(ms, it.round_count);
+        out[0] = (long long)sch.gather_slots.size(); out[1] = sch.gather_filled;
+        out[2] = (long long)sch.gather_ctas.size(); out[3] = mg;
+        out[4] = (long long)sch.scatter_slots.size(); out[5] = sch.scatter_filled;
+        out[6] = (long long)sch.scatter_ctas.size(); out[7] = ms;
+        out[8] = (long long)sch.merge_jobs.size(); out[9] = sch.n_partial_slots;
+        return RADON_OK;
+    } catch (...) {
+        return RADON_ENOMEM;
+    }
+}
+
+extern "C" int radon_kb_weights_host(int W, float sigma, float delta, float *w)
+{
+    if (!w || W < 2 || W > 12 || !(sigma > 1.0f) || !(delta >= 0.f && delta <= 1.f)) return RADON_EINVAL;
+    if (W != KW) return RADON_EUNSUPPORTED;
+    KbPoly kp;
+    build_kb_poly(W, sigma, kp);
+    float tmp[KW];
+    kb_poly_weights(kp, delta, tmp);
+    for (int l = 0; l < KW; ++l) w[l] = tmp[l];
+    return RADON_OK;
+}
+
+extern "C" long long radon_kernel_launch_count(void) { return launch_count(); }
+
+extern "C" const char *radon_strerror(int code)
+{
+    switch (code) {
+    case RADON_OK: return "ok";
+    case RADON_EINVAL: return "invalid argument";
+    case RADON_ENOMEM: return "out of memory";
+    case RADON_ECUDA: return "CUDA runtime error (see radon_last_cuda_error)";
+    case RADON_EARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
+    case RADON_EUNSUPPORTED: return "valid request outside this build (W != 6, or sigma*N not a power of two in [16, 8192], or 2*n_det-1 > 8192)";
+    default: return "unknown error";
+    }
+}
+
+extern "C" const char *radon_last_cuda_error(void) { return g_last_cuda_error.c_str(); }

@@ -1,0 +1,633 @@
+// plan_host.cpp -- host side of radon_plan_create: Fourier-slice geometry, tables and
+// the plan-time gather / scatter schedules.  Pure C++ (no CUDA calls) so that it can be
+// exercised on a machine without a GPU (radon_schedule_selfcheck).
+//
+// The schedules take the place of the paper's load-balanced bins ("recursively divides
+// the most computationally intensive bin into four"): the geometry of a plan
+// is fixed, so every decision the paper's kernels take at run time (which block owns which
+// samples, in which order they accumulate) is taken here once:
+//   * samples are binned into grid tiles by a counting sort;
+//   * inside a tile they are packed into ROUNDS of 32 (one per lane of a warp) such that
+//       - the 16 lanes of each half-warp start in 16 distinct shared-memory bank pairs, so
+//         every 64-bit tap access of the round is conflict free (all lanes add the same
+//         tap offset to their base), and
+//       - (scatter only) no two footprints of a round overlap, so the warp can accumulate
+//         with plain load/add/store into its private accumulator: no atomics, and the order
+//         of every floating-point addition is fixed -> bitwise reproducible;
+//   * tiles whose sample count (polar sampling is ~1/r dense: PAPER.md:57's imbalance) would
+//     make one block run long are split over several warps / blocks by dealing their samples
+//     round-robin; partial rectangles are summed in a fixed order by a merge kernel.
+#include "radon_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+namespace radon {
+
+static const double kPi = 3.14159265358979323846264338327950288;
+
+int next_pow2(int v)
+{
+    int p = 1;
+    while (p < v) p <<= 1;
+    return p;
+}
+
+// ---------------------------------------------------------------- geometry -------
+void Geometry::init(int N_, int n_angles_, int n_det_, double sigma_, int W_)
+{
+    N = N_; n_angles = n_angles_; n_det = n_det_; sigma = sigma_; W = W_;
+    G = (int)std::llround(sigma * N);
+    cs.resize(2 * (size_t)n_angles);
+    const double scale = (double)G / (double)n_det;
+    for (int a = 0; a < n_angles; ++a) {
+        double c, s;
+        if (2 * a == n_angles) { c = 0.0; s = 1.0; }         // theta = pi/2 exactly
+        else {
+            const double th = kPi * (double)a / (double)n_angles;
+            c = std::cos(th); s = std::sin(th);
+        }
+        cs[2 * a] = scale * c;
+        cs[2 * a + 1] = scale * s;
+    }
+}
+
+void Geometry::base(int a, int k, int &x0, int &y0) const
+{
+    const double jj = (double)(k - n_det / 2);
+    const double half = 0.5 * (double)G, hw = 0.5 * (double)W;
+    const double gx = std::fma(jj, cs[2 * a], half);
+    const double gy = std::fma(jj, cs[2 * a + 1], half);
+    x0 = (int)std::ceil(gx - hw);
+    y0 = (int)std::ceil(gy - hw);
+}
+
+// ---------------------------------------------------------------- tables ---------
+double kb_i0(double z)
+{
+    const double q = 0.25 * z * z;
+    double term = 1.0, sum = 1.0;
+    for (int m = 1; m < 1000; ++m) {
+        term *= q / ((double)m * (double)m);
+        sum += term;
+        if (term < 1e-18 * sum) break;
+    }
+    return sum;
+}
+
+double kb_beta(int W, double sigma)
+{
+    const double r = (double)W / sigma * (sigma - 0.5);
+    return kPi * std::sqrt(r * r - 0.8);
+}
+
+static double kb_phi(double u, int W, double beta, double inv_i0b)
+{
+    const double t = 2.0 * u / (double)W;
+    const double arg = 1.0 - t * t;
+    if (arg < 0.0) return (arg > -1e-12) ? inv_i0b : 0.0;   // |u| == W/2 up to rounding
+    return kb_i0(beta * std::sqrt(arg)) * inv_i0b;
+}
+
+void build_kb_lut(int W, double sigma, std::vector<float> &lut)
+{
+    const double beta = kb_beta(W, sigma), inv = 1.0 / kb_i0(beta);
+    lut.assign((size_t)LUT_S * 2 * W, 0.f);
+    for (int r = 0; r < LUT_S; ++r)
+        for (int l = 0; l < W; ++l) {
+            const double u0 = (double)r / LUT_S - 0.5 * W + l;
+            const double u1 = (double)(r + 1) / LUT_S - 0.5 * W + l;
+            const double v0 = kb_phi(u0, W, beta, inv), v1 = kb_phi(u1, W, beta, inv);
+            lut[((size_t)r * W + l) * 2 + 0] = (float)v0;
+            lut[((size_t)r * W + l) * 2 + 1] = (float)(v1 - v0);
+        }
+}
+
+// Polynomial pieces of the kernel: for tap l (l < W/2) and delta in [0,1), z = 2 delta - 1,
+//   phi(delta - W/2 + l) = p_l(z),  phi(delta - W/2 + (W-1-l)) = p_l(-z)   (phi is even).
+// p_l is the degree-KB_DEG truncation of the Chebyshev series of phi on the piece (64-node
+// discrete cosine transform in fp64), converted to the monomial basis and split into even
+// and odd parts.
+void build_kb_poly(int W, double sigma, KbPoly &kp)
+{
+    const double beta = kb_beta(W, sigma), inv = 1.0 / kb_i0(beta);
+    const int NN = 64, D = KB_DEG;
+    for (int l = 0; l < W / 2; ++l) {
+        double f[NN], c[D + 1];
+        for (int i = 0; i < NN; ++i) {
+            const double z = std::cos(kPi * (i + 0.5) / NN);
+            f[i] = kb_phi(0.5 * (z + 1.0) - 0.5 * W + l, W, beta, inv);
+        }
+        for (int k = 0; k <= D; ++k) {
+            double acc = 0.0;
+            for (int i = 0; i < NN; ++i) acc += f[i] * std::cos(kPi * k * (i + 0.5) / NN);
+            c[k] = (k == 0 ? 1.0 : 2.0) * acc / NN;
+        }
+        // Chebyshev -> monomial: T_0 = 1, T_1 = z, T_{k+1} = 2 z T_k - T_{k-1}
+        double mono[D + 1] = {0}, t0[D + 1] = {0}, t1[D + 1] = {0}, t2[D + 1];
+        t0[0] = 1.0; t1[1] = 1.0;
+        for (int i = 0; i <= D; ++i) mono[i] += c[0] * t0[i] + c[1] * t1[i];
+        for (int k = 2; k <= D; ++k) {
+            for (int i = 0; i <= D; ++i) t2[i] = (i > 0 ? 2.0 * t1[i - 1] : 0.0) - t0[i];
+            for (int i = 0; i <= D; ++i) { mono[i] += c[k] * t2[i]; t0[i] = t1[i]; t1[i] = t2[i]; }
+        }
+        for (int h = 0; h < KB_HALF; ++h) {
+            kp.e[l][h] = (float)mono[2 * h];
+            kp.o[l][h] = (2 * h + 1 <= D) ? (float)mono[2 * h + 1] : 0.f;
+        }
+    }
+}
+
+void build_deapod(int N, int G, int W, double sigma, std::vector<float> &d)
+{
+    const double beta = kb_beta(W, sigma), scale = (double)W / kb_i0(beta);
+    d.resize(N);
+    for (int i = 0; i < N; ++i) {
+        const double xi = (double)(i - N / 2) / (double)G;
+        const double a = kPi * W * xi, r = beta * beta - a * a;
+        double ph;
+        if (r > 0) { const double q = std::sqrt(r); ph = scale * std::sinh(q) / q; }
+        else if (r < 0) { const double q = std::sqrt(-r); ph = scale * std::sin(q) / q; }
+        else ph = scale;
+        d[i] = (float)(1.0 / ph);
+    }
+}
+
+void build_twiddles(int L, std::vector<float> &tw)
+{
+    tw.resize(2 * (size_t)L);
+    for (int q = 0; q < L; ++q) {
+        const double ang = 2.0 * kPi * (double)q / (double)L;
+        tw[2 * q] = (float)std::cos(ang);
+        tw[2 * q + 1] = (float)(-std::sin(ang));
+    }
+}
+
+// iterative radix-2 FFT in double (plan time only; L is a power of two)
+static void host_fft(std::vector<double> &re, std::vector<double> &im)
+{
+    const int L = (int)re.size();
+    for (int i = 1, j = 0; i < L; ++i) {
+        int bit = L >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { std::swap(re[i], re[j]); std::swap(im[i], im[j]); }
+    }
+    for (int len = 2; len <= L; len <<= 1) {
+        for (int i = 0; i < L; i += len)
+            for (int k = 0; k < len / 2; ++k) {
+                const double ang = -2.0 * kPi * (double)k / (double)len;
+                const double wr = std::cos(ang), wi = std::sin(ang);
+                const int p = i + k, q = p + len / 2;
+                const double tr = re[q] * wr - im[q] * wi, ti = re[q] * wi + im[q] * wr;
+                re[q] = re[p] - tr; im[q] = im[p] - ti;
+                re[p] += tr; im[p] += ti;
+            }
+    }
+}
+
+static inline long long posmod(long long v, long long m)
+{
+    long long r = v % m;
+    return r < 0 ? r + m : r;
+}
+
+void build_chirp(int n, int L, std::vector<float> &a, std::vector<float> &b, std::vector<float> &hf)
+{
+    // Centred DFT  Z[k] = (1/n) sum_s z[s] exp(-i 2 pi (k-c)(s-c)/n),  c = n/2.
+    //   (k-c)(s-c) = ks - c(k+s) + c^2
+    // direct (L == n):     a[s] = exp(+i 2 pi c s/n),  b[k] = (1/n) exp(+i 2 pi (c k - c^2)/n)
+    // Bluestein (L > n):   ks = (k^2 + s^2 - (k-s)^2)/2
+    //   a[s] = exp(i pi (-s^2 + 2 c s)/n), b[k] = (1/n) exp(i pi (-k^2 + 2 c k - 2 c^2)/n),
+    //   h[d] = exp(+i pi d^2/n), Z = b .* (a.*z (*) h); hf = FFT_L(h)/L.
+    const long long c = n / 2, n2 = 2LL * n;
+    const bool direct = (L == n);
+    a.resize(2 * (size_t)n); b.resize(2 * (size_t)n);
+    for (long long s = 0; s < n; ++s) {
+        const long long pa = direct ? posmod(2 * c * s, n2) : posmod(-s * s + 2 * c * s, n2);
+        const long long pb = direct ? posmod(2 * c * s - 2 * c * c, n2)
+                                    : posmod(-s * s + 2 * c * s - 2 * c * c, n2);
+        const double aa = kPi * (double)pa / (double)n, ab = kPi * (double)pb / (double)n;
+        a[2 * s] = (float)std::cos(aa); a[2 * s + 1] = (float)std::sin(aa);
+        b[2 * s] = (float)(std::cos(ab) / n); b[2 * s + 1] = (float)(std::sin(ab) / n);
+    }
+    hf.clear();
+    if (direct) return;
+    std::vector<double> hr(L, 0.0), hi(L, 0.0);
+    for (long long d = -(n - 1); d <= n - 1; ++d) {
+        const double ang = kPi * (double)posmod(d * d, n2) / (double)n;
+        const int idx = (int)posmod(d, L);
+        hr[idx] = std::cos(ang); hi[idx] = std::sin(ang);
+    }
+    host_fft(hr, hi);
+    hf.resize(2 * (size_t)L);
+    for (int q = 0; q < L; ++q) {
+        hf[2 * q] = (float)(hr[q] / L);
+        hf[2 * q + 1] = (float)(hi[q] / L);
+    }
+}
+
+// ---------------------------------------------------------------- rounds ---------
+struct Cand {
+    uint32_t ak;
+    int16_t lx, ly;
+};
+
+struct Occupancy {          // bitmap of up to 128 x 64 cells
+    uint64_t rows[SP_H > GT_ROWS ? SP_H : GT_ROWS][2];
+    void clear() { std::memset(rows, 0, sizeof(rows)); }
+    static inline void span(int lx, uint64_t &m0, uint64_t &m1)
+    {
+        // KW consecutive bits starting at lx (lx + KW <= 128)
+        const unsigned __int128 m = ((((unsigned __int128)1) << KW) - 1) << lx;
+        m0 = (uint64_t)m; m1 = (uint64_t)(m >> 64);
+    }
+    bool overlaps(int lx, int ly) const
+    {
+        uint64_t m0, m1; span(lx, m0, m1);
+        for (int r = 0; r < KW; ++r)
+            if ((rows[ly + r][0] & m0) | (rows[ly + r][1] & m1)) return true;
+        return false;
+    }
+    void mark(int lx, int ly)
+    {
+        uint64_t m0, m1; span(lx, m0, m1);
+        for (int r = 0; r < KW; ++r) { rows[ly + r][0] |= m0; rows[ly + r][1] |= m1; }
+    }
+};
+
+// Greedy packing of `cands` (in order) into rounds of 32 lanes.  Appends 32 slots per
+// round to `out`; returns the number of rounds.
+static int build_rounds(std::vector<Cand> &cands, bool disjoint, int pitch,
+                        std::vector<Slot> &out, long long &filled)
+{
+    int rounds = 0;
+    Occupancy occ;
+    std::vector<Cand> next;
+    next.reserve(cands.size());
+    while (!cands.empty()) {
+        if (disjoint) occ.clear();
+        uint32_t mask[2] = {0u, 0u};
+        int cnt[2] = {0, 0};
+        Slot lanes[32];
+        for (int i = 0; i < 32; ++i) { lanes[i].ak = SLOT_EMPTY; lanes[i].lxy = 0; }
+        next.clear();
+        size_t i = 0;
+        for (; i < cands.size(); ++i) {
+            if (cnt[0] == 16 && cnt[1] == 16) break;
+            const Cand &c = cands[i];
+            const uint32_t res = 1u << ((c.ly * pitch + c.lx) & 15);
+            int h = -1;
+            if (cnt[0] < 16 && !(mask[0] & res)) h = 0;
+            else if (cnt[1] < 16 && !(mask[1] & res)) h = 1;
+            if (h < 0 || (disjoint && occ.overlaps(c.lx, c.ly))) { next.push_back(c); continue; }
+            if (disjoint) occ.mark(c.lx, c.ly);
+            mask[h] |= res;
+            Slot &s = lanes[h * 16 + cnt[h]++];
+            s.ak = c.ak;
+            s.lxy = (uint32_t)c.lx | ((uint32_t)c.ly << 16);
+        }
+        for (; i < cands.size(); ++i) next.push_back(cands[i]);
+        filled += cnt[0] + cnt[1];
+        out.insert(out.end(), lanes, lanes + 32);
+        cands.swap(next);
+        ++rounds;
+    }
+    return rounds;
+}
+
+static inline int floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+// ---------------------------------------------------------------- gather ---------
+static void build_gather(const Geometry &g, Schedules &out)
+{
+    const int G = g.G;
+    const int ntx = (G + GT_X - 1) / GT_X, nty = (G + GT_Y - 1) / GT_Y;
+    const long long M = (long long)g.n_angles * g.n_det;
+    std::vector<uint32_t> count((size_t)ntx * nty + 1, 0);
+    std::vector<uint32_t> tile_of(M);
+    std::vector<Cand> all(M);
+    for (int a = 0; a < g.n_angles; ++a)
+        for (int k = 0; k < g.n_det; ++k) {
+            int x0, y0;
+            g.base(a, k, x0, y0);
+            const int bx = (int)posmod(x0, G), by = (int)posmod(y0, G);
+            const int t = (by / GT_Y) * ntx + (bx / GT_X);
+            const long long m = (long long)a * g.n_det + k;
+            tile_of[m] = (uint32_t)t;
+            all[m].ak = ((uint32_t)a << 16) | (uint32_t)k;
+            all[m].lx = (int16_t)(bx % GT_X);
+            all[m].ly = (int16_t)(by % GT_Y);
+            ++count[t + 1];
+        }
+    for (size_t t = 0; t < (size_t)ntx * nty; ++t) count[t + 1] += count[t];
+    std::vector<uint32_t> order(M), fill(count.begin(), count.end() - 1);
+    for (long long m = 0; m < M; ++m) order[fill[tile_of[m]]++] = (uint32_t)m;   // stable: (a,k) order
+
+    std::vector<Cand> cands;
+    for (int t = 0; t < ntx * nty; ++t) {
+        if (count[t + 1] == count[t]) continue;
+        cands.clear();
+        for (uint32_t q = count[t]; q < count[t + 1]; ++q) cands.push_back(all[order[q]]);
+        const int rb = (int)(out.gather_slots.size() / 32);
+        const int nr = build_rounds(cands, false, GT_PITCH, out.gather_slots, out.gather_filled);
+        for (int r = 0; r < nr; r += GATHER_ROUND_CAP) {
+            GatherCta c;
+            c.tx0 = (t % ntx) * GT_X; c.ty0 = (t / ntx) * GT_Y;
+            c.round_begin = rb + r;
+            c.round_count = std::min(GATHER_ROUND_CAP, nr - r);
+            out.gather_ctas.push_back(c);
+        }
+    }
+    std::stable_sort(out.gather_ctas.begin(), out.gather_ctas.end(),
+                     [](const GatherCta &x, const GatherCta &y) { return x.round_count > y.round_count; });
+}
+
+// ---------------------------------------------------------------- scatter --------
+struct Image { uint32_t ak; int bx, by; };   // one wrap image of a sample: base cell (may be < 0)
+
+static void build_scatter(const Geometry &g, Schedules &out)
+{
+    const int G = g.G;
+    const int nrx = (G + SR_X - 1) / SR_X, nry = (G + SR_Y - 1) / SR_Y;
+    const int nrect = nrx * nry;
+    // pass 1: count incidences (image, rect); pass 2: fill
+    std::vector<uint32_t> count((size_t)nrect + 1, 0);
+    std::vector<Image> inc;
+    for (int pass = 0; pass < 2; ++pass) {
+        std::vector<uint32_t> fill;
+        if (pass == 1) {
+            for (int r = 0; r < nrect; ++r) count[r + 1] += count[r];
+            inc.resize(count[nrect]);
+            fill.assign(count.begin(), count.end() - 1);
+        }
+        for (int a = 0; a < g.n_angles; ++a)
+            for (int k = 0; k < g.n_det; ++k) {
+                int x0, y0;
+                g.base(a, k, x0, y0);
+                for (int sy = -1; sy <= 1; ++sy) {
+                    const int by = y0 + sy * G;
+                    if (by + KH < 0 || by > G - 1) continue;
+                    for (int sx = -1; sx <= 1; ++sx) {
+                        const int bx = x0 + sx * G;
+                        if (bx + KH < 0 || bx > G - 1) continue;
+                        const int rx_lo = std::max(bx, 0) / SR_X, rx_hi = std::min(bx + KH, G - 1) / SR_X;
+                        const int ry_lo = std::max(by, 0) / SR_Y, ry_hi = std::min(by + KH, G - 1) / SR_Y;
+                        for (int ry = ry_lo; ry <= ry_hi; ++ry)
+                            for (int rx = rx_lo; rx <= rx_hi; ++rx) {
+                                const int r = ry * nrx + rx;
+                                if (pass == 0) ++count[r + 1];
+                                else inc[fill[r]++] = Image{((uint32_t)a << 16) | (uint32_t)k, bx, by};
+                            }
+                    }
+                }
+            }
+    }
+
+    struct Pending { ScatterCta cta; long long work; };
+    std::vector<Pending> ctas;
+    std::vector<Cand> item_c[SCATTER_ITEMS];
+    std::vector<Slot> tmp_slots;
+
+    for (int r = 0; r < nrect; ++r) {
+        const int rx0 = (r % nrx) * SR_X, ry0 = (r / nrx) * SR_Y;
+        const int rw = std::min(SR_X, G - rx0), rh = std::min(SR_Y, G - ry0);
+        const int nsx = (rw + ST_X - 1) / ST_X, nsy = (rh + ST_Y - 1) / ST_Y;
+        const uint32_t lo = count[r], hi = count[r + 1];
+
+        // --- try the light layout: one warp per sub-tile -------------------------
+        for (auto &v : item_c) v.clear();
+        for (uint32_t q = lo; q < hi; ++q) {
+            const Image &im = inc[q];
+            const int ix = std::min(std::max(floordiv(im.bx - rx0, ST_X), 0), nsx - 1);
+            const int iy = std::min(std::max(floordiv(im.by - ry0, ST_Y), 0), nsy - 1);
+            Cand c;
+            c.ak = im.ak;
+            c.lx = (int16_t)(im.bx - (rx0 + ix * ST_X - KH));
+            c.ly = (int16_t)(im.by - (ry0 + iy * ST_Y - KH));
+            item_c[iy * 2 + ix].push_back(c);
+        }
+        Pending p;
+        std::memset(&p.cta, 0, sizeof(p.cta));
+        p.cta.rx0 = rx0; p.cta.ry0 = ry0; p.cta.rw = rw; p.cta.rh = rh; p.cta.partial_slot = -1;
+        tmp_slots.clear();
+        long long tmp_filled = 0;
+        int max_rounds = 0, tmp_rounds[SCATTER_ITEMS], tmp_begin[SCATTER_ITEMS];
+        for (int it = 0; it < SCATTER_ITEMS; ++it) {
+            tmp_begin[it] = (int)(tmp_slots.size() / 32);
+            tmp_rounds[it] = build_rounds(item_c[it], true, SP_PITCH, tmp_slots, tmp_filled);
+            max_rounds = std::max(max_rounds, tmp_rounds[it]);
+        }
+        if (max_rounds <= SCATTER_ROUND_MAX) {
+            const int base = (int)(out.scatter_slots.size() / 32);
+            out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
+            out.scatter_filled += tmp_filled;
+            p.work = 0;
+            for (int it = 0; it < SCATTER_ITEMS; ++it) {
+                const int ix = it % 2, iy = it / 2;
+                p.cta.items[it].px0 = rx0 + ix * ST_X - KH;
+                p.cta.items[it].py0 = ry0 + iy * ST_Y - KH;
+                p.cta.items[it].round_begin = base + tmp_begin[it];
+                p.cta.items[it].round_count = tmp_rounds[it];
+                p.work = std::max<long long>(p.work, tmp_rounds[it]);
+            }
+            ctas.push_back(p);
+            continue;
+        }
+
+        // --- heavy rectangle: one output rectangle per sub-tile, samples dealt ------
+        // round-robin over 4*K warps that all cover the same sub-tile.
+        for (int iy = 0; iy < nsy; ++iy)
+            for (int ix = 0; ix < nsx; ++ix) {
+                const int sx0 = rx0 + ix * ST_X, sy0 = ry0 + iy * ST_Y;
+                const int sw = std::min(ST_X, rx0 + rw - sx0), sh = std::min(ST_Y, ry0 + rh - sy0);
+                std::vector<Cand> sub;
+                for (uint32_t q = lo; q < hi; ++q) {
+                    const Image &im = inc[q];
+                    if (im.bx + KH < sx0 || im.bx >= sx0 + sw || im.by + KH < sy0 || im.by >= sy0 + sh) continue;
+                    Cand c;
+                    c.ak = im.ak;
+                    c.lx = (int16_t)(im.bx - (sx0 - KH));
+                    c.ly = (int16_t)(im.by - (sy0 - KH));
+                    sub.push_back(c);
+                }
+                int K = std::max<int>(1, (int)((sub.size() + (size_t)SCATTER_ITEMS * 16 * SCATTER_ROUND_MAX - 1)
+                                                / ((size_t)SCATTER_ITEMS * 16 * SCATTER_ROUND_MAX)));
+                std::vector<std::vector<Cand>> deal;
+                std::vector<int> rb, rc;
+                long long f = 0;
+                for (int attempt = 0; attempt < 8; ++attempt) {
+                    const int ni = K * SCATTER_ITEMS;
+                    deal.assign(ni, {});
+                    for (size_t q = 0; q < sub.size(); ++q) deal[q % ni].push_back(sub[q]);
+                    tmp_slots.clear(); f = 0; rb.assign(ni, 0); rc.assign(ni, 0);
+                    int mr = 0;
+                    for (int it = 0; it < ni; ++it) {
+                        rb[it] = (int)(tmp_slots.size() / 32);
+                        rc[it] = build_rounds(deal[it], true, SP_PITCH, tmp_slots, f);
+                        mr = std::max(mr, rc[it]);
+                    }
+                    if (mr <= SCATTER_ROUND_MAX || attempt == 7) break;
+                    K = (int)std::ceil(K * (double)mr / SCATTER_ROUND_MAX * 1.15) + 1;
+                }
+                const int base = (int)(out.scatter_slots.size() / 32);
+                out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
+                out.scatter_filled += f;
+                int first_slot = -1;
+                if (K > 1) {
+                    first_slot = out.n_partial_slots;
+                    out.n_partial_slots += K;
+                    MergeJob mj{sx0, sy0, sw, sh, first_slot, K};
+                    out.merge_jobs.push_back(mj);
+                }
+                for (int kk = 0; kk < K; ++kk) {
+                    Pending hp;
+                    std::memset(&hp.cta, 0, sizeof(hp.cta));
+                    hp.cta.rx0 = sx0; hp.cta.ry0 = sy0; hp.cta.rw = sw; hp.cta.rh = sh;
+                    hp.cta.partial_slot = (K > 1) ? first_slot + kk : -1;
+                    hp.work = 0;
+                    for (int it = 0; it < SCATTER_ITEMS; ++it) {
+                        const int id = kk * SCATTER_ITEMS + it;
+                        hp.cta.items[it].px0 = sx0 - KH;
+                        hp.cta.items[it].py0 = sy0 - KH;
+                        hp.cta.items[it].round_begin = base + rb[id];
+                        hp.cta.items[it].round_count = rc[id];
+                        hp.work = std::max<long long>(hp.work, rc[id]);
+                    }
+                    ctas.push_back(hp);
+                }
+            }
+    }
+    std::stable_sort(ctas.begin(), ctas.end(),
+                     [](const Pending &x, const Pending &y) { return x.work > y.work; });
+    out.scatter_ctas.reserve(ctas.size());
+    for (auto &p : ctas) out.scatter_ctas.push_back(p.cta);
+}
+
+void build_schedules(const Geometry &g, Schedules &out)
+{
+    out = Schedules();
+    build_gather(g, out);
+    build_scatter(g, out);
+}
+
+// ---------------------------------------------------------------- self check -----
+static inline uint64_t tap_hash(uint32_t ak, int tx, int ty)
+{
+    uint64_t h = (uint64_t)ak * 0x9E3779B97F4A7C15ull + (uint64_t)(ty * KW + tx + 1) * 0xC2B2AE3D27D4EB4Full;
+    h ^= h >> 29;
+    return h | 1ull;
+}
+
+long long check_schedules(const Geometry &g, const Schedules &s)
+{
+    long long bad = 0;
+    const int G = g.G;
+    const long long M = (long long)g.n_angles * g.n_det;
+
+    auto check_round = [&](const Slot *lanes, int pitch, bool disjoint) {
+        Occupancy occ;
+        occ.clear();
+        for (int h = 0; h < 2; ++h) {
+            uint32_t mask = 0;
+            for (int l = 0; l < 16; ++l) {
+                const Slot &sl = lanes[h * 16 + l];
+                if (sl.ak == SLOT_EMPTY) continue;
+                const int lx = sl.lxy & 0xffff, ly = sl.lxy >> 16;
+                const uint32_t res = 1u << ((ly * pitch + lx) & 15);
+                if (mask & res) ++bad;
+                mask |= res;
+                if (disjoint) {
+                    if (lx + KW > SP_W || ly + KW > SP_H) { ++bad; continue; }
+                    if (occ.overlaps(lx, ly)) ++bad;
+                    occ.mark(lx, ly);
+                }
+            }
+        }
+    };
+
+    // gather: every sample exactly once, at the right place
+    std::vector<uint8_t> seen(M, 0);
+    for (const GatherCta &c : s.gather_ctas) {
+        if (c.tx0 % GT_X || c.ty0 % GT_Y || c.tx0 < 0 || c.ty0 < 0 || c.tx0 >= G || c.ty0 >= G) ++bad;
+        if (c.round_count < 1 || c.round_count > GATHER_ROUND_CAP) ++bad;
+        for (int r = 0; r < c.round_count; ++r) {
+            const Slot *lanes = &s.gather_slots[(size_t)(c.round_begin + r) * 32];
+            check_round(lanes, GT_PITCH, false);
+            for (int l = 0; l < 32; ++l) {
+                if (lanes[l].ak == SLOT_EMPTY) continue;
+                const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;
+                if (a >= g.n_angles || k >= g.n_det) { ++bad; continue; }
+                int x0, y0;
+                g.base(a, k, x0, y0);
+                const int lx = lanes[l].lxy & 0xffff, ly = lanes[l].lxy >> 16;
+                if (lx >= GT_X || ly >= GT_Y) ++bad;
+                if (posmod(c.tx0 + lx - x0, G) != 0 || posmod(c.ty0 + ly - y0, G) != 0) ++bad;
+                if (seen[(size_t)a * g.n_det + k]++) ++bad;
+            }
+        }
+    }
+    for (long long m = 0; m < M; ++m) if (!seen[m]) ++bad;
+
+    // scatter: simulate with hashed unit weights and compare with the definition
+    std::vector<uint64_t> expect((size_t)G * G, 0), got((size_t)G * G, 0);
+    std::vector<uint8_t> written((size_t)G * G, 0);
+    for (int a = 0; a < g.n_angles; ++a)
+        for (int k = 0; k < g.n_det; ++k) {
+            int x0, y0;
+            g.base(a, k, x0, y0);
+            const uint32_t ak = ((uint32_t)a << 16) | (uint32_t)k;
+            for (int ty = 0; ty < KW; ++ty)
+                for (int tx = 0; tx < KW; ++tx)
+                    expect[(size_t)posmod(y0 + ty, G) * G + posmod(x0 + tx, G)] += tap_hash(ak, tx, ty);
+        }
+    std::vector<int> slot_owner(s.n_partial_slots, 0);
+    for (const ScatterCta &c : s.scatter_ctas) {
+        if (c.rx0 < 0 || c.ry0 < 0 || c.rx0 + c.rw > G || c.ry0 + c.rh > G || c.rw < 1 || c.rh < 1) { ++bad; continue; }
+        if (c.partial_slot >= 0) {
+            if (c.partial_slot >= s.n_partial_slots || c.rw > ST_X || c.rh > ST_Y) { ++bad; continue; }
+            ++slot_owner[c.partial_slot];
+        } else {
+            for (int y = 0; y < c.rh; ++y)
+                for (int x = 0; x < c.rw; ++x) ++written[(size_t)(c.ry0 + y) * G + c.rx0 + x];
+        }
+        for (int it = 0; it < SCATTER_ITEMS; ++it) {
+            const ScatterItem &I = c.items[it];
+            if (I.round_count > 0 && (I.px0 + SP_W < c.rx0 || I.py0 + SP_H < c.ry0)) ++bad;
+            for (int r = 0; r < I.round_count; ++r) {
+                const Slot *lanes = &s.scatter_slots[(size_t)(I.round_begin + r) * 32];
+                check_round(lanes, SP_PITCH, true);
+                for (int l = 0; l < 32; ++l) {
+                    if (lanes[l].ak == SLOT_EMPTY) continue;
+                    const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;
+                    if (a >= g.n_angles || k >= g.n_det) { ++bad; continue; }
+                    int x0, y0;
+                    g.base(a, k, x0, y0);
+                    const int bx = I.px0 + (int)(lanes[l].lxy & 0xffff), by = I.py0 + (int)(lanes[l].lxy >> 16);
+                    if (posmod(bx - x0, G) != 0 || posmod(by - y0, G) != 0) ++bad;
+                    for (int ty = 0; ty < KW; ++ty)
+                        for (int tx = 0; tx < KW; ++tx) {
+                            const int cx = bx + tx, cy = by + ty;
+                            if (cx < c.rx0 || cx >= c.rx0 + c.rw || cy < c.ry0 || cy >= c.ry0 + c.rh) continue;
+                            got[(size_t)cy * G + cx] += tap_hash(lanes[l].ak, tx, ty);
+                        }
+                }
+            }
+        }
+    }
+    for (const MergeJob &mj : s.merge_jobs) {
+        for (int i = 0; i < mj.n_slots; ++i)
+            if (mj.first_slot + i >= s.n_partial_slots || slot_owner[mj.first_slot + i] != 1) ++bad;
+        for (int y = 0; y < mj.rh; ++y)
+            for (int x = 0; x < mj.rw; ++x) ++written[(size_t)(mj.ry0 + y) * G + mj.rx0 + x];
+    }
+    for (size_t i = 0; i < (size_t)G * G; ++i) {
+        if (written[i] != 1) ++bad;
+        if (got[i] != expect[i]) ++bad;
+    }
+    return bad;
+}
+
+}  // namespace radon

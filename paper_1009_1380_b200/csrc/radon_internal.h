@@ -1,0 +1,142 @@
+// radon_internal.h -- data structures shared by the host-side plan builder and the
+// CUDA kernels of libradon_b200.  Not part of the public ABI (include/radon.h is).
+#pragma once
+#include <cstdint>
+#include <vector>
+
+namespace radon {
+
+// ---- compile-time configuration -------------------------------------------------
+constexpr int KW = 6;                 // Kaiser-Bessel width this build is specialised for
+constexpr int KH = KW - 1;            // halo: a footprint reaches base .. base+KH
+// Kaiser-Bessel weight table.  Default: ONE polynomial piece per tap (degree KB_DEG in
+// z = 2*delta - 1, fitted in fp64 at plan time, max error ~7e-8), passed to the kernels in
+// the constant bank -- a lookup table whose rows are polynomial pieces, read as broadcast
+// operands, so it costs neither shared-memory bandwidth nor bank conflicts.
+// -DRADON_KB_LUT=1 builds the classic variant instead (LUT_S rows per grid unit in shared
+// memory, linear interpolation; ~3e-6 relative error at LUT_S = 256) for A/B measurements.
+#ifndef RADON_KB_LUT
+#define RADON_KB_LUT 0
+#endif
+constexpr int KB_DEG = 7;
+constexpr int KB_HALF = (KB_DEG + 1) / 2;   // coefficients of the even / odd part
+struct KbPoly {                       // tap l: E_l(z^2) + z O_l(z^2); tap KW-1-l: E_l - z O_l
+    float e[KW / 2][KB_HALF];
+    float o[KW / 2][KB_HALF];
+};
+#ifdef __CUDACC__
+#define RADON_HD __host__ __device__ __forceinline__
+#else
+#define RADON_HD inline
+#endif
+// w[l] = phi(delta - W/2 + l), l = 0..KW-1, delta in [0,1]: Horner in z^2 on the even and odd
+// parts.  In the kernels kp sits in the parameter constant bank, so its entries are FFMA
+// operands, not loads.  Host-callable for the CPU-side unit test.
+RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
+{
+    const float z = 2.f * delta - 1.f, z2 = z * z;
+#ifdef __CUDACC__
+#pragma unroll
+#endif
+    for (int l = 0; l < KW / 2; ++l) {
+        float e = kp.e[l][KB_HALF - 1], o = kp.o[l][KB_HALF - 1];
+#ifdef __CUDACC__
+#pragma unroll
+#endif
+        for (int h = KB_HALF - 2; h >= 0; --h) {
+            e = e * z2 + kp.e[l][h];
+            o = o * z2 + kp.o[l][h];
+        }
+        w[l] = e + z * o;
+        w[KW - 1 - l] = e - z * o;
+    }
+}
+constexpr int LUT_S = 256;            // (RADON_KB_LUT) rows per grid unit, linear interpolation
+constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, slope) per tap
+
+// Gather (inverse gridding): one CTA stages a GT_X x GT_Y tile of the grid (+halo).
+constexpr int GT_X = 128, GT_Y = 64;
+constexpr int GT_PITCH = GT_X + KH;   // 133 complex per smem row (odd: spreads bank pairs)
+constexpr int GT_ROWS = GT_Y + KH;    // 69
+constexpr int GATHER_WARPS = 8;
+constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
+
+// Scatter (gridding): each warp owns a private accumulator of one ST_X x ST_Y sub-tile
+// plus a KH margin on every side; a CTA merges its warps' accumulators in fixed order.
+constexpr int ST_X = 64, ST_Y = 32;
+constexpr int SP_W = ST_X + 2 * KH;   // 74
+constexpr int SP_H = ST_Y + 2 * KH;   // 42
+constexpr int SP_PITCH = SP_W + 1;    // 75 (odd)
+constexpr int SCATTER_ITEMS = 4;      // warps per CTA
+constexpr int SR_X = 2 * ST_X, SR_Y = 2 * ST_Y;   // light CTA output rectangle: 2 x 2 sub-tiles
+constexpr int SCATTER_ROUND_MAX = 48; // rounds per warp before a rectangle is split further
+
+// One lane's work in one round: which polar sample, and where its W x W footprint
+// starts inside the staged tile (gather) or the warp-private accumulator (scatter).
+struct Slot {
+    uint32_t ak;    // (a << 16) | k ; 0xFFFFFFFF = idle lane
+    uint32_t lxy;   // lx0 | (ly0 << 16)
+};
+constexpr uint32_t SLOT_EMPTY = 0xFFFFFFFFu;
+
+struct GatherCta {
+    int tx0, ty0;               // tile origin (cells, centred layout)
+    int round_begin, round_count;
+};
+
+struct ScatterItem {
+    int px0, py0;               // grid coordinates of the private accumulator's origin
+    int round_begin, round_count;
+};
+
+struct ScatterCta {
+    int rx0, ry0, rw, rh;       // output rectangle (cells this CTA, alone, writes)
+    int partial_slot;           // -1: write the grid; >= 0: write this scratch slot
+    int pad0, pad1, pad2;
+    ScatterItem items[SCATTER_ITEMS];
+};
+
+struct MergeJob {               // sum n_slots partial rectangles, in order, into the grid
+    int rx0, ry0, rw, rh;
+    int first_slot, n_slots;
+};
+
+// ---- host-side geometry + schedules ----------------------------------------------
+struct Geometry {
+    int N = 0, G = 0, n_angles = 0, n_det = 0, W = KW;
+    double sigma = 2.0;
+    std::vector<double> cs;     // per angle: (G/n) cos(theta_a), (G/n) sin(theta_a)
+
+    void init(int N_, int n_angles_, int n_det_, double sigma_, int W_);
+    // Base cell (centred layout, may lie in [-W/2, G - W/2]) of sample (a, k):
+    // x0 = ceil(G/2 + kappa_x - W/2).  Bit-identical to the device code (same fma).
+    void base(int a, int k, int &x0, int &y0) const;
+};
+
+struct Schedules {
+    std::vector<Slot> gather_slots;         // 32 per round
+    std::vector<GatherCta> gather_ctas;
+    std::vector<Slot> scatter_slots;
+    std::vector<ScatterCta> scatter_ctas;
+    std::vector<MergeJob> merge_jobs;
+    int n_partial_slots = 0;
+    long long gather_filled = 0, scatter_filled = 0;
+};
+
+void build_schedules(const Geometry &g, Schedules &out);
+// Returns the number of violated invariants (0 = schedules are valid).
+long long check_schedules(const Geometry &g, const Schedules &s);
+
+// ---- host-side tables (all derived in fp64, stored fp32) -------------------------
+double kb_beta(int W, double sigma);
+double kb_i0(double z);
+void build_kb_lut(int W, double sigma, std::vector<float> &lut);              // LUT_S x LUT_ROW
+void build_kb_poly(int W, double sigma, KbPoly &kp);                            // Chebyshev fit, fp64
+void build_deapod(int N, int G, int W, double sigma, std::vector<float> &d);   // N floats
+void build_twiddles(int L, std::vector<float> &tw);                            // L x (cos, -sin)
+// Bluestein / centred-DFT tables for length n, FFT length L (power of two >= 2n-1, or
+// L == n when n is a power of two: then hf is empty and a/b are the centring phases).
+void build_chirp(int n, int L, std::vector<float> &a, std::vector<float> &b, std::vector<float> &hf);
+int next_pow2(int v);
+
+}  // namespace radon

@@ -1,0 +1,80 @@
+"""CPU-only tests: the C-ABI library loads and exports every symbol include/radon.h declares,
+argument validation, and the plan-time schedule builder's invariants (no GPU compute)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1009_1380_b200 as rb
+from paper_1009_1380_b200 import build as rb_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    rb_build.build()
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "radon.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(radon_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations parsed"
+    L = ctypes.CDLL(rb.lib_path())
+    for name in declared:
+        assert hasattr(L, name), f"{name} declared in include/radon.h but not exported"
+    assert declared == set(rb.EXPORTED_SYMBOLS), declared ^ set(rb.EXPORTED_SYMBOLS)
+
+
+def test_strerror_and_validation_without_gpu():
+    L = rb.lib()
+    assert L.radon_strerror(0) == b"ok"
+    assert b"invalid" in L.radon_strerror(-1)
+    h = ctypes.c_void_p(123)
+    # invalid arguments are rejected before any CUDA call
+    assert L.radon_plan_create(ctypes.byref(h), 4, 10, 10, 2.0, 6) == -1 and not h.value     # N < 8
+    assert L.radon_plan_create(ctypes.byref(h), 64, 0, 91, 2.0, 6) == -1
+    assert L.radon_plan_create(ctypes.byref(h), 64, 90, 1, 2.0, 6) == -1
+    assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 13) == -1
+    assert L.radon_plan_create(ctypes.byref(h), 65, 90, 91, 1.5, 6) == -1                   # odd sigma*N
+    assert L.radon_plan_create(None, 64, 90, 91, 2.0, 6) == -1
+    assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 4) == -5                   # W != 6: not built
+    assert L.radon_plan_create(ctypes.byref(h), 96, 90, 91, 2.0, 6) == -5                   # G not a power of two
+    assert L.radon_plan_destroy(None) == 0
+    assert L.radon_forward(None, None, None, None) == -1
+
+
+@pytest.mark.parametrize("shape", [(8, 5, 9), (16, 7, 12), (32, 33, 47), (64, 90, 91), (128, 64, 181),
+                                   (256, 100, 256)])
+def test_schedule_invariants(shape):
+    """Every sample issued exactly once by the gather; every (sample, wrap image, tap, cell)
+    incidence accumulated exactly once by the scatter; footprints of a round disjoint; bank
+    pairs distinct per half-warp; every grid cell written exactly once."""
+    rc, bad = rb.schedule_selfcheck(*shape)
+    assert (rc, bad) == (0, 0)
+
+
+def test_schedule_stats_config2_shape():
+    st = rb.schedule_host_stats(512, 360, 725)
+    M = 360 * 725
+    assert st["gather_filled"] == M
+    assert st["scatter_filled"] >= M                       # owner-computes duplicates at tile borders
+    assert st["scatter_filled"] < 1.3 * M
+    assert st["gather_filled"] / st["gather_slots"] > 0.8  # lane utilisation of the gather rounds
+    assert st["scatter_max_rounds"] <= 64 and st["gather_max_rounds"] <= 64
+
+
+def test_kb_polynomial_weights_match_oracle_kernel():
+    """The kernels' tap weights (plan-time degree-7 polynomial pieces, fp32 Horner) against
+    the oracle's directly evaluated Kaiser-Bessel kernel: |err| < 3e-7 (fp32 round-off level)."""
+    import numpy as np
+    import oracle
+
+    worst = 0.0
+    for delta in np.linspace(0.0, 1.0, 257):
+        w = np.array(rb.kb_weights_host(float(delta)))
+        ref = oracle.kb_phi(np.float32(delta).astype(np.float64) - 3.0 + np.arange(6))
+        worst = max(worst, float(np.abs(w - ref).max()))
+    assert worst < 3e-7, worst

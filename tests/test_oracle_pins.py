@@ -54,6 +54,23 @@ def test_c1b_dirichlet_closed_form_function_matches_direct_sum():
         assert np.abs(oracle.forward(x, 9, n_det) - oracle.dirichlet_forward(x, 9, n_det)).max() < 1e-11
 
 
+def test_c1c_closed_form_subset_and_adjoint_match_direct_sums():
+    """The closed-form subset/adjoint routines (used for sampled outputs at full sizes)
+    against the by-the-definition double sums, odd and even n_det, and the dot test."""
+    x = RNG.standard_normal((12, 12)); x[3, 4] = 0.0
+    for n_det in (19, 20):
+        y = RNG.standard_normal((7, n_det)); y[2, 5] = 0.0
+        idx = RNG.choice(7 * n_det, 30, replace=False)
+        assert np.abs(oracle.dirichlet_forward_subset(x, 7, n_det, idx)
+                      - oracle.forward(x, 7, n_det).ravel()[idx]).max() < 1e-11
+        A = oracle.adjoint(y, 12)
+        assert np.abs(oracle.dirichlet_adjoint(y, 12) - A).max() < 1e-11
+        pix = RNG.choice(144, 17, replace=False)
+        assert np.abs(oracle.dirichlet_adjoint(y, 12, pix=pix) - A.ravel()[pix]).max() < 1e-11
+        lhs = np.vdot(oracle.dirichlet_forward(x, 7, n_det), y); rhs = np.vdot(x, oracle.dirichlet_adjoint(y, 12))
+        assert abs(lhs - rhs) < 1e-11 * abs(lhs)
+
+
 # --------------------------------------------------- C2 axis-aligned slices ----
 def test_c2_axis_rows_are_column_and_row_sums():
     N, n_angles, n_det = 24, 8, 31          # n_det >= N, even n_angles
