@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py -- NUFFT-Radon forward+adjoint pairs/s on B200 (BASELINE.json metric).
+
+A step = one pass of the whole hot path (radon_forward_batch then radon_adjoint_batch: stages
+F1-F4 and A1-A4 of SURVEY.md 8(a)) over one batch of `--slices` synthetic 2048^2 slices with
+1025 x 2048 projections (BASELINE.json configs[3] shape, batched as configs[4]).  `value` is
+whole-job pairs/s with inputs resident in HBM; `e2e` is the same metric through the host-buffer
+C-ABI calls (pinned host memory, copies inside the timed region).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--slices B] [--impl reference]
+  torchrun ... bench.py --gpus N ...      one rank per GPU; slice-parallel replicas (weak scaling)
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "nufft_radon_fwd_adj_pairs_per_s"
+UNIT = "pairs/s"
+WORKLOAD = "config4_beamline_2048 (2048^2 fp32, 1025 angles x 2048 bins, sigma=2, W=6)"
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def stage_bytes(N, G, M):
+    """Algorithmic bytes per launch of each stage."""
+    return {
+        "F1_colfft": 4 * N * N + 8 * G * N, "F2_rowfft": 8 * G * N + 8 * G * G,
+        "F3_gather": 8 * G * G + 8 * M, "F4_proj_ifft": 8 * M + 4 * M,
+        "A1_proj_fft": 4 * M + 8 * M, "A2_scatter": 8 * M + 8 * G * G,
+        "A3_rowifft": 8 * G * G + 8 * G * N, "A4_colifft": 8 * G * N + 4 * N * N,
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_pairs_per_s(cfg, n_sample, seed=77):
+    """The oracle as it stands (closed-form O-direct, the routine the full-size parity tests
+    use) on a bounded sample: n_sample sinogram entries + n_sample pixels of one slice;
+    cost is exactly linear in the number of outputs, so pairs/s is extrapolated."""
+    import numpy as np
+
+    import oracle
+    import workloads
+
+    x = workloads.make_batch_slice(0, cfg.N).astype(np.float64)
+    rng = np.random.default_rng(seed)
+    idx = rng.choice(cfg.M, n_sample, replace=False)
+    pix = rng.choice(cfg.N * cfg.N, n_sample, replace=False)
+    y = rng.standard_normal((cfg.n_angles, cfg.n_det))
+    t0 = time.perf_counter(); oracle.dirichlet_forward_subset(x, cfg.n_angles, cfg.n_det, idx)
+    t1 = time.perf_counter(); oracle.dirichlet_adjoint(y, cfg.N, pix=pix)
+    t2 = time.perf_counter()
+    t_pair = (t1 - t0) / n_sample * cfg.M + (t2 - t1) / n_sample * cfg.N * cfg.N
+    return 1.0 / t_pair, oracle.num_threads(), (t2 - t0)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same metric/config."""
+    import workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = workloads.get_config(4)
+    n_sample = args.ref_sample
+    for _ in range(args.warmup and 1):
+        cpu_oracle_pairs_per_s(cfg, max(n_sample // 8, 8))
+    vals, t_total = [], 0.0
+    for _ in range(args.steps):
+        v, cores, dt = cpu_oracle_pairs_per_s(cfg, n_sample)
+        vals.append(v); t_total += dt
+    value = len(vals) / sum(1.0 / v for v in vals)
+    sample = (f"{n_sample} sinogram entries + {n_sample} pixels of one slice per step, closed-form "
+              f"O-direct (oracle.dirichlet_forward_subset / dirichlet_adjoint), extrapolated x M/{n_sample}, x N^2/{n_sample}")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value * args.slices,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "slices_per_step": args.slices, "kind": "cpu oracle, extrapolated"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--slices", type=int, default=32, help="slices per step per GPU (configs[4]: 32)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--ref-sample", type=int, default=512)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+
+    import paper_1009_1380_b200 as rb
+    import workloads
+    from paper_1009_1380_b200 import dist as rdist
+
+    rb.lib()                                   # fail loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    rank, local_rank, world = rdist.init("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    cfg = workloads.get_config(4)
+    B = args.slices
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+
+    # synthetic slices (configs[4] recipe), distinct per rank; resident in HBM before timing
+    n_unique = min(B, 8)
+    uniq = np.stack([workloads.make_batch_slice(rank * B + i, cfg.N) for i in range(n_unique)])
+    hx = torch.from_numpy(np.concatenate([uniq] * ((B + n_unique - 1) // n_unique))[:B].copy())
+    # every slice distinct in memory (no aliasing): scale repeats slightly
+    for i in range(B):
+        hx[i] *= 1.0 + 1e-3 * (i // n_unique)
+    x = hx.to(dev)
+    sino = torch.empty((B, cfg.n_angles, cfg.n_det), dtype=torch.float32, device=dev)
+    xt = torch.empty_like(x)
+
+    def step():
+        plan.radon_forward_batch(x, sino)
+        plan.radon_adjoint_batch(sino, xt)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    plan.stage_times()                          # clear
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.stage_timing(True)
+    rdist.barrier(); torch.cuda.synchronize()
+    n0 = rb.kernel_launch_count()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize(); rdist.barrier()
+    launches = rb.kernel_launch_count() - n0
+    plan.stage_timing(False)
+    stages = plan.stage_times()
+    clocks = sampler.stop()
+    t_ms = rdist.max_over_ranks(ev0.elapsed_time(ev1), dev)
+    pairs = world * B * args.steps
+    value = pairs / (t_ms * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region ------------
+    e2e = None
+    if not args.no_e2e:
+        hxp = hx.pin_memory()
+        hs = torch.empty((B, cfg.n_angles, cfg.n_det), dtype=torch.float32).pin_memory()
+        hxt = torch.empty((B, cfg.N, cfg.N), dtype=torch.float32).pin_memory()
+
+        def step_host():
+            plan.radon_forward_host(hxp, hs)
+            plan.radon_adjoint_host(hs, hxt)
+
+        step_host()
+        rdist.barrier(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 3))
+        for _ in range(n_e2e):
+            step_host()
+        torch.cuda.synchronize()
+        dt = rdist.max_over_ranks(time.perf_counter() - t0, dev)
+        e2e = {"value": world * B * n_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(hxp.numel() * 4 + hs.numel() * 4),
+               "d2h_bytes_per_step": int(hs.numel() * 4 + hxt.numel() * 4),
+               "steps": n_e2e, "api": "radon_forward_host + radon_adjoint_host (pinned host buffers)"}
+
+    # ---- roofline of the dominant kernel (stage with the largest device time) -----------
+    peak, peak_src = measured_peaks()
+    sbytes = stage_bytes(cfg.N, plan.G, cfg.M)
+    per_stage = {}
+    for k, (ms, n) in stages.items():
+        if n:
+            us = ms / n * 1e3
+            per_stage[k] = {"us_per_launch": round(us, 2), "launches_timed": n,
+                            "algorithmic_MB": round(sbytes[k] / 1e6, 1),
+                            "GBps": round(sbytes[k] / (us * 1e-6) / 1e9, 1),
+                            "frac_of_hbm_peak": round(sbytes[k] / (us * 1e-6) / 1e9 / peak, 4)}
+    dom = max(per_stage, key=lambda k: per_stage[k]["us_per_launch"] * per_stage[k]["launches_timed"]) if per_stage else None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "ncu_dram_traffic.json")
+    if dom and os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(dom, {}).get("dram_bytes_per_launch")
+    roofline = None
+    if dom:
+        ach = per_stage[dom]["GBps"]
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                    "frac": round(ach / peak, 4), "traffic": traffic, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": sbytes[dom],
+                    "us_per_launch": per_stage[dom]["us_per_launch"]}
+
+    if rank != 0:
+        return 0
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        v, cores, dt = cpu_oracle_pairs_per_s(cfg, args.ref_sample)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"{args.ref_sample} sinogram entries + {args.ref_sample} pixels of one slice "
+                                  f"({dt:.1f} s of CPU work), closed-form O-direct, extrapolated linearly to M and N^2 outputs"}
+    t_pair_us = t_ms * 1e3 / (B * args.steps)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "slices_per_step_per_gpu": B, "parallelism": f"slice-parallel replicas x{world}",
+                   "l2": f"inputs {B * cfg.N * cfg.N * 4 / 1e6:.0f} MB/step cycle through HBM (> 126 MB L2); per-slice grid 134 MB > L2"},
+        "samples_per_s": 2.0 * cfg.M * value, "us_per_pair": t_pair_us,
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": roofline, "stages": per_stage, "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

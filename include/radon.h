@@ -121,6 +121,17 @@ int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *st
 int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream);
 int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *stream);
 
+/* Stage timing (measurement only).  While enabled, radon_forward / radon_adjoint (and the
+ * batch, host and nufft entry points) record one CUDA event on their stream at every stage
+ * boundary (pool of 8192 events; recording stops silently when it is full).
+ * radon_plan_stage_times waits for the last recorded event, adds the elapsed device time of
+ * every recorded stage to total_ms[stage] and its count to launches[stage], then clears the
+ * pool.  Stages: 0 de-apodise+pad+column FFT, 1 row FFT, 2 inverse gridding (gather),
+ * 3 projection inverse DFT, 4 projection DFT, 5 gridding (scatter + merge), 6 row inverse
+ * FFT, 7 column inverse FFT + crop + de-apodise. */
+int radon_plan_stage_timing(radon_plan *p, int enable);
+int radon_plan_stage_times(radon_plan *p, double total_ms[8], long long launches[8]);
+
 /* Any of the out pointers may be NULL.  workspace_bytes = device bytes the plan owns. */
 int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_det,
                     long long *M, size_t *workspace_bytes);

@@ -26,6 +26,8 @@ _SIGNATURES = {
     "radon_grid_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_proj_ifft": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_proj_fft": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_plan_stage_timing": (c_int, [c_void_p, c_int]),
+    "radon_plan_stage_times": (c_int, [c_void_p, P(ctypes.c_double), P(c_ll)]),
     "radon_plan_info": (c_int, [c_void_p, P(c_int), P(c_int), P(c_int), P(c_int), P(c_ll), P(c_size_t)]),
     "radon_plan_schedule_stats": (c_int, [c_void_p, P(c_ll), P(c_ll), P(c_int), P(c_ll), P(c_ll), P(c_int)]),
     "radon_schedule_selfcheck": (c_int, [c_int, c_int, c_int, c_float, c_int, P(c_ll)]),
@@ -155,6 +157,18 @@ class RadonPlan:
         _check(lib().radon_plan_schedule_stats(self._h, *v), "radon_plan_schedule_stats")
         k = ["gather_slots", "gather_filled", "gather_ctas", "scatter_slots", "scatter_filled", "scatter_ctas"]
         return {a: b.value for a, b in zip(k, v)}
+
+    STAGES = ("F1_colfft", "F2_rowfft", "F3_gather", "F4_proj_ifft",
+              "A1_proj_fft", "A2_scatter", "A3_rowifft", "A4_colifft")
+
+    def stage_timing(self, enable: bool):
+        _check(lib().radon_plan_stage_timing(self._h, int(enable)), "radon_plan_stage_timing")
+
+    def stage_times(self):
+        """{stage: (total_ms, launches)} accumulated since the last call (synchronises)."""
+        ms = (ctypes.c_double * 8)(); n = (c_ll * 8)()
+        _check(lib().radon_plan_stage_times(self._h, ms, n), "radon_plan_stage_times")
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(self.STAGES)}
 
     # -- the operators (same names as the C ABI) ------------------------------------------
     def radon_forward(self, x, sino=None):

@@ -30,7 +30,19 @@ struct Workspace {
     float *sino = nullptr;     // M       (host-buffer entry points only)
 };
 
+// Optional stage timing: one CUDA event at every stage boundary of forward / adjoint.
+struct StageTimer {
+    bool enabled = false;
+    std::vector<cudaEvent_t> ev;      // pool, created on first enable
+    std::vector<int> stage;           // stage id that STARTS at ev[i]; -1 = end of a sequence
+    size_t used = 0;
+    double acc_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+constexpr size_t STAGE_EVENT_POOL = 8192;
+
 struct radon_plan {
+    StageTimer timer;
     Geometry geo;
     DevicePlan dev;
     Workspace ws[2];
@@ -91,6 +103,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     cudaFree(d.gather_ctas); cudaFree(d.gather_slots); cudaFree(d.scatter_ctas); cudaFree(d.scatter_slots);
     cudaFree(d.merge_jobs); cudaFree(d.scratch);
     for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.img); cudaFree(w.sino); }
+    for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     for (int i = 0; i < 2; ++i) {
         if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
@@ -190,18 +203,34 @@ static int check_launch()
 }
 
 // ---- stage sequences ------------------------------------------------------------------
+// stage ids: 0 F1 colpass_fwd, 1 F2 rowpass_fwd, 2 F3 gather, 3 F4 proj_ifft,
+//            4 A1 proj_fft, 5 A2 scatter(+merge), 6 A3 rowpass_inv, 7 A4 colpass_inv
+static inline void mark(radon_plan *p, cudaStream_t st, int stage)
+{
+    StageTimer &t = p->timer;
+    if (!t.enabled || t.used >= t.ev.size()) return;
+    cudaEventRecord(t.ev[t.used], st);
+    t.stage[t.used++] = stage;
+}
+
 static int nufft2_ws(radon_plan *p, Workspace &w, const float *d_x, float2 *d_polar, cudaStream_t st)
 {
+    mark(p, st, 0);
     if (launch_fft2d_pass(0, p->dev, d_x, w.T, st)) return RADON_ECUDA;        // F1 + F2 (columns)
+    mark(p, st, 1);
     if (launch_fft2d_pass(1, p->dev, w.T, w.grid, st)) return RADON_ECUDA;     // F2 (rows)
+    mark(p, st, 2);
     if (launch_gather(p->dev, w.grid, d_polar, st)) return RADON_ECUDA;        // F3
     return check_launch();
 }
 
 static int nufft1_ws(radon_plan *p, Workspace &w, const float2 *d_polar, float *d_x, cudaStream_t st)
 {
+    mark(p, st, 5);
     if (launch_scatter(p->dev, d_polar, w.grid, st)) return RADON_ECUDA;       // A2
+    mark(p, st, 6);
     if (launch_fft2d_pass(2, p->dev, w.grid, w.T, st)) return RADON_ECUDA;     // A3 (rows)
+    mark(p, st, 7);
     if (launch_fft2d_pass(3, p->dev, w.T, d_x, st)) return RADON_ECUDA;        // A3 (columns) + A4
     return check_launch();
 }
@@ -210,16 +239,56 @@ static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_si
 {
     int rc = nufft2_ws(p, w, d_x, w.polar, st);
     if (rc) return rc;
+    mark(p, st, 3);
     if (launch_proj(true, p->dev, (const float *)w.polar, d_sino, st)) return RADON_ECUDA;   // F4
+    mark(p, st, -1);
     return check_launch();
 }
 
 static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st)
 {
+    mark(p, st, 4);
     if (launch_proj(false, p->dev, d_sino, (float *)w.polar, st)) return RADON_ECUDA;        // A1
     int rc = check_launch();
     if (rc) return rc;
-    return nufft1_ws(p, w, w.polar, d_x, st);
+    rc = nufft1_ws(p, w, w.polar, d_x, st);
+    mark(p, st, -1);
+    return rc;
+}
+
+extern "C" int radon_plan_stage_timing(radon_plan *p, int enable)
+{
+    if (!p) return RADON_EINVAL;
+    StageTimer &t = p->timer;
+    if (enable && t.ev.empty()) {
+        t.ev.resize(STAGE_EVENT_POOL);
+        t.stage.assign(STAGE_EVENT_POOL, -1);
+        for (auto &e : t.ev) CUDA_TRY(cudaEventCreate(&e));
+    }
+    t.enabled = enable != 0;
+    return RADON_OK;
+}
+
+extern "C" int radon_plan_stage_times(radon_plan *p, double total_ms[8], long long launches[8])
+{
+    if (!p) return RADON_EINVAL;
+    StageTimer &t = p->timer;
+    if (t.used) CUDA_TRY(cudaEventSynchronize(t.ev[t.used - 1]));
+    for (size_t i = 0; i + 1 < t.used; ++i) {
+        if (t.stage[i] < 0) continue;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, t.ev[i], t.ev[i + 1]) == cudaSuccess) {
+            t.acc_ms[t.stage[i]] += ms;
+            t.cnt[t.stage[i]] += 1;
+        }
+    }
+    t.used = 0;
+    for (int s = 0; s < 8; ++s) {
+        if (total_ms) total_ms[s] = t.acc_ms[s];
+        if (launches) launches[s] = t.cnt[s];
+        t.acc_ms[s] = 0; t.cnt[s] = 0;
+    }
+    return RADON_OK;
 }
 
 extern "C" int radon_forward(radon_plan *p, const float *d_x, float *d_sino, void *stream)
@@ -305,13 +374,17 @@ extern "C" int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x
 extern "C" int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, void *stream)
 {
     if (!p || !d_x || !d_polar) return RADON_EINVAL;
-    return nufft2_ws(p, p->ws[0], d_x, (float2 *)d_polar, (cudaStream_t)stream);
+    int rc = nufft2_ws(p, p->ws[0], d_x, (float2 *)d_polar, (cudaStream_t)stream);
+    mark(p, (cudaStream_t)stream, -1);
+    return rc;
 }
 
 extern "C" int radon_nufft1(radon_plan *p, const float *d_polar, float *d_x, void *stream)
 {
     if (!p || !d_x || !d_polar) return RADON_EINVAL;
-    return nufft1_ws(p, p->ws[0], (const float2 *)d_polar, d_x, (cudaStream_t)stream);
+    int rc = nufft1_ws(p, p->ws[0], (const float2 *)d_polar, d_x, (cudaStream_t)stream);
+    mark(p, (cudaStream_t)stream, -1);
+    return rc;
 }
 
 extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *stream)
