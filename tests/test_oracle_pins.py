@@ -315,3 +315,19 @@ def test_fast_algorithm_within_kernel_error_bound_of_exact_operator():
     x2 = RNG.standard_normal((64, 64)); y2 = RNG.standard_normal((90, 91))
     lhs = np.vdot(oracle.fast_forward(x2, 90, 91), y2); rhs = np.vdot(x2, oracle.fast_adjoint(y2, 64))
     assert abs(lhs - rhs) < 1e-11 * abs(lhs)
+
+
+def test_golden_regression_fixture():
+    """tests/golden/odirect_tiny.txt (written by make_golden.py from oracle/ only) still
+    matches: guards the oracle's arithmetic against accidental edits."""
+    import os
+    import sys
+
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, here)
+    import make_golden
+
+    ref = np.loadtxt(os.path.join(here, "odirect_tiny.txt"))
+    got = make_golden.compute()
+    assert ref.shape == got.shape
+    assert np.abs(ref - got).max() < 1e-12 * np.abs(ref).max()
