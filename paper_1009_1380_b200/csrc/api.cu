@@ -23,7 +23,7 @@ static thread_local std::string g_last_cuda_error;
     } while (0)
 
 struct Workspace {
-    float2 *T = nullptr;       // G x N intermediate of the 2-D FFT
+    float2 *T = nullptr;       // (G/2+1) x N Hermitian-half intermediate of the 2-D FFT
     float2 *grid = nullptr;    // G x G oversampled spectrum (centred)
     float2 *polar = nullptr;   // M polar samples
     float *img = nullptr;      // N x N   (host-buffer entry points only)
@@ -164,7 +164,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if ((rc = dev_alloc(p, &d.scratch, (size_t)sch.n_partial_slots * ST_X * ST_Y))) return rc;
     // workspace (two sets: the host-buffer entry points overlap copies with kernels)
     for (auto &w : p->ws) {
-        if ((rc = dev_alloc(p, &w.T, (size_t)G * N))) return rc;
+        if ((rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
         if ((rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
         if ((rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
     }
@@ -216,9 +216,9 @@ static inline void mark(radon_plan *p, cudaStream_t st, int stage)
 static int nufft2_ws(radon_plan *p, Workspace &w, const float *d_x, float2 *d_polar, cudaStream_t st)
 {
     mark(p, st, 0);
-    if (launch_fft2d_pass(0, p->dev, d_x, w.T, st)) return RADON_ECUDA;        // F1 + F2 (columns)
+    if (launch_fft2d_pass(0, p->dev, d_x, w.T, 0, st)) return RADON_ECUDA;        // F1 + F2 (columns)
     mark(p, st, 1);
-    if (launch_fft2d_pass(1, p->dev, w.T, w.grid, st)) return RADON_ECUDA;     // F2 (rows)
+    if (launch_fft2d_pass(1, p->dev, w.T, w.grid, 1, st)) return RADON_ECUDA;     // F2 (rows)
     mark(p, st, 2);
     if (launch_gather(p->dev, w.grid, d_polar, st)) return RADON_ECUDA;        // F3
     return check_launch();
@@ -229,9 +229,9 @@ static int nufft1_ws(radon_plan *p, Workspace &w, const float2 *d_polar, float *
     mark(p, st, 5);
     if (launch_scatter(p->dev, d_polar, w.grid, st)) return RADON_ECUDA;       // A2
     mark(p, st, 6);
-    if (launch_fft2d_pass(2, p->dev, w.grid, w.T, st)) return RADON_ECUDA;     // A3 (rows)
+    if (launch_fft2d_pass(2, p->dev, w.grid, w.T, 1, st)) return RADON_ECUDA;     // A3 (rows)
     mark(p, st, 7);
-    if (launch_fft2d_pass(3, p->dev, w.T, d_x, st)) return RADON_ECUDA;        // A3 (columns) + A4
+    if (launch_fft2d_pass(3, p->dev, w.T, d_x, 0, st)) return RADON_ECUDA;        // A3 (columns) + A4
     return check_launch();
 }
 

@@ -28,12 +28,42 @@ struct DevicePlan {
 bool fft_length_supported(int L);
 int init_kernel_attributes();
 long long launch_count();
+void count_launch();
+
+// Opt a kernel in to more than 48 KB of dynamic shared memory.
+template <typename F>
+static inline int set_smem(F kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+            return -1;
+    }
+    return 0;
+}
+
+// Dispatch a runtime power-of-two FFT length to a template instance (LL).
+#define RADON_FOR_L(L, BODY)                         \
+    switch (L) {                                     \
+    case 16: { constexpr int LL = 16; BODY } break;  \
+    case 32: { constexpr int LL = 32; BODY } break;  \
+    case 64: { constexpr int LL = 64; BODY } break;  \
+    case 128: { constexpr int LL = 128; BODY } break;    \
+    case 256: { constexpr int LL = 256; BODY } break;    \
+    case 512: { constexpr int LL = 512; BODY } break;    \
+    case 1024: { constexpr int LL = 1024; BODY } break;  \
+    case 2048: { constexpr int LL = 2048; BODY } break;  \
+    case 4096: { constexpr int LL = 4096; BODY } break;  \
+    case 8192: { constexpr int LL = 8192; BODY } break;  \
+    default: return -1;                              \
+    }
 
 // F3 / A2 (+ merge)
 int launch_gather(const DevicePlan &p, const float2 *grid, float2 *polar, cudaStream_t st);
 int launch_scatter(const DevicePlan &p, const float2 *polar, float2 *grid, cudaStream_t st);
-// which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid), 2 rowpass_inv (grid -> T), 3 colpass_inv (T -> x)
-int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, cudaStream_t st);
+// which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid; flag: also write the mirrored rows),
+// 2 rowpass_inv (grid -> T; flag: fold the mirrored rows in), 3 colpass_inv (T -> x).
+// T holds the rows ky = 0..G/2 only (Hermitian half), N complex each.
+int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st);
 // inv == false: sinogram -> polar (A1); inv == true: polar -> sinogram (F4)
 int launch_proj(bool inv, const DevicePlan &p, const float *in, float *out, cudaStream_t st);
 
