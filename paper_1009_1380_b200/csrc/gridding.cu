@@ -70,68 +70,135 @@ __device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__re
 }
 
 // =====================================================================================
+// Bulk asynchronous copies (TMA engine, sm_90+): global -> shared, completion on an mbarrier
+// =====================================================================================
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 16-byte aligned src/dst, bytes a multiple of 16
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// =====================================================================================
 // F3: inverse gridding (gather)
 // =====================================================================================
+// One CTA = one GT_X x GT_Y tile of the grid (+KH halo up/right) and up to GATHER_ROUND_CAP
+// rounds of 32 samples whose footprints start inside the tile.  The tile is staged by the
+// copy engine (one bulk copy per tile row, rows and columns wrapped mod G) while the warps
+// already fetch their first slots and evaluate the Kaiser-Bessel weights; the 36 taps of a
+// sample are 64-bit shared-memory loads that the plan-time schedule made conflict free.
 constexpr int GATHER_THREADS = GATHER_WARPS * 32;
 constexpr size_t LUT_SMEM = RADON_KB_LUT ? (size_t)LUT_S * LUT_ROW * sizeof(float) : 0;
-constexpr size_t GATHER_SMEM = (size_t)GT_ROWS * GT_PITCH * sizeof(float2) + LUT_SMEM;
+constexpr size_t GATHER_TILE_BYTES = (size_t)GT_ROWS * GT_PITCH * sizeof(float2);
+constexpr size_t GATHER_SMEM = GATHER_TILE_BYTES + LUT_SMEM;
+static_assert((GT_PITCH * sizeof(float2)) % 16 == 0 && GT_X % 2 == 0, "bulk copies need 16-byte rows");
 
-__global__ void __launch_bounds__(GATHER_THREADS, 2)
+__global__ void __launch_bounds__(GATHER_THREADS, GATHER_CTAS_PER_SM)
 gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
               const GatherCta *__restrict__ ctas, const Slot *__restrict__ slots,
               const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
               int G, int n_det)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float *s_lut = reinterpret_cast<float *>(smem_raw);
-    float2 *tile = reinterpret_cast<float2 *>(smem_raw + LUT_SMEM);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *tile = reinterpret_cast<float2 *>(smem_raw);
+    float *s_lut = reinterpret_cast<float *>(smem_raw + GATHER_TILE_BYTES);
+    __shared__ __align__(8) uint64_t bar;
 
     const GatherCta cta = ctas[blockIdx.x];
-    load_lut_to_smem(s_lut, g_lut);
-
-    // stage the tile (+KH halo up/right), indices wrap mod G
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int ly = warp; ly < GT_ROWS; ly += GATHER_WARPS) {
-        int gy = cta.ty0 + ly;
-        gy = gy % G;
-        const float2 *src = grid + (size_t)gy * G;
-        for (int lx = lane; lx < GT_PITCH; lx += 32) {
-            int gx = cta.tx0 + lx;
-            gx = gx % G;
-            tile[ly * GT_PITCH + lx] = __ldg(&src[gx]);
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    load_lut_to_smem(s_lut, g_lut);
+    __syncthreads();
+    if (warp == 0) {
+        if (lane == 0) mbar_expect_tx(&bar, (uint32_t)GATHER_TILE_BYTES);
+        __syncwarp();
+        for (int ly = lane; ly < GT_ROWS; ly += 32) {
+            const float2 *src = grid + (size_t)((cta.ty0 + ly) % G) * G;
+            float2 *dst = tile + ly * GT_PITCH;
+            int gx = cta.tx0, done = 0;                       // tx0 is even, G is even
+            while (done < GT_PITCH) {
+                const int n = min(GT_PITCH - done, G - gx);
+                bulk_g2s(dst + done, src + gx, (uint32_t)(n * sizeof(float2)), &bar);
+                done += n;
+                gx = 0;
+            }
         }
     }
-    __syncthreads();
 
     const int cd = n_det / 2;
     const double halfG = 0.5 * (double)G;
-    for (int r = warp; r < cta.round_count; r += GATHER_WARPS) {
-        const Slot sl = slots[(size_t)(cta.round_begin + r) * 32 + lane];
-        if (sl.ak == SLOT_EMPTY) continue;
-        const int a = sl.ak >> 16, k = sl.ak & 0xffff;
+    const Slot *my = slots + (size_t)cta.round_begin * 32 + lane;
+    int r = warp;
+    Slot sl;
+    sl.ak = SLOT_EMPTY; sl.lxy = 0;
+    if (r < cta.round_count) sl = my[(size_t)r * 32];
+    bool staged = false;
+    while (r < cta.round_count) {
+        const int rn = r + GATHER_WARPS;
+        Slot nx;
+        nx.ak = SLOT_EMPTY; nx.lxy = 0;
+        if (rn < cta.round_count) nx = my[(size_t)rn * 32];
+        const bool act = sl.ak != SLOT_EMPTY;
+        const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
         Taps tp;
         sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
-        const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
-        float accr = 0.f, acci = 0.f;
+        if (!staged) { mbar_wait(&bar, 0); staged = true; }
+        if (act) {
+            const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
+            float accr = 0.f, acci = 0.f;
 #pragma unroll
-        for (int ly = 0; ly < KW; ++ly) {
-            float rr = 0.f, ri = 0.f;
+            for (int ly = 0; ly < KW; ++ly) {
+                float rr = 0.f, ri = 0.f;
 #pragma unroll
-            for (int lx = 0; lx < KW; ++lx) {
-                const float2 v = base[ly * GT_PITCH + lx];
-                rr = fmaf(v.x, tp.wx[lx], rr);
-                ri = fmaf(v.y, tp.wx[lx], ri);
+                for (int lx = 0; lx < KW; ++lx) {
+                    const float2 v = base[ly * GT_PITCH + lx];
+                    rr = fmaf(v.x, tp.wx[lx], rr);
+                    ri = fmaf(v.y, tp.wx[lx], ri);
+                }
+                accr = fmaf(rr, tp.wy[ly], accr);
+                acci = fmaf(ri, tp.wy[ly], acci);
             }
-            accr = fmaf(rr, tp.wy[ly], accr);
-            acci = fmaf(ri, tp.wy[ly], acci);
+            polar[(size_t)a * n_det + k] = make_float2(accr, acci);
         }
-        polar[(size_t)a * n_det + k] = make_float2(accr, acci);
+        sl = nx;
+        r = rn;
     }
+    // a CTA must not exit while bulk copies into its shared memory are in flight
+    if (!staged) mbar_wait(&bar, 0);
 }
 
 // =====================================================================================
 // A2: gridding (scatter) -- warp-private accumulators, conflict-free rounds, fixed-order merge
 // =====================================================================================
+// A warp accumulates its samples into a private (ST_X + 2 KH) x (ST_Y + 2 KH) shared-memory
+// array with plain load / FMA / store: no atomics, every addition in a fixed order (bitwise
+// reproducible).  A round is 32 samples, one per lane, processed one footprint ROW at a time
+// (W loads, 2 W FMAs, W stores, warp barrier); the plan-time schedule guarantees that within
+// a row step no two lanes touch the same cell and that every 64-bit access of a half-warp is
+// bank-conflict free.  Slots and sample values are prefetched one round ahead.
 constexpr int SCATTER_THREADS = SCATTER_ITEMS * 32;
 constexpr int SP_CELLS = SP_H * SP_PITCH;
 constexpr size_t SCATTER_SMEM = (size_t)SCATTER_ITEMS * SP_CELLS * sizeof(float2) + LUT_SMEM;
@@ -142,19 +209,14 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
                const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
                int G, int n_det)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float *s_lut = reinterpret_cast<float *>(smem_raw);
-    float2 *priv = reinterpret_cast<float2 *>(smem_raw + LUT_SMEM);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *priv = reinterpret_cast<float2 *>(smem_raw);
+    float *s_lut = reinterpret_cast<float *>(smem_raw + (size_t)SCATTER_ITEMS * SP_CELLS * sizeof(float2));
     __shared__ ScatterCta cta;
 
     if (threadIdx.x < sizeof(ScatterCta) / 4)
         reinterpret_cast<int *>(&cta)[threadIdx.x] = reinterpret_cast<const int *>(&ctas[blockIdx.x])[threadIdx.x];
     load_lut_to_smem(s_lut, g_lut);
-    {
-        float4 *z = reinterpret_cast<float4 *>(priv);
-        for (int i = threadIdx.x; i < SCATTER_ITEMS * SP_CELLS / 2; i += SCATTER_THREADS)
-            z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
     __syncthreads();
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -163,27 +225,49 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     {
         const ScatterItem item = cta.items[warp];
         float2 *mine = priv + warp * SP_CELLS;
-        for (int r = 0; r < item.round_count; ++r) {
-            const Slot sl = slots[(size_t)(item.round_begin + r) * 32 + lane];
-            if (sl.ak != SLOT_EMPTY) {
-                const int a = sl.ak >> 16, k = sl.ak & 0xffff;
-                Taps tp;
-                sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
-                const float2 val = __ldg(&polar[(size_t)a * n_det + k]);
-                float2 *base = mine + (sl.lxy >> 16) * SP_PITCH + (sl.lxy & 0xffff);
+        const Slot *my = slots + (size_t)item.round_begin * 32 + lane;
+        const int nr = item.round_count;
+        // prefetch: slot of round 0 and 1, value of round 0
+        Slot s0, s1;
+        s0.ak = SLOT_EMPTY; s0.lxy = 0; s1 = s0;
+        if (nr > 0) s0 = my[0];
+        if (nr > 1) s1 = my[32];
+        {   // zero the private accumulator while the first loads are in flight
+            float4 *z = reinterpret_cast<float4 *>(mine);
+            for (int i = lane; i < SP_CELLS / 2; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        float2 v0 = make_float2(0.f, 0.f);
+        if (s0.ak != SLOT_EMPTY) v0 = __ldg(&polar[(size_t)(s0.ak >> 16) * n_det + (s0.ak & 0xffff)]);
+        __syncwarp();
+        for (int r = 0; r < nr; ++r) {
+            Slot s2;
+            s2.ak = SLOT_EMPTY; s2.lxy = 0;
+            if (r + 2 < nr) s2 = my[(size_t)(r + 2) * 32];
+            float2 v1 = make_float2(0.f, 0.f);
+            if (s1.ak != SLOT_EMPTY) v1 = __ldg(&polar[(size_t)(s1.ak >> 16) * n_det + (s1.ak & 0xffff)]);
+            const bool act = s0.ak != SLOT_EMPTY;
+            const int a = act ? (int)(s0.ak >> 16) : 0, k = act ? (int)(s0.ak & 0xffff) : 0;
+            Taps tp;
+            sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
+            float2 *base = mine + (s0.lxy >> 16) * SP_PITCH + (s0.lxy & 0xffff);
 #pragma unroll
-                for (int ly = 0; ly < KW; ++ly) {
-                    const float vr = val.x * tp.wy[ly], vi = val.y * tp.wy[ly];
+            for (int ly = 0; ly < KW; ++ly) {
+                if (act) {
+                    const float vr = v0.x * tp.wy[ly], vi = v0.y * tp.wy[ly];
+                    float2 c[KW];
+#pragma unroll
+                    for (int lx = 0; lx < KW; ++lx) c[lx] = base[ly * SP_PITCH + lx];
 #pragma unroll
                     for (int lx = 0; lx < KW; ++lx) {
-                        float2 c = base[ly * SP_PITCH + lx];
-                        c.x = fmaf(vr, tp.wx[lx], c.x);
-                        c.y = fmaf(vi, tp.wx[lx], c.y);
-                        base[ly * SP_PITCH + lx] = c;
+                        c[lx].x = fmaf(vr, tp.wx[lx], c[lx].x);
+                        c[lx].y = fmaf(vi, tp.wx[lx], c[lx].y);
                     }
+#pragma unroll
+                    for (int lx = 0; lx < KW; ++lx) base[ly * SP_PITCH + lx] = c[lx];
                 }
+                __syncwarp();   // row steps of different lanes may touch the same cells
             }
-            __syncwarp();   // footprints of one round are disjoint; rounds must not overlap in time
+            s0 = s1; s1 = s2; v0 = v1;
         }
     }
     __syncthreads();
@@ -210,21 +294,26 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     }
 }
 
-__global__ void __launch_bounds__(256)
+// Fixed-order sum of the partial rectangles of a split (heavy) sub-tile: one thread per cell.
+constexpr int MERGE_THREADS = 256;
+constexpr int MERGE_CHUNKS = (ST_X * ST_Y + MERGE_THREADS - 1) / MERGE_THREADS;
+__global__ void __launch_bounds__(MERGE_THREADS)
 merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
              const MergeJob *__restrict__ jobs, int G)
 {
-    const MergeJob j = jobs[blockIdx.x];
-    for (int i = threadIdx.x; i < j.rw * j.rh; i += blockDim.x) {
-        const int y = i / j.rw, x = i - y * j.rw;
-        float sr = 0.f, si = 0.f;
-        for (int s = 0; s < j.n_slots; ++s) {
-            const float2 c = scratch[(size_t)(j.first_slot + s) * (ST_X * ST_Y) + y * ST_X + x];
-            sr += c.x;
-            si += c.y;
-        }
-        grid[(size_t)(j.ry0 + y) * G + j.rx0 + x] = make_float2(sr, si);
+    const MergeJob j = jobs[blockIdx.x / MERGE_CHUNKS];
+    const int i = (blockIdx.x % MERGE_CHUNKS) * MERGE_THREADS + threadIdx.x;
+    if (i >= j.rw * j.rh) return;
+    const int y = i / j.rw, x = i - y * j.rw;
+    const float2 *src = scratch + (size_t)j.first_slot * (ST_X * ST_Y) + y * ST_X + x;
+    float sr = 0.f, si = 0.f;
+#pragma unroll 4
+    for (int s = 0; s < j.n_slots; ++s) {
+        const float2 c = __ldg(&src[(size_t)s * (ST_X * ST_Y)]);
+        sr += c.x;
+        si += c.y;
     }
+    grid[(size_t)(j.ry0 + y) * G + j.rx0 + x] = make_float2(sr, si);
 }
 
 int launch_gather(const DevicePlan &p, const float2 *grid, float2 *polar, cudaStream_t st)
@@ -242,7 +331,7 @@ int launch_scatter(const DevicePlan &p, const float2 *polar, float2 *grid, cudaS
         polar, grid, p.scratch, p.scatter_ctas, p.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
     count_launch();
     if (p.n_merge_jobs > 0) {
-        merge_kernel<<<p.n_merge_jobs, 256, 0, st>>>(p.scratch, grid, p.merge_jobs, p.G);
+        merge_kernel<<<p.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(p.scratch, grid, p.merge_jobs, p.G);
         count_launch();
     }
     return 0;

@@ -235,26 +235,23 @@ struct Cand {
     int16_t lx, ly;
 };
 
-struct Occupancy {          // bitmap of up to 128 x 64 cells
+// Which base cells a new sample of the round may NOT take.  The scatter kernel accumulates a
+// footprint one ROW at a time (W loads, W FMAs, W stores, then a warp barrier), so two lanes
+// only collide if they touch the same cells within one row step: same base row and base
+// columns closer than W.  (Footprints of a round may overlap otherwise: lane i's row step l
+// and lane j's row step l' != l are separated by a barrier.)
+struct Occupancy {          // one bitmap row per base row, up to 128 base columns
     uint64_t rows[SP_H > GT_ROWS ? SP_H : GT_ROWS][2];
     void clear() { std::memset(rows, 0, sizeof(rows)); }
-    static inline void span(int lx, uint64_t &m0, uint64_t &m1)
-    {
-        // KW consecutive bits starting at lx (lx + KW <= 128)
-        const unsigned __int128 m = ((((unsigned __int128)1) << KW) - 1) << lx;
-        m0 = (uint64_t)m; m1 = (uint64_t)(m >> 64);
-    }
     bool overlaps(int lx, int ly) const
     {
-        uint64_t m0, m1; span(lx, m0, m1);
-        for (int r = 0; r < KW; ++r)
-            if ((rows[ly + r][0] & m0) | (rows[ly + r][1] & m1)) return true;
-        return false;
+        return (lx < 64 ? (rows[ly][0] >> lx) : (rows[ly][1] >> (lx - 64))) & 1u;
     }
     void mark(int lx, int ly)
     {
-        uint64_t m0, m1; span(lx, m0, m1);
-        for (int r = 0; r < KW; ++r) { rows[ly + r][0] |= m0; rows[ly + r][1] |= m1; }
+        const int lo = std::max(lx - KH, 0), hi = std::min(lx + KH, 127);
+        unsigned __int128 m = ((((unsigned __int128)1) << (hi - lo + 1)) - 1) << lo;
+        rows[ly][0] |= (uint64_t)m; rows[ly][1] |= (uint64_t)(m >> 64);
     }
 };
 
@@ -527,23 +524,20 @@ long long check_schedules(const Geometry &g, const Schedules &s)
     const int G = g.G;
     const long long M = (long long)g.n_angles * g.n_det;
 
+    // Pairwise (brute force, independent of the builder's bitmap): bank pairs distinct per
+    // half-warp; for the scatter, no two lanes of a round with the same base row and base
+    // columns closer than W (the kernel's row-step rule), and every footprint inside the
+    // accumulator.
     auto check_round = [&](const Slot *lanes, int pitch, bool disjoint) {
-        Occupancy occ;
-        occ.clear();
-        for (int h = 0; h < 2; ++h) {
-            uint32_t mask = 0;
-            for (int l = 0; l < 16; ++l) {
-                const Slot &sl = lanes[h * 16 + l];
-                if (sl.ak == SLOT_EMPTY) continue;
-                const int lx = sl.lxy & 0xffff, ly = sl.lxy >> 16;
-                const uint32_t res = 1u << ((ly * pitch + lx) & 15);
-                if (mask & res) ++bad;
-                mask |= res;
-                if (disjoint) {
-                    if (lx + KW > SP_W || ly + KW > SP_H) { ++bad; continue; }
-                    if (occ.overlaps(lx, ly)) ++bad;
-                    occ.mark(lx, ly);
-                }
+        for (int i = 0; i < 32; ++i) {
+            if (lanes[i].ak == SLOT_EMPTY) continue;
+            const int xi = lanes[i].lxy & 0xffff, yi = lanes[i].lxy >> 16;
+            if (disjoint && (xi + KW > SP_W || yi + KW > SP_H)) ++bad;
+            for (int j = i + 1; j < 32; ++j) {
+                if (lanes[j].ak == SLOT_EMPTY) continue;
+                const int xj = lanes[j].lxy & 0xffff, yj = lanes[j].lxy >> 16;
+                if ((i >> 4) == (j >> 4) && ((yi * pitch + xi) & 15) == ((yj * pitch + xj) & 15)) ++bad;
+                if (disjoint && yi == yj && std::abs(xi - xj) < KW) ++bad;
             }
         }
     };

@@ -56,9 +56,10 @@ constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, 
 
 // Gather (inverse gridding): one CTA stages a GT_X x GT_Y tile of the grid (+halo).
 constexpr int GT_X = 128, GT_Y = 64;
-constexpr int GT_PITCH = GT_X + KH;   // 133 complex per smem row (odd: spreads bank pairs)
+constexpr int GT_PITCH = GT_X + KH + 1;   // 134 complex per smem row: 16-byte multiple for the bulk copies
 constexpr int GT_ROWS = GT_Y + KH;    // 69
 constexpr int GATHER_WARPS = 8;
+constexpr int GATHER_CTAS_PER_SM = 3;
 constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
 
 // Scatter (gridding): each warp owns a private accumulator of one ST_X x ST_Y sub-tile
