@@ -161,7 +161,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if ((rc = dev_upload(p, &d.scatter_ctas, sch.scatter_ctas))) return rc;
     if ((rc = dev_upload(p, &d.scatter_slots, sch.scatter_slots))) return rc;
     if ((rc = dev_upload(p, &d.merge_jobs, sch.merge_jobs))) return rc;
-    if ((rc = dev_alloc(p, &d.scratch, (size_t)sch.n_partial_slots * ST_X * ST_Y))) return rc;
+    if ((rc = dev_alloc(p, &d.scratch, (size_t)sch.n_partial_slots * SR_X * SR_Y))) return rc;
     // workspace (two sets: the host-buffer entry points overlap copies with kernels)
     for (auto &w : p->ws) {
         if ((rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;

@@ -191,27 +191,37 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
 }
 
 // =====================================================================================
-// A2: gridding (scatter) -- warp-private accumulators, conflict-free rounds, fixed-order merge
+// A2: gridding (scatter) -- CTA-local accumulation in shared memory, no atomics
 // =====================================================================================
-// A warp accumulates its samples into a private (ST_X + 2 KH) x (ST_Y + 2 KH) shared-memory
-// array with plain load / FMA / store: no atomics, every addition in a fixed order (bitwise
-// reproducible).  A round is 32 samples, one per lane, processed one footprint ROW at a time
-// (W loads, 2 W FMAs, W stores, warp barrier); the plan-time schedule guarantees that within
-// a row step no two lanes touch the same cell and that every 64-bit access of a half-warp is
-// bank-conflict free.  Slots and sample values are prefetched one round ahead.
+// A CTA accumulates one SR_X x SR_Y output rectangle in shared memory.  Each warp owns one
+// quadrant of it and processes, in rounds of 32 (one sample per lane), every sample whose
+// footprint intersects the quadrant, with plain load / FMA / store and the taps clipped to the
+// quadrant: warps never share a cell, so there are no atomics and every addition happens in
+// a fixed order (bitwise reproducible).  A footprint is processed one ROW at a time (W loads,
+// W packed FMAs, W stores, warp barrier); the plan-time schedule guarantees that within a
+// row step no two lanes touch the same cell and that every 64-bit access of a half-warp is
+// bank-conflict free.  Slots and sample values are prefetched ahead of use.  The finished
+// rectangle leaves through the copy engine (bulk shared -> global stores, one per row).
 constexpr int SCATTER_THREADS = SCATTER_ITEMS * 32;
-constexpr int SP_CELLS = SP_H * SP_PITCH;
-constexpr size_t SCATTER_SMEM = (size_t)SCATTER_ITEMS * SP_CELLS * sizeof(float2) + LUT_SMEM;
+constexpr size_t SCATTER_ACC_BYTES = (size_t)SR_Y * ACC_PITCH * sizeof(float2);
+constexpr size_t SCATTER_SMEM = SCATTER_ACC_BYTES + LUT_SMEM;
+static_assert((ACC_PITCH * sizeof(float2)) % 16 == 0, "bulk stores need 16-byte rows");
 
-__global__ void __launch_bounds__(SCATTER_THREADS, 2)
+__device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+
+__global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
                const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
                int G, int n_det)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2 *priv = reinterpret_cast<float2 *>(smem_raw);
-    float *s_lut = reinterpret_cast<float *>(smem_raw + (size_t)SCATTER_ITEMS * SP_CELLS * sizeof(float2));
+    float2 *acc = reinterpret_cast<float2 *>(smem_raw);
+    float *s_lut = reinterpret_cast<float *>(smem_raw + SCATTER_ACC_BYTES);
     __shared__ ScatterCta cta;
 
     if (threadIdx.x < sizeof(ScatterCta) / 4)
@@ -222,81 +232,79 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int cd = n_det / 2;
     const double halfG = 0.5 * (double)G;
-    {
-        const ScatterItem item = cta.items[warp];
-        float2 *mine = priv + warp * SP_CELLS;
-        const Slot *my = slots + (size_t)item.round_begin * 32 + lane;
-        const int nr = item.round_count;
-        // prefetch: slot of round 0 and 1, value of round 0
-        Slot s0, s1;
-        s0.ak = SLOT_EMPTY; s0.lxy = 0; s1 = s0;
-        if (nr > 0) s0 = my[0];
-        if (nr > 1) s1 = my[32];
-        {   // zero the private accumulator while the first loads are in flight
-            float4 *z = reinterpret_cast<float4 *>(mine);
-            for (int i = lane; i < SP_CELLS / 2; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        float2 v0 = make_float2(0.f, 0.f);
-        if (s0.ak != SLOT_EMPTY) v0 = __ldg(&polar[(size_t)(s0.ak >> 16) * n_det + (s0.ak & 0xffff)]);
-        __syncwarp();
-        for (int r = 0; r < nr; ++r) {
-            Slot s2;
-            s2.ak = SLOT_EMPTY; s2.lxy = 0;
-            if (r + 2 < nr) s2 = my[(size_t)(r + 2) * 32];
-            float2 v1 = make_float2(0.f, 0.f);
-            if (s1.ak != SLOT_EMPTY) v1 = __ldg(&polar[(size_t)(s1.ak >> 16) * n_det + (s1.ak & 0xffff)]);
-            const bool act = s0.ak != SLOT_EMPTY;
-            const int a = act ? (int)(s0.ak >> 16) : 0, k = act ? (int)(s0.ak & 0xffff) : 0;
-            Taps tp;
-            sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
-            float2 *base = mine + (s0.lxy >> 16) * SP_PITCH + (s0.lxy & 0xffff);
-#pragma unroll
-            for (int ly = 0; ly < KW; ++ly) {
-                if (act) {
-                    const float vr = v0.x * tp.wy[ly], vi = v0.y * tp.wy[ly];
-                    float2 c[KW];
-#pragma unroll
-                    for (int lx = 0; lx < KW; ++lx) c[lx] = base[ly * SP_PITCH + lx];
-#pragma unroll
-                    for (int lx = 0; lx < KW; ++lx) {
-                        c[lx].x = fmaf(vr, tp.wx[lx], c[lx].x);
-                        c[lx].y = fmaf(vi, tp.wx[lx], c[lx].y);
-                    }
-#pragma unroll
-                    for (int lx = 0; lx < KW; ++lx) base[ly * SP_PITCH + lx] = c[lx];
-                }
-                __syncwarp();   // row steps of different lanes may touch the same cells
-            }
-            s0 = s1; s1 = s2; v0 = v1;
-        }
+    const ScatterItem item = cta.items[warp];
+    const Slot *my = slots + (size_t)item.round_begin * 32 + lane;
+    const int nr = item.round_count;
+    // prefetch: slots of rounds 0 and 1, value of round 0
+    Slot s0, s1;
+    s0.ak = SLOT_EMPTY; s0.lxy = 0; s1 = s0;
+    if (nr > 0) s0 = my[0];
+    if (nr > 1) s1 = my[32];
+    {   // zero the accumulator while those loads are in flight
+        float4 *z = reinterpret_cast<float4 *>(acc);
+        for (int i = threadIdx.x; i < (int)(SCATTER_ACC_BYTES / 16); i += SCATTER_THREADS)
+            z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
+    float2 v0 = make_float2(0.f, 0.f);
+    if (s0.ak != SLOT_EMPTY) v0 = __ldg(&polar[(size_t)(s0.ak >> 16) * n_det + (s0.ak & 0xffff)]);
     __syncthreads();
 
-    // merge the warps' accumulators in warp order and write the rectangle exactly once
+    float2 *origin = acc + (item.sy0 - KH) * ACC_PITCH + (item.sx0 - KH);   // slot (0,0); never dereferenced outside the quadrant
+    for (int r = 0; r < nr; ++r) {
+        Slot s2;
+        s2.ak = SLOT_EMPTY; s2.lxy = 0;
+        if (r + 2 < nr) s2 = my[(size_t)(r + 2) * 32];
+        float2 v1 = make_float2(0.f, 0.f);
+        if (s1.ak != SLOT_EMPTY) v1 = __ldg(&polar[(size_t)(s1.ak >> 16) * n_det + (s1.ak & 0xffff)]);
+        const bool act = s0.ak != SLOT_EMPTY;
+        const int a = act ? (int)(s0.ak >> 16) : 0, k = act ? (int)(s0.ak & 0xffff) : 0;
+        Taps tp;
+        sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
+        const int bx = (int)(s0.lxy & 0xffff), by = (int)(s0.lxy >> 16);   // biased by KH
+        float2 *base = origin + by * ACC_PITCH + bx;
+        // taps inside the quadrant: KH <= bx + lx < KH + sw, likewise rows
+        const int xlo = KH - bx, xhi = KH + item.sw - bx, ylo = KH - by, yhi = KH + item.sh - by;
+        bool px[KW];
+#pragma unroll
+        for (int lx = 0; lx < KW; ++lx) px[lx] = act && lx >= xlo && lx < xhi;
+#pragma unroll
+        for (int ly = 0; ly < KW; ++ly) {
+            if (ly >= ylo && ly < yhi) {
+                const float vr = v0.x * tp.wy[ly], vi = v0.y * tp.wy[ly];
+                float2 c[KW];
+#pragma unroll
+                for (int lx = 0; lx < KW; ++lx)
+                    if (px[lx]) c[lx] = base[ly * ACC_PITCH + lx];
+#pragma unroll
+                for (int lx = 0; lx < KW; ++lx) {
+                    c[lx].x = fmaf(vr, tp.wx[lx], c[lx].x);
+                    c[lx].y = fmaf(vi, tp.wx[lx], c[lx].y);
+                }
+#pragma unroll
+                for (int lx = 0; lx < KW; ++lx)
+                    if (px[lx]) base[ly * ACC_PITCH + lx] = c[lx];
+            }
+            __syncwarp();   // row steps of different lanes may touch the same cells
+        }
+        s0 = s1; s1 = s2; v0 = v1;
+    }
+
+    // flush: the rectangle is written exactly once, by the copy engine
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> async proxy
+    __syncthreads();
     float2 *dst;
     int dpitch;
-    if (cta.partial_slot >= 0) { dst = scratch + (size_t)cta.partial_slot * (ST_X * ST_Y); dpitch = ST_X; }
+    if (cta.partial_slot >= 0) { dst = scratch + (size_t)cta.partial_slot * (SR_X * SR_Y); dpitch = SR_X; }
     else { dst = grid + (size_t)cta.ry0 * G + cta.rx0; dpitch = G; }
-    const int cells = cta.rw * cta.rh;
-    for (int i = threadIdx.x; i < cells; i += SCATTER_THREADS) {
-        const int y = i / cta.rw, x = i - y * cta.rw;
-        float sr = 0.f, si = 0.f;
-#pragma unroll
-        for (int it = 0; it < SCATTER_ITEMS; ++it) {
-            const int lx = cta.rx0 + x - cta.items[it].px0, ly = cta.ry0 + y - cta.items[it].py0;
-            if (cta.items[it].round_count > 0 && (unsigned)lx < (unsigned)SP_W && (unsigned)ly < (unsigned)SP_H) {
-                const float2 c = priv[it * SP_CELLS + ly * SP_PITCH + lx];
-                sr += c.x;
-                si += c.y;
-            }
-        }
-        dst[(size_t)y * dpitch + x] = make_float2(sr, si);
-    }
+    if (threadIdx.x < cta.rh)
+        bulk_s2g(dst + (size_t)threadIdx.x * dpitch, acc + threadIdx.x * ACC_PITCH, (uint32_t)(cta.rw * sizeof(float2)));
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the reads
 }
 
-// Fixed-order sum of the partial rectangles of a split (heavy) sub-tile: one thread per cell.
+// Fixed-order sum of the partial rectangles of a split (heavy) rectangle: one thread per cell.
 constexpr int MERGE_THREADS = 256;
-constexpr int MERGE_CHUNKS = (ST_X * ST_Y + MERGE_THREADS - 1) / MERGE_THREADS;
+constexpr int MERGE_CHUNKS = (SR_X * SR_Y + MERGE_THREADS - 1) / MERGE_THREADS;
 __global__ void __launch_bounds__(MERGE_THREADS)
 merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
              const MergeJob *__restrict__ jobs, int G)
@@ -305,11 +313,11 @@ merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
     const int i = (blockIdx.x % MERGE_CHUNKS) * MERGE_THREADS + threadIdx.x;
     if (i >= j.rw * j.rh) return;
     const int y = i / j.rw, x = i - y * j.rw;
-    const float2 *src = scratch + (size_t)j.first_slot * (ST_X * ST_Y) + y * ST_X + x;
+    const float2 *src = scratch + (size_t)j.first_slot * (SR_X * SR_Y) + y * SR_X + x;
     float sr = 0.f, si = 0.f;
 #pragma unroll 4
     for (int s = 0; s < j.n_slots; ++s) {
-        const float2 c = __ldg(&src[(size_t)s * (ST_X * ST_Y)]);
+        const float2 c = __ldg(&src[(size_t)s * (SR_X * SR_Y)]);
         sr += c.x;
         si += c.y;
     }

@@ -241,7 +241,7 @@ struct Cand {
 // columns closer than W.  (Footprints of a round may overlap otherwise: lane i's row step l
 // and lane j's row step l' != l are separated by a barrier.)
 struct Occupancy {          // one bitmap row per base row, up to 128 base columns
-    uint64_t rows[SP_H > GT_ROWS ? SP_H : GT_ROWS][2];
+    uint64_t rows[SB_H > GT_ROWS ? SB_H : GT_ROWS][2];
     void clear() { std::memset(rows, 0, sizeof(rows)); }
     bool overlaps(int lx, int ly) const
     {
@@ -385,7 +385,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
 
     struct Pending { ScatterCta cta; long long work; };
     std::vector<Pending> ctas;
-    std::vector<Cand> item_c[SCATTER_ITEMS];
+    std::vector<Cand> quad[SCATTER_ITEMS];
     std::vector<Slot> tmp_slots;
 
     for (int r = 0; r < nrect; ++r) {
@@ -394,108 +394,75 @@ static void build_scatter(const Geometry &g, Schedules &out)
         const int nsx = (rw + ST_X - 1) / ST_X, nsy = (rh + ST_Y - 1) / ST_Y;
         const uint32_t lo = count[r], hi = count[r + 1];
 
-        // --- try the light layout: one warp per sub-tile -------------------------
-        for (auto &v : item_c) v.clear();
-        for (uint32_t q = lo; q < hi; ++q) {
-            const Image &im = inc[q];
-            const int ix = std::min(std::max(floordiv(im.bx - rx0, ST_X), 0), nsx - 1);
-            const int iy = std::min(std::max(floordiv(im.by - ry0, ST_Y), 0), nsy - 1);
-            Cand c;
-            c.ak = im.ak;
-            c.lx = (int16_t)(im.bx - (rx0 + ix * ST_X - KH));
-            c.ly = (int16_t)(im.by - (ry0 + iy * ST_Y - KH));
-            item_c[iy * 2 + ix].push_back(c);
-        }
-        Pending p;
-        std::memset(&p.cta, 0, sizeof(p.cta));
-        p.cta.rx0 = rx0; p.cta.ry0 = ry0; p.cta.rw = rw; p.cta.rh = rh; p.cta.partial_slot = -1;
-        tmp_slots.clear();
-        long long tmp_filled = 0;
-        int max_rounds = 0, tmp_rounds[SCATTER_ITEMS], tmp_begin[SCATTER_ITEMS];
-        for (int it = 0; it < SCATTER_ITEMS; ++it) {
-            tmp_begin[it] = (int)(tmp_slots.size() / 32);
-            tmp_rounds[it] = build_rounds(item_c[it], true, SP_PITCH, tmp_slots, tmp_filled);
-            max_rounds = std::max(max_rounds, tmp_rounds[it]);
-        }
-        if (max_rounds <= SCATTER_ROUND_MAX) {
-            const int base = (int)(out.scatter_slots.size() / 32);
-            out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
-            out.scatter_filled += tmp_filled;
-            p.work = 0;
-            for (int it = 0; it < SCATTER_ITEMS; ++it) {
-                const int ix = it % 2, iy = it / 2;
-                p.cta.items[it].px0 = rx0 + ix * ST_X - KH;
-                p.cta.items[it].py0 = ry0 + iy * ST_Y - KH;
-                p.cta.items[it].round_begin = base + tmp_begin[it];
-                p.cta.items[it].round_count = tmp_rounds[it];
-                p.work = std::max<long long>(p.work, tmp_rounds[it]);
-            }
-            ctas.push_back(p);
-            continue;
-        }
-
-        // --- heavy rectangle: one output rectangle per sub-tile, samples dealt ------
-        // round-robin over 4*K warps that all cover the same sub-tile.
+        // quadrants of the rectangle and, for each, every sample image whose footprint
+        // intersects it (a sample near a quadrant border is listed in both: each warp applies
+        // only the taps inside its own quadrant)
+        ScatterItem geom[SCATTER_ITEMS];
+        std::memset(geom, 0, sizeof(geom));
+        for (auto &v : quad) v.clear();
         for (int iy = 0; iy < nsy; ++iy)
             for (int ix = 0; ix < nsx; ++ix) {
-                const int sx0 = rx0 + ix * ST_X, sy0 = ry0 + iy * ST_Y;
-                const int sw = std::min(ST_X, rx0 + rw - sx0), sh = std::min(ST_Y, ry0 + rh - sy0);
-                std::vector<Cand> sub;
+                ScatterItem &I = geom[iy * 2 + ix];
+                I.sx0 = ix * ST_X; I.sy0 = iy * ST_Y;
+                I.sw = std::min(ST_X, rw - I.sx0); I.sh = std::min(ST_Y, rh - I.sy0);
+                const int ax0 = rx0 + I.sx0, ay0 = ry0 + I.sy0;          // absolute origin
                 for (uint32_t q = lo; q < hi; ++q) {
                     const Image &im = inc[q];
-                    if (im.bx + KH < sx0 || im.bx >= sx0 + sw || im.by + KH < sy0 || im.by >= sy0 + sh) continue;
+                    if (im.bx + KH < ax0 || im.bx >= ax0 + I.sw || im.by + KH < ay0 || im.by >= ay0 + I.sh) continue;
                     Cand c;
                     c.ak = im.ak;
-                    c.lx = (int16_t)(im.bx - (sx0 - KH));
-                    c.ly = (int16_t)(im.by - (sy0 - KH));
-                    sub.push_back(c);
-                }
-                int K = std::max<int>(1, (int)((sub.size() + (size_t)SCATTER_ITEMS * 16 * SCATTER_ROUND_MAX - 1)
-                                                / ((size_t)SCATTER_ITEMS * 16 * SCATTER_ROUND_MAX)));
-                std::vector<std::vector<Cand>> deal;
-                std::vector<int> rb, rc;
-                long long f = 0;
-                for (int attempt = 0; attempt < 8; ++attempt) {
-                    const int ni = K * SCATTER_ITEMS;
-                    deal.assign(ni, {});
-                    for (size_t q = 0; q < sub.size(); ++q) deal[q % ni].push_back(sub[q]);
-                    tmp_slots.clear(); f = 0; rb.assign(ni, 0); rc.assign(ni, 0);
-                    int mr = 0;
-                    for (int it = 0; it < ni; ++it) {
-                        rb[it] = (int)(tmp_slots.size() / 32);
-                        rc[it] = build_rounds(deal[it], true, SP_PITCH, tmp_slots, f);
-                        mr = std::max(mr, rc[it]);
-                    }
-                    if (mr <= SCATTER_ROUND_MAX || attempt == 7) break;
-                    K = (int)std::ceil(K * (double)mr / SCATTER_ROUND_MAX * 1.15) + 1;
-                }
-                const int base = (int)(out.scatter_slots.size() / 32);
-                out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
-                out.scatter_filled += f;
-                int first_slot = -1;
-                if (K > 1) {
-                    first_slot = out.n_partial_slots;
-                    out.n_partial_slots += K;
-                    MergeJob mj{sx0, sy0, sw, sh, first_slot, K};
-                    out.merge_jobs.push_back(mj);
-                }
-                for (int kk = 0; kk < K; ++kk) {
-                    Pending hp;
-                    std::memset(&hp.cta, 0, sizeof(hp.cta));
-                    hp.cta.rx0 = sx0; hp.cta.ry0 = sy0; hp.cta.rw = sw; hp.cta.rh = sh;
-                    hp.cta.partial_slot = (K > 1) ? first_slot + kk : -1;
-                    hp.work = 0;
-                    for (int it = 0; it < SCATTER_ITEMS; ++it) {
-                        const int id = kk * SCATTER_ITEMS + it;
-                        hp.cta.items[it].px0 = sx0 - KH;
-                        hp.cta.items[it].py0 = sy0 - KH;
-                        hp.cta.items[it].round_begin = base + rb[id];
-                        hp.cta.items[it].round_count = rc[id];
-                        hp.work = std::max<long long>(hp.work, rc[id]);
-                    }
-                    ctas.push_back(hp);
+                    c.lx = (int16_t)(im.bx - (ax0 - KH));
+                    c.ly = (int16_t)(im.by - (ay0 - KH));
+                    quad[iy * 2 + ix].push_back(c);
                 }
             }
+
+        // K CTAs share the rectangle: each quadrant's samples are dealt round-robin over them
+        size_t biggest = 0;
+        for (auto &v : quad) biggest = std::max(biggest, v.size());
+        int K = std::max<int>(1, (int)((biggest + (size_t)24 * SCATTER_ROUND_MAX - 1) / ((size_t)24 * SCATTER_ROUND_MAX)));
+        std::vector<Cand> part;
+        std::vector<int> rb, rc;
+        long long f = 0;
+        for (int attempt = 0; attempt < 8; ++attempt) {
+            tmp_slots.clear(); f = 0;
+            rb.assign((size_t)K * SCATTER_ITEMS, 0); rc.assign((size_t)K * SCATTER_ITEMS, 0);
+            int mr = 0;
+            for (int kk = 0; kk < K; ++kk)
+                for (int it = 0; it < SCATTER_ITEMS; ++it) {
+                    part.clear();
+                    for (size_t q = kk; q < quad[it].size(); q += K) part.push_back(quad[it][q]);
+                    rb[kk * SCATTER_ITEMS + it] = (int)(tmp_slots.size() / 32);
+                    rc[kk * SCATTER_ITEMS + it] = build_rounds(part, true, ACC_PITCH, tmp_slots, f);
+                    mr = std::max(mr, rc[kk * SCATTER_ITEMS + it]);
+                }
+            if (mr <= SCATTER_ROUND_MAX || attempt == 7) break;
+            K = (int)std::ceil(K * (double)mr / SCATTER_ROUND_MAX * 1.1) + (attempt > 2);
+        }
+        const int base = (int)(out.scatter_slots.size() / 32);
+        out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
+        out.scatter_filled += f;
+        int first_slot = -1;
+        if (K > 1) {
+            first_slot = out.n_partial_slots;
+            out.n_partial_slots += K;
+            MergeJob mj{rx0, ry0, rw, rh, first_slot, K};
+            out.merge_jobs.push_back(mj);
+        }
+        for (int kk = 0; kk < K; ++kk) {
+            Pending p;
+            std::memset(&p.cta, 0, sizeof(p.cta));
+            p.cta.rx0 = rx0; p.cta.ry0 = ry0; p.cta.rw = rw; p.cta.rh = rh;
+            p.cta.partial_slot = (K > 1) ? first_slot + kk : -1;
+            p.work = 0;
+            for (int it = 0; it < SCATTER_ITEMS; ++it) {
+                p.cta.items[it] = geom[it];
+                p.cta.items[it].round_begin = base + rb[kk * SCATTER_ITEMS + it];
+                p.cta.items[it].round_count = rc[kk * SCATTER_ITEMS + it];
+                p.work = std::max<long long>(p.work, rc[kk * SCATTER_ITEMS + it]);
+            }
+            ctas.push_back(p);
+        }
     }
     std::stable_sort(ctas.begin(), ctas.end(),
                      [](const Pending &x, const Pending &y) { return x.work > y.work; });
@@ -532,7 +499,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         for (int i = 0; i < 32; ++i) {
             if (lanes[i].ak == SLOT_EMPTY) continue;
             const int xi = lanes[i].lxy & 0xffff, yi = lanes[i].lxy >> 16;
-            if (disjoint && (xi + KW > SP_W || yi + KW > SP_H)) ++bad;
+            if (disjoint && (xi >= SB_W || yi >= SB_H)) ++bad;
             for (int j = i + 1; j < 32; ++j) {
                 if (lanes[j].ak == SLOT_EMPTY) continue;
                 const int xj = lanes[j].lxy & 0xffff, yj = lanes[j].lxy >> 16;
@@ -579,32 +546,46 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         }
     std::vector<int> slot_owner(s.n_partial_slots, 0);
     for (const ScatterCta &c : s.scatter_ctas) {
-        if (c.rx0 < 0 || c.ry0 < 0 || c.rx0 + c.rw > G || c.ry0 + c.rh > G || c.rw < 1 || c.rh < 1) { ++bad; continue; }
+        if (c.rx0 < 0 || c.ry0 < 0 || c.rx0 + c.rw > G || c.ry0 + c.rh > G || c.rw < 1 || c.rh < 1 ||
+            c.rw > SR_X || c.rh > SR_Y || (c.rw & 1) || (c.rx0 & 1)) { ++bad; continue; }
         if (c.partial_slot >= 0) {
-            if (c.partial_slot >= s.n_partial_slots || c.rw > ST_X || c.rh > ST_Y) { ++bad; continue; }
+            if (c.partial_slot >= s.n_partial_slots) { ++bad; continue; }
             ++slot_owner[c.partial_slot];
         } else {
             for (int y = 0; y < c.rh; ++y)
                 for (int x = 0; x < c.rw; ++x) ++written[(size_t)(c.ry0 + y) * G + c.rx0 + x];
         }
+        // the warps' quadrants must be pairwise disjoint and inside the rectangle
+        for (int i = 0; i < SCATTER_ITEMS; ++i) {
+            const ScatterItem &A = c.items[i];
+            if (A.round_count == 0) continue;
+            if (A.sx0 < 0 || A.sy0 < 0 || A.sw < 1 || A.sh < 1 || A.sx0 + A.sw > c.rw || A.sy0 + A.sh > c.rh ||
+                A.sw > ST_X || A.sh > ST_Y) ++bad;
+            for (int j = i + 1; j < SCATTER_ITEMS; ++j) {
+                const ScatterItem &B = c.items[j];
+                if (B.round_count == 0) continue;
+                if (A.sx0 < B.sx0 + B.sw && B.sx0 < A.sx0 + A.sw && A.sy0 < B.sy0 + B.sh && B.sy0 < A.sy0 + A.sh) ++bad;
+            }
+        }
         for (int it = 0; it < SCATTER_ITEMS; ++it) {
             const ScatterItem &I = c.items[it];
-            if (I.round_count > 0 && (I.px0 + SP_W < c.rx0 || I.py0 + SP_H < c.ry0)) ++bad;
+            if (I.round_count > SCATTER_ROUND_MAX * 2) ++bad;
+            const int ax0 = c.rx0 + I.sx0, ay0 = c.ry0 + I.sy0;
             for (int r = 0; r < I.round_count; ++r) {
                 const Slot *lanes = &s.scatter_slots[(size_t)(I.round_begin + r) * 32];
-                check_round(lanes, SP_PITCH, true);
+                check_round(lanes, ACC_PITCH, true);
                 for (int l = 0; l < 32; ++l) {
                     if (lanes[l].ak == SLOT_EMPTY) continue;
                     const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;
                     if (a >= g.n_angles || k >= g.n_det) { ++bad; continue; }
                     int x0, y0;
                     g.base(a, k, x0, y0);
-                    const int bx = I.px0 + (int)(lanes[l].lxy & 0xffff), by = I.py0 + (int)(lanes[l].lxy >> 16);
+                    const int bx = ax0 - KH + (int)(lanes[l].lxy & 0xffff), by = ay0 - KH + (int)(lanes[l].lxy >> 16);
                     if (posmod(bx - x0, G) != 0 || posmod(by - y0, G) != 0) ++bad;
                     for (int ty = 0; ty < KW; ++ty)
                         for (int tx = 0; tx < KW; ++tx) {
-                            const int cx = bx + tx, cy = by + ty;
-                            if (cx < c.rx0 || cx >= c.rx0 + c.rw || cy < c.ry0 || cy >= c.ry0 + c.rh) continue;
+                            const int cx = bx + tx, cy = by + ty;       // the kernel clips to the quadrant
+                            if (cx < ax0 || cx >= ax0 + I.sw || cy < ay0 || cy >= ay0 + I.sh) continue;
                             got[(size_t)cy * G + cx] += tap_hash(lanes[l].ak, tx, ty);
                         }
                 }

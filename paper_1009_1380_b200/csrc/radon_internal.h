@@ -62,15 +62,17 @@ constexpr int GATHER_WARPS = 8;
 constexpr int GATHER_CTAS_PER_SM = 3;
 constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
 
-// Scatter (gridding): each warp owns a private accumulator of one ST_X x ST_Y sub-tile
-// plus a KH margin on every side; a CTA merges its warps' accumulators in fixed order.
+// Scatter (gridding): a CTA accumulates one SR_X x SR_Y output rectangle in shared memory;
+// each of its warps owns one ST_X x ST_Y quadrant of it and processes every sample whose
+// footprint intersects that quadrant, taps clipped to the quadrant (so warps never share a
+// cell, and the accumulator needs no margins).
 constexpr int ST_X = 64, ST_Y = 32;
-constexpr int SP_W = ST_X + 2 * KH;   // 74
-constexpr int SP_H = ST_Y + 2 * KH;   // 42
-constexpr int SP_PITCH = SP_W + 1;    // 75 (odd)
+constexpr int SR_X = 2 * ST_X, SR_Y = 2 * ST_Y;   // CTA output rectangle: 2 x 2 quadrants
 constexpr int SCATTER_ITEMS = 4;      // warps per CTA
-constexpr int SR_X = 2 * ST_X, SR_Y = 2 * ST_Y;   // light CTA output rectangle: 2 x 2 sub-tiles
-constexpr int SCATTER_ROUND_MAX = 48; // rounds per warp before a rectangle is split further
+constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
+constexpr int SB_W = ST_X + KH, SB_H = ST_Y + KH;   // range of biased base coordinates in a quadrant
+constexpr int SCATTER_ROUND_MAX = 48; // rounds per warp before a rectangle's samples are split over CTAs
+constexpr int SCATTER_CTAS_PER_SM = 3;
 
 // One lane's work in one round: which polar sample, and where its W x W footprint
 // starts inside the staged tile (gather) or the warp-private accumulator (scatter).
@@ -85,8 +87,8 @@ struct GatherCta {
     int round_begin, round_count;
 };
 
-struct ScatterItem {
-    int px0, py0;               // grid coordinates of the private accumulator's origin
+struct ScatterItem {            // one warp: quadrant (relative to the rectangle) and its rounds
+    int sx0, sy0, sw, sh;       // slot coordinates are relative to (sx0 - KH, sy0 - KH)
     int round_begin, round_count;
 };
 
