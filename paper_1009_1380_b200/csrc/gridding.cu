@@ -41,10 +41,10 @@ __device__ __forceinline__ void lut_weights(const float *lut, float delta, float
 
 // Polar sample (a,k) -> fractional offsets of its first tap: delta = x0 - (gx - W/2) in [0,1).
 // fp64 on purpose (an fp32 product G*j/n*cos loses 2.6e-5 at G = 4096).
-__device__ __forceinline__ void sample_taps(const double2 *__restrict__ cs, const float *lut, const KbPoly &kp,
-                                            int a, int k, int cd, double halfG, Taps &tp)
+// d = cs[a] = (G/n)(cos theta_a, sin theta_a).
+__device__ __forceinline__ void sample_taps_dir(const double2 d, const float *lut, const KbPoly &kp,
+                                                int k, int cd, double halfG, Taps &tp)
 {
-    const double2 d = __ldg(&cs[a]);
     const double jj = (double)(k - cd);
     const double gx = fma(jj, d.x, halfG) - 0.5 * KW;
     const double gy = fma(jj, d.y, halfG) - 0.5 * KW;
@@ -57,6 +57,11 @@ __device__ __forceinline__ void sample_taps(const double2 *__restrict__ cs, cons
     kb_poly_weights(kp, dx, tp.wx);
     kb_poly_weights(kp, dy, tp.wy);
 #endif
+}
+__device__ __forceinline__ void sample_taps(const double2 *__restrict__ cs, const float *lut, const KbPoly &kp,
+                                            int a, int k, int cd, double halfG, Taps &tp)
+{
+    sample_taps_dir(__ldg(&cs[a]), lut, kp, k, cd, halfG, tp);
 }
 
 __device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__restrict__ g_lut)
@@ -213,6 +218,43 @@ __device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t by
                  ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
 
+// One footprint row of one sample: cell[lx] += (vr, vi) * wx[lx] for the taps whose bit is set
+// in `mask`.  Written as one PTX block on a 32-bit shared-window address with immediate
+// offsets: W predicated 64-bit loads, 2 W FMAs, W predicated stores, nothing else.
+__device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float vr, float vi, const float (&wx)[KW])
+{
+    static_assert(KW == 6, "row step is written for W = 6");
+    asm volatile(
+        "{\n"
+        ".reg .pred p0, p1, p2, p3, p4, p5;\n"
+        ".reg .b32 t0, t1, t2, t3, t4, t5;\n"
+        ".reg .f32 r0, i0, r1, i1, r2, i2, r3, i3, r4, i4, r5, i5;\n"
+        "and.b32 t0, %1, 1;\n and.b32 t1, %1, 2;\n and.b32 t2, %1, 4;\n"
+        "and.b32 t3, %1, 8;\n and.b32 t4, %1, 16;\n and.b32 t5, %1, 32;\n"
+        "setp.ne.b32 p0, t0, 0;\n setp.ne.b32 p1, t1, 0;\n setp.ne.b32 p2, t2, 0;\n"
+        "setp.ne.b32 p3, t3, 0;\n setp.ne.b32 p4, t4, 0;\n setp.ne.b32 p5, t5, 0;\n"
+        "@p0 ld.shared.v2.f32 {r0, i0}, [%0];\n"
+        "@p1 ld.shared.v2.f32 {r1, i1}, [%0+8];\n"
+        "@p2 ld.shared.v2.f32 {r2, i2}, [%0+16];\n"
+        "@p3 ld.shared.v2.f32 {r3, i3}, [%0+24];\n"
+        "@p4 ld.shared.v2.f32 {r4, i4}, [%0+32];\n"
+        "@p5 ld.shared.v2.f32 {r5, i5}, [%0+40];\n"
+        "fma.rn.f32 r0, %2, %4, r0;\n fma.rn.f32 i0, %3, %4, i0;\n"
+        "fma.rn.f32 r1, %2, %5, r1;\n fma.rn.f32 i1, %3, %5, i1;\n"
+        "fma.rn.f32 r2, %2, %6, r2;\n fma.rn.f32 i2, %3, %6, i2;\n"
+        "fma.rn.f32 r3, %2, %7, r3;\n fma.rn.f32 i3, %3, %7, i3;\n"
+        "fma.rn.f32 r4, %2, %8, r4;\n fma.rn.f32 i4, %3, %8, i4;\n"
+        "fma.rn.f32 r5, %2, %9, r5;\n fma.rn.f32 i5, %3, %9, i5;\n"
+        "@p0 st.shared.v2.f32 [%0], {r0, i0};\n"
+        "@p1 st.shared.v2.f32 [%0+8], {r1, i1};\n"
+        "@p2 st.shared.v2.f32 [%0+16], {r2, i2};\n"
+        "@p3 st.shared.v2.f32 [%0+24], {r3, i3};\n"
+        "@p4 st.shared.v2.f32 [%0+32], {r4, i4};\n"
+        "@p5 st.shared.v2.f32 [%0+40], {r5, i5};\n"
+        "}\n" ::"r"(addr), "r"(mask), "f"(vr), "f"(vi),
+        "f"(wx[0]), "f"(wx[1]), "f"(wx[2]), "f"(wx[3]), "f"(wx[4]), "f"(wx[5]) : "memory");
+}
+
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
@@ -235,58 +277,60 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     const ScatterItem item = cta.items[warp];
     const Slot *my = slots + (size_t)item.round_begin * 32 + lane;
     const int nr = item.round_count;
-    // prefetch: slots of rounds 0 and 1, value of round 0
-    Slot s0, s1;
-    s0.ak = SLOT_EMPTY; s0.lxy = 0; s1 = s0;
-    if (nr > 0) s0 = my[0];
-    if (nr > 1) s1 = my[32];
+    // software pipeline (the slot stream comes from HBM, the sample values from L2): slots are
+    // fetched four rounds ahead, sample values and ray directions two rounds ahead
+    auto load_slot = [&](int r) {
+        Slot s;
+        s.ak = SLOT_EMPTY; s.lxy = 0;
+        if (r < nr) s = my[(size_t)r * 32];
+        return s;
+    };
+    auto load_value = [&](const Slot &s, float2 &v, double2 &d) {
+        v = make_float2(0.f, 0.f);
+        d = make_double2(0.0, 0.0);
+        if (s.ak != SLOT_EMPTY) {
+            v = __ldg(&polar[(size_t)(s.ak >> 16) * n_det + (s.ak & 0xffff)]);
+            d = __ldg(&cs[s.ak >> 16]);
+        }
+    };
+    Slot s0 = load_slot(0), s1 = load_slot(1), s2 = load_slot(2), s3 = load_slot(3);
     {   // zero the accumulator while those loads are in flight
         float4 *z = reinterpret_cast<float4 *>(acc);
         for (int i = threadIdx.x; i < (int)(SCATTER_ACC_BYTES / 16); i += SCATTER_THREADS)
             z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    float2 v0 = make_float2(0.f, 0.f);
-    if (s0.ak != SLOT_EMPTY) v0 = __ldg(&polar[(size_t)(s0.ak >> 16) * n_det + (s0.ak & 0xffff)]);
+    float2 v0, v1;
+    double2 d0, d1;
+    load_value(s0, v0, d0);
+    load_value(s1, v1, d1);
     __syncthreads();
 
-    float2 *origin = acc + (item.sy0 - KH) * ACC_PITCH + (item.sx0 - KH);   // slot (0,0); never dereferenced outside the quadrant
+    // shared-window address of slot (0,0); never dereferenced outside the quadrant
+    const uint32_t origin = smem_u32(acc) + (uint32_t)(((item.sy0 - KH) * ACC_PITCH + (item.sx0 - KH)) * (int)sizeof(float2));
     for (int r = 0; r < nr; ++r) {
-        Slot s2;
-        s2.ak = SLOT_EMPTY; s2.lxy = 0;
-        if (r + 2 < nr) s2 = my[(size_t)(r + 2) * 32];
-        float2 v1 = make_float2(0.f, 0.f);
-        if (s1.ak != SLOT_EMPTY) v1 = __ldg(&polar[(size_t)(s1.ak >> 16) * n_det + (s1.ak & 0xffff)]);
+        const Slot s4 = load_slot(r + 4);
+        float2 v2;
+        double2 d2;
+        load_value(s2, v2, d2);
         const bool act = s0.ak != SLOT_EMPTY;
-        const int a = act ? (int)(s0.ak >> 16) : 0, k = act ? (int)(s0.ak & 0xffff) : 0;
         Taps tp;
-        sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
+        sample_taps_dir(d0, s_lut, kp, (int)(s0.ak & 0xffff), cd, halfG, tp);
         const int bx = (int)(s0.lxy & 0xffff), by = (int)(s0.lxy >> 16);   // biased by KH
-        float2 *base = origin + by * ACC_PITCH + bx;
-        // taps inside the quadrant: KH <= bx + lx < KH + sw, likewise rows
-        const int xlo = KH - bx, xhi = KH + item.sw - bx, ylo = KH - by, yhi = KH + item.sh - by;
-        bool px[KW];
-#pragma unroll
-        for (int lx = 0; lx < KW; ++lx) px[lx] = act && lx >= xlo && lx < xhi;
+        const uint32_t base = origin + (uint32_t)((by * ACC_PITCH + bx) * (int)sizeof(float2));
+        // taps inside the quadrant: KH <= bx + lx < KH + sw, likewise rows -> bit masks
+        const int xlo = min(max(KH - bx, 0), KW), xhi = min(max(KH + item.sw - bx, 0), KW);
+        const int ylo = min(max(KH - by, 0), KW), yhi = min(max(KH + item.sh - by, 0), KW);
+        const uint32_t xmask = act ? (((1u << xhi) - 1u) & ~((1u << xlo) - 1u)) : 0u;
+        const uint32_t ymask = ((1u << yhi) - 1u) & ~((1u << ylo) - 1u);
 #pragma unroll
         for (int ly = 0; ly < KW; ++ly) {
-            if (ly >= ylo && ly < yhi) {
-                const float vr = v0.x * tp.wy[ly], vi = v0.y * tp.wy[ly];
-                float2 c[KW];
-#pragma unroll
-                for (int lx = 0; lx < KW; ++lx)
-                    if (px[lx]) c[lx] = base[ly * ACC_PITCH + lx];
-#pragma unroll
-                for (int lx = 0; lx < KW; ++lx) {
-                    c[lx].x = fmaf(vr, tp.wx[lx], c[lx].x);
-                    c[lx].y = fmaf(vi, tp.wx[lx], c[lx].y);
-                }
-#pragma unroll
-                for (int lx = 0; lx < KW; ++lx)
-                    if (px[lx]) base[ly * ACC_PITCH + lx] = c[lx];
-            }
+            const uint32_t m = (ymask & (1u << ly)) ? xmask : 0u;
+            scatter_row(base + (uint32_t)(ly * ACC_PITCH * (int)sizeof(float2)), m,
+                        v0.x * tp.wy[ly], v0.y * tp.wy[ly], tp.wx);
             __syncwarp();   // row steps of different lanes may touch the same cells
         }
-        s0 = s1; s1 = s2; v0 = v1;
+        s0 = s1; s1 = s2; s2 = s3; s3 = s4;
+        v0 = v1; v1 = v2; d0 = d1; d1 = d2;
     }
 
     // flush: the rectangle is written exactly once, by the copy engine
