@@ -136,10 +136,17 @@ int radon_plan_stage_times(radon_plan *p, double total_ms[8], long long launches
 int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_det,
                     long long *M, size_t *workspace_bytes);
 
-/* Schedule statistics of a plan (all host data; out pointers may be NULL):
+/* A plan holds two schedule sets.  half = 0: every polar sample and the whole grid (arbitrary
+ * complex data: radon_nufft2/1, radon_interp_only, radon_grid_only).  half = 1: the Hermitian
+ * half used by radon_forward / radon_adjoint, whose image and sinogram are real: the polar
+ * samples obey F[a,-j] = conj F[a,j] and the gridded spectrum G(-k) = conj G(k), so only the
+ * samples j >= 0 (plus, for even n_det, the mirror image j = +n/2 of the unpaired j = -n/2) are
+ * interpolated, and only the grid rows ky = 0 .. G/2 are gridded.
+ *
+ * Schedule statistics of a plan (all host data; out pointers may be NULL):
  * slots = 32 * rounds issued, filled = slots holding a sample, ctas = thread blocks
  * per launch, for the gather (interp) and the scatter (grid) kernels. */
-int radon_plan_schedule_stats(const radon_plan *p,
+int radon_plan_schedule_stats(const radon_plan *p, int half,
                               long long *gather_slots, long long *gather_filled, int *gather_ctas,
                               long long *scatter_slots, long long *scatter_filled, int *scatter_ctas);
 
@@ -151,14 +158,14 @@ int radon_plan_schedule_stats(const radon_plan *p,
  * (write-conflict freedom without atomics) and that the 16 lanes of every
  * half-warp start in distinct shared-memory bank pairs.  Returns RADON_OK or
  * RADON_EINVAL; *n_violations (may be NULL) receives the number of violations. */
-int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W,
+int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W, int half,
                              long long *n_violations);
 
 /* Host-only statistics of the schedules for a geometry (no GPU, no plan needed):
  * out[0..9] = gather slots, gather filled, gather CTAs, max gather rounds per CTA,
  * scatter slots, scatter filled, scatter CTAs, max scatter rounds per warp,
  * merge jobs, partial rectangles. */
-int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, long long out[10]);
+int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, int half, long long out[10]);
 
 /* Host-only evaluation of the W Kaiser-Bessel tap weights exactly as the kernels compute
  * them (plan-time polynomial pieces, fp32 Horner): w[l] = phi(delta - W/2 + l), l = 0..W-1,

@@ -29,9 +29,9 @@ _SIGNATURES = {
     "radon_plan_stage_timing": (c_int, [c_void_p, c_int]),
     "radon_plan_stage_times": (c_int, [c_void_p, P(ctypes.c_double), P(c_ll)]),
     "radon_plan_info": (c_int, [c_void_p, P(c_int), P(c_int), P(c_int), P(c_int), P(c_ll), P(c_size_t)]),
-    "radon_plan_schedule_stats": (c_int, [c_void_p, P(c_ll), P(c_ll), P(c_int), P(c_ll), P(c_ll), P(c_int)]),
-    "radon_schedule_selfcheck": (c_int, [c_int, c_int, c_int, c_float, c_int, P(c_ll)]),
-    "radon_schedule_host_stats": (c_int, [c_int, c_int, c_int, c_float, c_int, P(c_ll)]),
+    "radon_plan_schedule_stats": (c_int, [c_void_p, c_int, P(c_ll), P(c_ll), P(c_int), P(c_ll), P(c_ll), P(c_int)]),
+    "radon_schedule_selfcheck": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
+    "radon_schedule_host_stats": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_kb_weights_host": (c_int, [c_int, c_float, c_float, P(c_float)]),
     "radon_kernel_launch_count": (c_ll, []),
     "radon_strerror": (ctypes.c_char_p, [c_int]),
@@ -79,17 +79,17 @@ def kernel_launch_count() -> int:
     return int(lib().radon_kernel_launch_count())
 
 
-def schedule_selfcheck(N, n_angles, n_det, sigma=2.0, W=6):
+def schedule_selfcheck(N, n_angles, n_det, sigma=2.0, W=6, half=False):
     """Host-only check of the plan-time schedules (no GPU). Returns (rc, n_violations)."""
     bad = c_ll(-1)
-    rc = lib().radon_schedule_selfcheck(N, n_angles, n_det, sigma, W, ctypes.byref(bad))
+    rc = lib().radon_schedule_selfcheck(N, n_angles, n_det, sigma, W, int(half), ctypes.byref(bad))
     return rc, int(bad.value)
 
 
-def schedule_host_stats(N, n_angles, n_det, sigma=2.0, W=6):
+def schedule_host_stats(N, n_angles, n_det, sigma=2.0, W=6, half=False):
     """Host-only schedule statistics (no GPU): dict of slot / CTA counts."""
     out = (c_ll * 10)()
-    _check(lib().radon_schedule_host_stats(N, n_angles, n_det, sigma, W, out), "radon_schedule_host_stats")
+    _check(lib().radon_schedule_host_stats(N, n_angles, n_det, sigma, W, int(half), out), "radon_schedule_host_stats")
     keys = ["gather_slots", "gather_filled", "gather_ctas", "gather_max_rounds", "scatter_slots",
             "scatter_filled", "scatter_ctas", "scatter_max_rounds", "merge_jobs", "partial_rects"]
     return dict(zip(keys, [int(v) for v in out]))
@@ -152,9 +152,9 @@ class RadonPlan:
 
         return torch.empty(shape, dtype=dtype, device="cuda")
 
-    def schedule_stats(self):
+    def schedule_stats(self, half=False):
         v = [c_ll(), c_ll(), c_int(), c_ll(), c_ll(), c_int()]
-        _check(lib().radon_plan_schedule_stats(self._h, *v), "radon_plan_schedule_stats")
+        _check(lib().radon_plan_schedule_stats(self._h, int(half), *v), "radon_plan_schedule_stats")
         k = ["gather_slots", "gather_filled", "gather_ctas", "scatter_slots", "scatter_filled", "scatter_ctas"]
         return {a: b.value for a, b in zip(k, v)}
 

@@ -48,7 +48,7 @@ struct radon_plan {
     Workspace ws[2];
     long long M = 0;
     size_t device_bytes = 0;
-    long long gather_slots = 0, gather_filled = 0, scatter_slots = 0, scatter_filled = 0;
+    long long gather_slots[2] = {0, 0}, gather_filled[2] = {0, 0}, scatter_slots[2] = {0, 0}, scatter_filled[2] = {0, 0};
     cudaStream_t hstream[2] = {nullptr, nullptr};
     cudaEvent_t hevent[2] = {nullptr, nullptr};
 };
@@ -80,7 +80,7 @@ static int dev_upload(radon_plan *p, T **ptr, const std::vector<H> &host)
 
 static int validate(int N, int n_angles, int n_det, float sigma, int W, int *G_out)
 {
-    if (N < 8 || n_angles < 1 || n_det < 2 || n_angles > 65535 || n_det > 65535) return RADON_EINVAL;
+    if (N < 8 || n_angles < 1 || n_det < 2 || n_angles > 65535 || n_det > 65533) return RADON_EINVAL;
     if (W < 2 || W > 12) return RADON_EINVAL;
     if (!(sigma > 1.0f) || sigma > 8.0f) return RADON_EINVAL;
     const double g = (double)sigma * N;
@@ -100,8 +100,10 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     DevicePlan &d = p->dev;
     cudaFree(d.cs); cudaFree(d.lut); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
     cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
-    cudaFree(d.gather_ctas); cudaFree(d.gather_slots); cudaFree(d.scatter_ctas); cudaFree(d.scatter_slots);
-    cudaFree(d.merge_jobs); cudaFree(d.scratch);
+    for (auto &q : d.sched) {
+        cudaFree(q.gather_ctas); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
+        cudaFree(q.merge_jobs); cudaFree(q.scratch);
+    }
     for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     for (int i = 0; i < 2; ++i) {
@@ -149,19 +151,22 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if ((rc = dev_upload(p, &d.chirp_b, cb))) return rc;
     if (!hf.empty() && (rc = dev_upload(p, &d.chirp_hf, hf))) return rc;
     // P3: schedules
-    Schedules sch;
-    build_schedules(p->geo, sch);
-    p->gather_slots = (long long)sch.gather_slots.size(); p->gather_filled = sch.gather_filled;
-    p->scatter_slots = (long long)sch.scatter_slots.size(); p->scatter_filled = sch.scatter_filled;
-    d.n_gather_ctas = (int)sch.gather_ctas.size();
-    d.n_scatter_ctas = (int)sch.scatter_ctas.size();
-    d.n_merge_jobs = (int)sch.merge_jobs.size();
-    if ((rc = dev_upload(p, &d.gather_ctas, sch.gather_ctas))) return rc;
-    if ((rc = dev_upload(p, &d.gather_slots, sch.gather_slots))) return rc;
-    if ((rc = dev_upload(p, &d.scatter_ctas, sch.scatter_ctas))) return rc;
-    if ((rc = dev_upload(p, &d.scatter_slots, sch.scatter_slots))) return rc;
-    if ((rc = dev_upload(p, &d.merge_jobs, sch.merge_jobs))) return rc;
-    if ((rc = dev_alloc(p, &d.scratch, (size_t)sch.n_partial_slots * SR_X * SR_Y))) return rc;
+    for (int h = 0; h < 2; ++h) {
+        Schedules sch;
+        build_schedules(p->geo, sch, h == 1);
+        DevicePlan::Sched &q = d.sched[h];
+        p->gather_slots[h] = (long long)sch.gather_slots.size(); p->gather_filled[h] = sch.gather_filled;
+        p->scatter_slots[h] = (long long)sch.scatter_slots.size(); p->scatter_filled[h] = sch.scatter_filled;
+        q.n_gather_ctas = (int)sch.gather_ctas.size();
+        q.n_scatter_ctas = (int)sch.scatter_ctas.size();
+        q.n_merge_jobs = (int)sch.merge_jobs.size();
+        if ((rc = dev_upload(p, &q.gather_ctas, sch.gather_ctas))) return rc;
+        if ((rc = dev_upload(p, &q.gather_slots, sch.gather_slots))) return rc;
+        if ((rc = dev_upload(p, &q.scatter_ctas, sch.scatter_ctas))) return rc;
+        if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;
+        if ((rc = dev_upload(p, &q.merge_jobs, sch.merge_jobs))) return rc;
+        if ((rc = dev_alloc(p, &q.scratch, (size_t)sch.n_partial_slots * SR_X * SR_Y))) return rc;
+    }
     // workspace (two sets: the host-buffer entry points overlap copies with kernels)
     for (auto &w : p->ws) {
         if ((rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
@@ -213,23 +218,26 @@ static inline void mark(radon_plan *p, cudaStream_t st, int stage)
     t.stage[t.used++] = stage;
 }
 
-static int nufft2_ws(radon_plan *p, Workspace &w, const float *d_x, float2 *d_polar, cudaStream_t st)
+// half: Hermitian-half schedules (d_polar then holds k >= n/2 of every row, and k = 0 for even n)
+static int nufft2_ws(radon_plan *p, Workspace &w, bool half, const float *d_x, float2 *d_polar, cudaStream_t st)
 {
     mark(p, st, 0);
-    if (launch_fft2d_pass(0, p->dev, d_x, w.T, 0, st)) return RADON_ECUDA;        // F1 + F2 (columns)
+    if (launch_fft2d_pass(0, p->dev, d_x, w.T, 0, st)) return RADON_ECUDA;                 // F1 + F2 (columns)
     mark(p, st, 1);
-    if (launch_fft2d_pass(1, p->dev, w.T, w.grid, 1, st)) return RADON_ECUDA;     // F2 (rows)
+    if (launch_fft2d_pass(1, p->dev, w.T, w.grid, half ? 2 : 1, st)) return RADON_ECUDA;   // F2 (rows)
     mark(p, st, 2);
-    if (launch_gather(p->dev, w.grid, d_polar, st)) return RADON_ECUDA;        // F3
+    if (launch_gather(p->dev, half, w.grid, d_polar, st)) return RADON_ECUDA;              // F3
     return check_launch();
 }
 
-static int nufft1_ws(radon_plan *p, Workspace &w, const float2 *d_polar, float *d_x, cudaStream_t st)
+// half: d_polar is Hermitian along every row (the DFT of a real sinogram); only the grid rows
+// ky = 0 .. G/2 are gridded and the row pass reads them without folding.
+static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st)
 {
     mark(p, st, 5);
-    if (launch_scatter(p->dev, d_polar, w.grid, st)) return RADON_ECUDA;       // A2
+    if (launch_scatter(p->dev, half, d_polar, w.grid, st)) return RADON_ECUDA;             // A2
     mark(p, st, 6);
-    if (launch_fft2d_pass(2, p->dev, w.grid, w.T, 1, st)) return RADON_ECUDA;     // A3 (rows)
+    if (launch_fft2d_pass(2, p->dev, w.grid, w.T, half ? 0 : 1, st)) return RADON_ECUDA;   // A3 (rows)
     mark(p, st, 7);
     if (launch_fft2d_pass(3, p->dev, w.T, d_x, 0, st)) return RADON_ECUDA;        // A3 (columns) + A4
     return check_launch();
@@ -237,10 +245,10 @@ static int nufft1_ws(radon_plan *p, Workspace &w, const float2 *d_polar, float *
 
 static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_sino, cudaStream_t st)
 {
-    int rc = nufft2_ws(p, w, d_x, w.polar, st);
+    int rc = nufft2_ws(p, w, true, d_x, w.polar, st);
     if (rc) return rc;
     mark(p, st, 3);
-    if (launch_proj(true, p->dev, (const float *)w.polar, d_sino, st)) return RADON_ECUDA;   // F4
+    if (launch_proj(true, true, p->dev, (const float *)w.polar, d_sino, st)) return RADON_ECUDA;   // F4
     mark(p, st, -1);
     return check_launch();
 }
@@ -248,10 +256,10 @@ static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_si
 static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st)
 {
     mark(p, st, 4);
-    if (launch_proj(false, p->dev, d_sino, (float *)w.polar, st)) return RADON_ECUDA;        // A1
+    if (launch_proj(false, false, p->dev, d_sino, (float *)w.polar, st)) return RADON_ECUDA;        // A1
     int rc = check_launch();
     if (rc) return rc;
-    rc = nufft1_ws(p, w, w.polar, d_x, st);
+    rc = nufft1_ws(p, w, true, w.polar, d_x, st);
     mark(p, st, -1);
     return rc;
 }
@@ -374,7 +382,7 @@ extern "C" int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x
 extern "C" int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, void *stream)
 {
     if (!p || !d_x || !d_polar) return RADON_EINVAL;
-    int rc = nufft2_ws(p, p->ws[0], d_x, (float2 *)d_polar, (cudaStream_t)stream);
+    int rc = nufft2_ws(p, p->ws[0], false, d_x, (float2 *)d_polar, (cudaStream_t)stream);
     mark(p, (cudaStream_t)stream, -1);
     return rc;
 }
@@ -382,7 +390,7 @@ extern "C" int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, voi
 extern "C" int radon_nufft1(radon_plan *p, const float *d_polar, float *d_x, void *stream)
 {
     if (!p || !d_x || !d_polar) return RADON_EINVAL;
-    int rc = nufft1_ws(p, p->ws[0], (const float2 *)d_polar, d_x, (cudaStream_t)stream);
+    int rc = nufft1_ws(p, p->ws[0], false, (const float2 *)d_polar, d_x, (cudaStream_t)stream);
     mark(p, (cudaStream_t)stream, -1);
     return rc;
 }
@@ -390,28 +398,28 @@ extern "C" int radon_nufft1(radon_plan *p, const float *d_polar, float *d_x, voi
 extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *stream)
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
-    if (launch_gather(p->dev, (const float2 *)d_grid, (float2 *)d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_gather(p->dev, false, (const float2 *)d_grid, (float2 *)d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
 extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
-    if (launch_scatter(p->dev, (const float2 *)d_polar, (float2 *)d_grid, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
 extern "C" int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream)
 {
     if (!p || !d_polar || !d_sino) return RADON_EINVAL;
-    if (launch_proj(true, p->dev, d_polar, d_sino, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_proj(true, false, p->dev, d_polar, d_sino, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
 extern "C" int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *stream)
 {
     if (!p || !d_polar || !d_sino) return RADON_EINVAL;
-    if (launch_proj(false, p->dev, d_sino, d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_proj(false, false, p->dev, d_sino, d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
@@ -428,21 +436,22 @@ extern "C" int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angle
     return RADON_OK;
 }
 
-extern "C" int radon_plan_schedule_stats(const radon_plan *p,
+extern "C" int radon_plan_schedule_stats(const radon_plan *p, int half,
                                          long long *gather_slots, long long *gather_filled, int *gather_ctas,
                                          long long *scatter_slots, long long *scatter_filled, int *scatter_ctas)
 {
     if (!p) return RADON_EINVAL;
-    if (gather_slots) *gather_slots = p->gather_slots;
-    if (gather_filled) *gather_filled = p->gather_filled;
-    if (gather_ctas) *gather_ctas = p->dev.n_gather_ctas;
-    if (scatter_slots) *scatter_slots = p->scatter_slots;
-    if (scatter_filled) *scatter_filled = p->scatter_filled;
-    if (scatter_ctas) *scatter_ctas = p->dev.n_scatter_ctas;
+    const int h = half ? 1 : 0;
+    if (gather_slots) *gather_slots = p->gather_slots[h];
+    if (gather_filled) *gather_filled = p->gather_filled[h];
+    if (gather_ctas) *gather_ctas = p->dev.sched[h].n_gather_ctas;
+    if (scatter_slots) *scatter_slots = p->scatter_slots[h];
+    if (scatter_filled) *scatter_filled = p->scatter_filled[h];
+    if (scatter_ctas) *scatter_ctas = p->dev.sched[h].n_scatter_ctas;
     return RADON_OK;
 }
 
-extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W,
+extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W, int half,
                                         long long *n_violations)
 {
     if (n_violations) *n_violations = -1;
@@ -453,7 +462,7 @@ extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float si
         Geometry geo;
         geo.init(N, n_angles, n_det, (double)sigma, W);
         Schedules sch;
-        build_schedules(geo, sch);
+        build_schedules(geo, sch, half != 0);
         const long long bad = check_schedules(geo, sch);
         if (n_violations) *n_violations = bad;
         return bad == 0 ? RADON_OK : RADON_EINVAL;
@@ -462,7 +471,8 @@ extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float si
     }
 }
 
-extern "C" int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, long long out[10])
+extern "C" int radon_schedule_host_stats(int N, int n_angles, int n_det, float sigma, int W, int half,
+                                         long long out[10])
 {
     if (!out) return RADON_EINVAL;
     int G = 0;
@@ -472,7 +482,7 @@ extern "C" int radon_schedule_host_stats(int N, int n_angles, int n_det, float s
         Geometry geo;
         geo.init(N, n_angles, n_det, (double)sigma, W);
         Schedules sch;
-        build_schedules(geo, sch);
+        build_schedules(geo, sch, half != 0);
         long long mg = 0, ms = 0;
         for (const auto &c : sch.gather_ctas) mg = std::max<long long>(mg, c.round_count);
         for (const auto &c : sch.scatter_ctas)

@@ -31,54 +31,81 @@ struct FftCfg {
     static constexpr size_t SMEM = (size_t)NF * PADLEN * sizeof(float2);
 };
 
+// Column passes: a CTA transforms NFC column PAIRS (2 NFC adjacent image columns).  All global
+// traffic is cooperative, the pair index fastest across lanes, so that a warp touches 2 NFC
+// adjacent floats of each image row / NFC adjacent (A, B) pairs of each T row -- whole 32-byte
+// sectors -- instead of one sector per lane; the FFT threads pick their registers up from
+// shared memory (ncu, round 1b: the per-lane version spent its time in the L1 sector stage,
+// 31.5 sectors per store request, 4x write amplification into L2).
+template <int L>
+struct ColCfg {
+    static constexpr int TF = L / 16;
+    static constexpr int NFC_WANT = (128 / TF > 4) ? 128 / TF : 4;
+    static constexpr int NFC = (NFC_WANT * TF > 1024) ? 1024 / TF : NFC_WANT;   // column pairs per CTA
+    static constexpr int THREADS = NFC * TF;
+    static constexpr int SKEW = (16 / NFC > 1) ? 16 / NFC : 1;   // pairs start in distinct bank pairs
+    static constexpr int STRIDE = fft_padded_len(L) + SKEW;
+    static constexpr size_t SMEM = (size_t)NFC * STRIDE * sizeof(float2);
+};
+
 // ---- F1 + first half of F2 ------------------------------------------------------------------
 template <int L>
-__global__ void __launch_bounds__(FftCfg<L>::THREADS)
+__global__ void __launch_bounds__(ColCfg<L>::THREADS)
 colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod,
                    float2 *__restrict__ T, const float2 *__restrict__ tw, int N)
 {
     extern __shared__ __align__(16) float2 s_fft[];
-    using C = FftCfg<L>;
-    constexpr int TF = C::TF;
-    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
-    float2 *s = s_fft + f * C::PADLEN;
-    const int p = blockIdx.x * C::NF + f, ix = 2 * p;
-    const bool live = ix < N, has_b = ix + 1 < N;
+    using C = ColCfg<L>;
+    constexpr int TF = C::TF, NFC = C::NFC;
     const int c = N / 2;
-    const float da = live ? __ldg(&deapod[ix]) : 0.f, db = has_b ? __ldg(&deapod[ix + 1]) : 0.f;
-
+    const bool even = (N & 1) == 0;
+    {   // cooperative load: thread -> (row iy, pair fc), fc fastest; de-apodise; FFT position (iy - c) mod L
+        const int fc = threadIdx.x % NFC, ix = 2 * (blockIdx.x * NFC + fc);
+        float2 *sf = s_fft + fc * C::STRIDE;
+        if (ix < N) {
+            const bool has_b = ix + 1 < N;
+            const float da = __ldg(&deapod[ix]), db = has_b ? __ldg(&deapod[ix + 1]) : 0.f;
+            for (int iy = threadIdx.x / NFC; iy < N; iy += C::THREADS / NFC) {
+                const float dy = __ldg(&deapod[iy]);
+                const float *row = x + (size_t)iy * N + ix;
+                float2 v;
+                if (even) v = __ldg(reinterpret_cast<const float2 *>(row));
+                else { v.x = __ldg(row); v.y = has_b ? __ldg(row + 1) : 0.f; }
+                sf[FFT_PAD((iy - c) & (L - 1))] = make_float2(v.x * da * dy, v.y * db * dy);
+            }
+        }
+    }
+    __syncthreads();
+    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
+    float2 *s = s_fft + f * C::STRIDE;
+    const bool live = 2 * (blockIdx.x * NFC + f) < N;
     float2 v[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-        const int iy = (t + i * TF + c) & (L - 1);         // FFT position (iy - c) mod L
-        v[i] = make_float2(0.f, 0.f);
-        if (live && iy < N) {
-            const float dy = __ldg(&deapod[iy]);
-            const float *row = x + (size_t)iy * N + ix;
-            v[i].x = __ldg(row) * da * dy;
-            if (has_b) v[i].y = __ldg(row + 1) * db * dy;
-        }
+        const int iy = (t + i * TF + c) & (L - 1);         // zero padding pruned: rows >= N were never staged
+        v[i] = (live && iy < N) ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
     }
+    __syncthreads();
     fft_reg<L, -1>(v, s, tw, t);
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
     __syncthreads();
-    if (!live) return;
-    // untangle: A[k] = (Z[k] + conj Z[-k])/2, B[k] = (Z[k] - conj Z[-k])/(2i), k = 0..L/2
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int k = t + i * TF;
-        const float2 zk = v[i], zm = s[FFT_PAD((L - k) & (L - 1))];
-        float2 *dst = T + (size_t)k * N + ix;
-        dst[0] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-        if (has_b) dst[1] = make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x));
-    }
-    if (t == 0) {
-        const float2 z = v[8];                              // k = L/2 is its own mirror
-        float2 *dst = T + (size_t)(L / 2) * N + ix;
-        dst[0] = make_float2(z.x, 0.f);
-        if (has_b) dst[1] = make_float2(z.y, 0.f);
+    {   // cooperative store: thread -> (ky, pair fc); untangle the packed pair:
+        // A[k] = (Z[k] + conj Z[-k])/2, B[k] = (Z[k] - conj Z[-k])/(2i), k = 0..L/2
+        const int fc = threadIdx.x % NFC, ix = 2 * (blockIdx.x * NFC + fc);
+        const float2 *sf = s_fft + fc * C::STRIDE;
+        if (ix < N) {
+            const bool has_b = ix + 1 < N;
+            for (int k = threadIdx.x / NFC; k <= L / 2; k += C::THREADS / NFC) {
+                const float2 zk = sf[FFT_PAD(k)], zm = sf[FFT_PAD((L - k) & (L - 1))];
+                const float2 A = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+                const float2 B = make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x));
+                float2 *dst = T + (size_t)k * N + ix;
+                if (even) *reinterpret_cast<float4 *>(dst) = make_float4(A.x, A.y, B.x, B.y);
+                else { dst[0] = A; if (has_b) dst[1] = B; }
+            }
+        }
     }
 }
 
@@ -109,7 +136,10 @@ rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
     float2 *row = grid + (size_t)cy * L;
 #pragma unroll
     for (int i = 0; i < 16; ++i) row[(t + i * TF + L / 2) & (L - 1)] = v[i];
-    if (mirror && ky != 0 && ky != L / 2) {
+    // mirror == 1: every row -ky; mirror == 2: only the rows the Hermitian-half gather reads
+    // besides ky = 0 .. L/2, i.e. -KW/2 <= ky' < 0 and L/2 < ky' <= L/2 + KW/2 - 1 (mod L)
+    const bool want = mirror == 1 || (mirror == 2 && (ky <= KW / 2 || ky >= L / 2 - (KW / 2 - 1)));
+    if (want && ky != 0 && ky != L / 2) {
         float2 *mrow = grid + (size_t)(L - cy) * L;
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
@@ -160,44 +190,53 @@ rowpass_inv_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
 
 // ---- second half of A3 + A4: column pairs of T -> image ---------------------------------------
 template <int L>
-__global__ void __launch_bounds__(FftCfg<L>::THREADS)
+__global__ void __launch_bounds__(ColCfg<L>::THREADS)
 colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapod,
                    float *__restrict__ x, const float2 *__restrict__ tw, int N)
 {
     extern __shared__ __align__(16) float2 s_fft[];
-    using C = FftCfg<L>;
-    constexpr int TF = C::TF;
-    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
-    float2 *s = s_fft + f * C::PADLEN;
-    const int p = blockIdx.x * C::NF + f, ix = 2 * p;
-    const bool live = ix < N, has_b = ix + 1 < N;
+    using C = ColCfg<L>;
+    constexpr int TF = C::TF, NFC = C::NFC;
     const int c = N / 2;
-
-    float2 v[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int k = t + i * TF;
-        v[i] = make_float2(0.f, 0.f);
-        if (live) {
-            const bool up = k > L / 2;
-            const float2 *src = T + (size_t)(up ? L - k : k) * N + ix;
-            const float2 A = __ldg(src), B = has_b ? __ldg(src + 1) : make_float2(0.f, 0.f);
-            if (k == 0 || k == L / 2) v[i] = make_float2(A.x, B.x);            // real by symmetry
-            else if (!up) v[i] = make_float2(A.x - B.y, A.y + B.x);            // A + i B
-            else v[i] = make_float2(A.x + B.y, B.x - A.y);                     // conj A + i conj B
+    const bool even = (N & 1) == 0;
+    const int fc = threadIdx.x % NFC, ixc = 2 * (blockIdx.x * NFC + fc);
+    float2 *sf = s_fft + fc * C::STRIDE;
+    if (ixc < N) {   // cooperative load: thread -> (ky, pair fc); pack Z = A + i B, Z[-k] = conj A + i conj B
+        const bool has_b = ixc + 1 < N;
+        for (int k = threadIdx.x / NFC; k <= L / 2; k += C::THREADS / NFC) {
+            const float2 *src = T + (size_t)k * N + ixc;
+            float2 A, B;
+            if (even) { const float4 q = __ldg(reinterpret_cast<const float4 *>(src)); A = make_float2(q.x, q.y); B = make_float2(q.z, q.w); }
+            else { A = __ldg(src); B = has_b ? __ldg(src + 1) : make_float2(0.f, 0.f); }
+            if (k == 0 || k == L / 2) sf[FFT_PAD(k)] = make_float2(A.x, B.x);        // real by symmetry
+            else {
+                sf[FFT_PAD(k)] = make_float2(A.x - B.y, A.y + B.x);
+                sf[FFT_PAD(L - k)] = make_float2(A.x + B.y, B.x - A.y);
+            }
         }
     }
-    fft_reg<L, +1>(v, s, tw, t);
-    if (!live) return;
-    const float da = __ldg(&deapod[ix]), db = has_b ? __ldg(&deapod[ix + 1]) : 0.f;
+    __syncthreads();
+    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
+    float2 *s = s_fft + f * C::STRIDE;
+    const bool live = 2 * (blockIdx.x * NFC + f) < N;
+    float2 v[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int iy = (t + i * TF + c) & (L - 1);
-        if (iy < N) {
+    for (int i = 0; i < 16; ++i) v[i] = live ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
+    __syncthreads();
+    fft_reg<L, +1>(v, s, tw, t);
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
+    __syncthreads();
+    if (ixc < N) {   // cooperative store: thread -> (row iy, pair fc); crop, de-apodise
+        const bool has_b = ixc + 1 < N;
+        const float da = __ldg(&deapod[ixc]), db = has_b ? __ldg(&deapod[ixc + 1]) : 0.f;
+        for (int iy = threadIdx.x / NFC; iy < N; iy += C::THREADS / NFC) {
             const float dy = __ldg(&deapod[iy]);
-            float *row = x + (size_t)iy * N + ix;
-            row[0] = v[i].x * da * dy;
-            if (has_b) row[1] = v[i].y * db * dy;
+            const float2 z = sf[FFT_PAD((iy - c) & (L - 1))];
+            float *row = x + (size_t)iy * N + ixc;
+            if (even) *reinterpret_cast<float2 *>(row) = make_float2(z.x * da * dy, z.y * db * dy);
+            else { row[0] = z.x * da * dy; if (has_b) row[1] = z.y * db * dy; }
         }
     }
 }
@@ -209,13 +248,14 @@ template <int L>
 static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st)
 {
     using C = FftCfg<L>;
+    using CC = ColCfg<L>;
     const int N = p.N;
-    const int col_blocks = ((N + 1) / 2 + C::NF - 1) / C::NF, row_blocks = (L / 2 + 1 + C::NF - 1) / C::NF;
+    const int col_blocks = ((N + 1) / 2 + CC::NFC - 1) / CC::NFC, row_blocks = (L / 2 + 1 + C::NF - 1) / C::NF;
     const float2 *tw = p.tw_G;
     switch (which) {
     case 0:
-        if (set_smem(colpass_fwd_kernel<L>, C::SMEM)) return -1;
-        colpass_fwd_kernel<L><<<col_blocks, C::THREADS, C::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+        if (set_smem(colpass_fwd_kernel<L>, CC::SMEM)) return -1;
+        colpass_fwd_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
         break;
     case 1:
         if (set_smem(rowpass_fwd_kernel<L>, C::SMEM)) return -1;
@@ -226,8 +266,8 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
         rowpass_inv_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
         break;
     case 3:
-        if (set_smem(colpass_inv_kernel<L>, C::SMEM)) return -1;
-        colpass_inv_kernel<L><<<col_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N);
+        if (set_smem(colpass_inv_kernel<L>, CC::SMEM)) return -1;
+        colpass_inv_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N);
         break;
     default:
         return -1;

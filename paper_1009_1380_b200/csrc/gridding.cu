@@ -186,7 +186,9 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
                 accr = fmaf(rr, tp.wy[ly], accr);
                 acci = fmaf(ri, tp.wy[ly], acci);
             }
-            polar[(size_t)a * n_det + k] = make_float2(accr, acci);
+            // ghost k = n_det (Hermitian-half schedule, even n): F[a, j = -n/2] = conj F[a, j = +n/2]
+            if (k == n_det) polar[(size_t)a * n_det] = make_float2(accr, -acci);
+            else polar[(size_t)a * n_det + k] = make_float2(accr, acci);
         }
         sl = nx;
         r = rn;
@@ -259,7 +261,7 @@ __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
                const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
-               int G, int n_det)
+               int G, int n_det, int nyq_split)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *acc = reinterpret_cast<float2 *>(smem_raw);
@@ -289,8 +291,12 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         v = make_float2(0.f, 0.f);
         d = make_double2(0.0, 0.0);
         if (s.ak != SLOT_EMPTY) {
-            v = __ldg(&polar[(size_t)(s.ak >> 16) * n_det + (s.ak & 0xffff)]);
+            const int k = (int)(s.ak & 0xffff);
+            v = __ldg(&polar[(size_t)(s.ak >> 16) * n_det + (k == n_det ? 0 : k)]);
             d = __ldg(&cs[s.ak >> 16]);
+            // Hermitian-half schedule, even n: the unpaired Nyquist sample k = 0 (j = -n/2) and
+            // its ghost k = n (j = +n/2) carry half the value each, the ghost conjugated
+            if (nyq_split && (k == 0 || k == n_det)) v = make_float2(0.5f * v.x, k == 0 ? 0.5f * v.y : -0.5f * v.y);
         }
     };
     Slot s0 = load_slot(0), s1 = load_slot(1), s2 = load_slot(2), s3 = load_slot(3);
@@ -368,24 +374,93 @@ merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
     grid[(size_t)(j.ry0 + y) * G + j.rx0 + x] = make_float2(sr, si);
 }
 
-int launch_gather(const DevicePlan &p, const float2 *grid, float2 *polar, cudaStream_t st)
+// The j = 0 samples (k = n/2) of all angles sit at kappa = (0,0) and share one footprint, so
+// they are left out of the scatter schedules: their values are summed here (fixed order) and
+// the footprint is added once, after scatter + merge, one thread per cell (no atomics).
+// Full grid: V * wA(kx) wA(ky), wA = the rule-A taps [-W/2, W/2) of an exact tie (delta = 0).
+// Hermitian half (rows ky >= 0 only; the rows below are implied by symmetry): the Hermitian
+// part of that footprint, (V wA(kx) wA(ky) + conj(V) wB(kx) wB(ky)) / 2, wB(u) = wA(-u) the
+// mirrored taps (-W/2, W/2] (delta = 1) -- what the full gridding followed by Re{.} computes
+// (reading R-tie).
+constexpr int DC_THREADS = 256;
+static_assert((KW + 1) * (KW + 1) <= DC_THREADS, "one thread per cell of the (W+1)^2 window");
+__global__ void __launch_bounds__(DC_THREADS)
+dc_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, const float *__restrict__ g_lut,
+          const KbPoly kp, int G, int n_det, int n_angles, int half)
 {
-    if (p.n_gather_ctas == 0) return 0;
-    gather_kernel<<<p.n_gather_ctas, GATHER_THREADS, GATHER_SMEM, st>>>(
-        grid, polar, p.gather_ctas, p.gather_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
+    __shared__ float2 part[DC_THREADS];
+    const int t = threadIdx.x, cd = n_det / 2;
+    float sr = 0.f, si = 0.f;
+    for (int a0 = 0; a0 < n_angles; a0 += 8 * DC_THREADS) {      // 8 independent loads in flight
+        float2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int a = a0 + q * DC_THREADS + t;
+            v[q] = a < n_angles ? __ldg(&polar[(size_t)a * n_det + cd]) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { sr += v[q].x; si += v[q].y; }
+    }
+    part[t] = make_float2(sr, si);
+    __syncthreads();
+    for (int h = DC_THREADS / 2; h > 0; h >>= 1) {
+        if (t < h) { part[t].x += part[t + h].x; part[t].y += part[t + h].y; }
+        __syncthreads();
+    }
+    const float2 V = part[0];
+    float wa[KW], wb[KW];
+#if RADON_KB_LUT
+    lut_weights(g_lut, 0.f, wa);
+    lut_weights(g_lut, 1.f, wb);
+#else
+    kb_poly_weights(kp, 0.f, wa);
+    kb_poly_weights(kp, 1.f, wb);
+#endif
+    if (t >= (KW + 1) * (KW + 1)) return;
+    const int ux = t % (KW + 1) - KW / 2, uy = t / (KW + 1) - KW / 2;     // cell offset from DC: -W/2 .. W/2
+    auto tap = [](const float (&w)[KW], int l) {
+        float r = 0.f;
+#pragma unroll
+        for (int q = 0; q < KW; ++q) r = (q == l) ? w[q] : r;
+        return r;
+    };
+    const float a2 = tap(wa, ux + KW / 2) * tap(wa, uy + KW / 2);           // taps -W/2 .. W/2-1
+    const float b2 = tap(wb, ux + KW / 2 - 1) * tap(wb, uy + KW / 2 - 1);   // taps -W/2+1 .. W/2
+    float2 add;
+    if (half) {
+        if (uy < 0) return;
+        add = make_float2(0.5f * V.x * (a2 + b2), 0.5f * V.y * (a2 - b2));
+    } else {
+        add = make_float2(V.x * a2, V.y * a2);
+    }
+    if (a2 == 0.f && (b2 == 0.f || !half)) return;
+    float2 *cell = grid + (size_t)((G / 2 + uy) & (G - 1)) * G + ((G / 2 + ux) & (G - 1));
+    const float2 c = *cell;
+    *cell = make_float2(c.x + add.x, c.y + add.y);
+}
+
+int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *polar, cudaStream_t st)
+{
+    const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
+    if (q.n_gather_ctas == 0) return 0;
+    gather_kernel<<<q.n_gather_ctas, GATHER_THREADS, GATHER_SMEM, st>>>(
+        grid, polar, q.gather_ctas, q.gather_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
     count_launch();
     return 0;
 }
 
-int launch_scatter(const DevicePlan &p, const float2 *polar, float2 *grid, cudaStream_t st)
+int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, cudaStream_t st)
 {
-    scatter_kernel<<<p.n_scatter_ctas, SCATTER_THREADS, SCATTER_SMEM, st>>>(
-        polar, grid, p.scratch, p.scatter_ctas, p.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
+    const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
+    scatter_kernel<<<q.n_scatter_ctas, SCATTER_THREADS, SCATTER_SMEM, st>>>(
+        polar, grid, q.scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, (half && (p.n_det & 1) == 0) ? 1 : 0);
     count_launch();
-    if (p.n_merge_jobs > 0) {
-        merge_kernel<<<p.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(p.scratch, grid, p.merge_jobs, p.G);
+    if (q.n_merge_jobs > 0) {
+        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(q.scratch, grid, q.merge_jobs, p.G);
         count_launch();
     }
+    dc_kernel<<<1, DC_THREADS, 0, st>>>(polar, grid, p.lut, p.kb, p.G, p.n_det, p.n_angles, half ? 1 : 0);
+    count_launch();
     return 0;
 }
 

@@ -16,13 +16,16 @@ struct DevicePlan {
     float2 *tw_G = nullptr;       // twiddles for length G
     float2 *tw_P = nullptr;       // twiddles for length LP
     float2 *chirp_a = nullptr, *chirp_b = nullptr, *chirp_hf = nullptr;   // hf == nullptr: direct FFT
-    // schedules
-    GatherCta *gather_ctas = nullptr;   int n_gather_ctas = 0;
-    Slot *gather_slots = nullptr;
-    ScatterCta *scatter_ctas = nullptr; int n_scatter_ctas = 0;
-    Slot *scatter_slots = nullptr;
-    MergeJob *merge_jobs = nullptr;     int n_merge_jobs = 0;
-    float2 *scratch = nullptr;          // partial rectangles of split tiles
+    // schedules: [0] every sample / whole grid (arbitrary complex data: the test hooks),
+    //            [1] Hermitian half (real image / real sinogram: radon_forward, radon_adjoint)
+    struct Sched {
+        GatherCta *gather_ctas = nullptr;   int n_gather_ctas = 0;
+        Slot *gather_slots = nullptr;
+        ScatterCta *scatter_ctas = nullptr; int n_scatter_ctas = 0;
+        Slot *scatter_slots = nullptr;
+        MergeJob *merge_jobs = nullptr;     int n_merge_jobs = 0;
+        float2 *scratch = nullptr;          // partial rectangles of split tiles
+    } sched[2];
 };
 
 bool fft_length_supported(int L);
@@ -58,13 +61,18 @@ static inline int set_smem(F kernel, size_t bytes)
     }
 
 // F3 / A2 (+ merge)
-int launch_gather(const DevicePlan &p, const float2 *grid, float2 *polar, cudaStream_t st);
-int launch_scatter(const DevicePlan &p, const float2 *polar, float2 *grid, cudaStream_t st);
-// which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid; flag: also write the mirrored rows),
+// half: use the Hermitian-half schedule (sched[1]).  Gather: only k >= n/2 of every polar row
+// is written (plus k = 0 for even n, from the ghost sample); scatter: only grid rows
+// [G/2, G) and row 0 are written.
+int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *polar, cudaStream_t st);
+int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, cudaStream_t st);
+// which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid; flag 1: also write every mirrored row,
+// flag 2: only the mirrored rows the half gather reads, |ky| <= W/2 and |ky - G/2| <= W/2),
 // 2 rowpass_inv (grid -> T; flag: fold the mirrored rows in), 3 colpass_inv (T -> x).
 // T holds the rows ky = 0..G/2 only (Hermitian half), N complex each.
 int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st);
-// inv == false: sinogram -> polar (A1); inv == true: polar -> sinogram (F4)
-int launch_proj(bool inv, const DevicePlan &p, const float *in, float *out, cudaStream_t st);
+// inv == false: sinogram -> polar (A1); inv == true: polar -> sinogram (F4).  half (F4 only):
+// the polar rows hold k >= n/2 (and k = 0 for even n); the rest is their conjugate mirror.
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st);
 
 }  // namespace radon

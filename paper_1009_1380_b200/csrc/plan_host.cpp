@@ -298,27 +298,45 @@ static int build_rounds(std::vector<Cand> &cands, bool disjoint, int pitch,
 static inline int floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
 // ---------------------------------------------------------------- gather ---------
+// Samples a schedule covers.  Full: every (a, k), k < n_det.  Hermitian half (real image /
+// real sinogram: F[a,-j] = conj F[a,j]): the gather needs j >= 0 only, i.e. k in [n/2, n), plus,
+// for even n, the GHOST k = n (j = +n/2), the mirror image of the unpaired j = -n/2.
+static inline int half_k_begin(const Geometry &g) { return g.n_det / 2; }
+static inline int half_k_end(const Geometry &g) { return g.n_det + ((g.n_det & 1) ? 0 : 1); }
+// Samples the SCATTER schedules cover.  Full: k < n_det; Hermitian half: additionally the
+// Nyquist ghost k = n_det (even n).  In both, j = 0 (k = n/2) is LEFT OUT: it sits at
+// kappa = (0,0) for every angle, so its n_angles footprints coincide (they could only be
+// accumulated one per round); dc_kernel sums the n_angles values first and adds one footprint.
+static inline int scatter_k_end(const Geometry &g, bool half) { return half ? half_k_end(g) : g.n_det; }
+static inline bool scatter_k_valid(const Geometry &g, int k) { return k != g.n_det / 2; }
+
 static void build_gather(const Geometry &g, Schedules &out)
 {
     const int G = g.G;
-    const int ntx = (G + GT_X - 1) / GT_X, nty = (G + GT_Y - 1) / GT_Y;
-    const long long M = (long long)g.n_angles * g.n_det;
-    std::vector<uint32_t> count((size_t)ntx * nty + 1, 0);
+    const bool half = out.half;
+    const int k0 = half ? half_k_begin(g) : 0, k1 = half ? half_k_end(g) : g.n_det, nk = k1 - k0;
+    // half: bases of the j >= 0 samples lie in rows [G/2 - W/2, G - W/2]; tiles start there
+    const int yorg = half ? (int)posmod(G / 2 - KW / 2, G) : 0;
+    const int ntx = (G + GT_X - 1) / GT_X;
+    const long long M = (long long)g.n_angles * nk;
     std::vector<uint32_t> tile_of(M);
     std::vector<Cand> all(M);
+    int nty = 1;
     for (int a = 0; a < g.n_angles; ++a)
-        for (int k = 0; k < g.n_det; ++k) {
+        for (int k = k0; k < k1; ++k) {
             int x0, y0;
             g.base(a, k, x0, y0);
-            const int bx = (int)posmod(x0, G), by = (int)posmod(y0, G);
+            const int bx = (int)posmod(x0, G), by = (int)posmod(y0 - yorg, G);
             const int t = (by / GT_Y) * ntx + (bx / GT_X);
-            const long long m = (long long)a * g.n_det + k;
+            nty = std::max(nty, by / GT_Y + 1);
+            const long long m = (long long)a * nk + (k - k0);
             tile_of[m] = (uint32_t)t;
             all[m].ak = ((uint32_t)a << 16) | (uint32_t)k;
             all[m].lx = (int16_t)(bx % GT_X);
             all[m].ly = (int16_t)(by % GT_Y);
-            ++count[t + 1];
         }
+    std::vector<uint32_t> count((size_t)ntx * nty + 1, 0);
+    for (long long m = 0; m < M; ++m) ++count[tile_of[m] + 1];
     for (size_t t = 0; t < (size_t)ntx * nty; ++t) count[t + 1] += count[t];
     std::vector<uint32_t> order(M), fill(count.begin(), count.end() - 1);
     for (long long m = 0; m < M; ++m) order[fill[tile_of[m]]++] = (uint32_t)m;   // stable: (a,k) order
@@ -332,7 +350,7 @@ static void build_gather(const Geometry &g, Schedules &out)
         const int nr = build_rounds(cands, false, GT_PITCH, out.gather_slots, out.gather_filled);
         for (int r = 0; r < nr; r += GATHER_ROUND_CAP) {
             GatherCta c;
-            c.tx0 = (t % ntx) * GT_X; c.ty0 = (t / ntx) * GT_Y;
+            c.tx0 = (t % ntx) * GT_X; c.ty0 = (int)posmod(yorg + (t / ntx) * GT_Y, G);
             c.round_begin = rb + r;
             c.round_count = std::min(GATHER_ROUND_CAP, nr - r);
             out.gather_ctas.push_back(c);
@@ -345,11 +363,40 @@ static void build_gather(const Geometry &g, Schedules &out)
 // ---------------------------------------------------------------- scatter --------
 struct Image { uint32_t ak; int bx, by; };   // one wrap image of a sample: base cell (may be < 0)
 
+// Output rows a scatter schedule produces.  Full: [0, G).  Hermitian half (real sinogram: the
+// gridded spectrum is Hermitian, the 2-D inverse FFT reads ky = 0 .. G/2 only): centred rows
+// [G/2, G) and row 0 (ky = -G/2 == +G/2).  Samples: every (a, k), k < n_det, plus, for even n,
+// the ghost k = n (the kernel gives it half the conjugated value of k = 0, and k = 0 half its
+// own: Re{.} of the unpaired Nyquist sample).
+struct RowSeg { int y0, y1; };
+struct RectGeom { int rx0, ry0, rw, rh; };
+
+static void scatter_rects(const Geometry &g, bool half, std::vector<RowSeg> &segs, std::vector<RectGeom> &rects,
+                          std::vector<int> &seg_first)
+{
+    const int G = g.G;
+    segs.clear(); rects.clear(); seg_first.clear();
+    if (half) { segs.push_back(RowSeg{0, 1}); segs.push_back(RowSeg{G / 2, G}); }
+    else segs.push_back(RowSeg{0, G});
+    for (const RowSeg &sg : segs) {
+        seg_first.push_back((int)rects.size());
+        for (int ry0 = sg.y0; ry0 < sg.y1; ry0 += SR_Y)
+            for (int rx0 = 0; rx0 < G; rx0 += SR_X)
+                rects.push_back(RectGeom{rx0, ry0, std::min(SR_X, G - rx0), std::min(SR_Y, sg.y1 - ry0)});
+    }
+}
+
 static void build_scatter(const Geometry &g, Schedules &out)
 {
     const int G = g.G;
-    const int nrx = (G + SR_X - 1) / SR_X, nry = (G + SR_Y - 1) / SR_Y;
-    const int nrect = nrx * nry;
+    const bool half = out.half;
+    const int k_end = scatter_k_end(g, half);
+    const int nrx = (G + SR_X - 1) / SR_X;
+    std::vector<RowSeg> segs;
+    std::vector<RectGeom> rects;
+    std::vector<int> seg_first;
+    scatter_rects(g, half, segs, rects, seg_first);
+    const int nrect = (int)rects.size();
     // pass 1: count incidences (image, rect); pass 2: fill
     std::vector<uint32_t> count((size_t)nrect + 1, 0);
     std::vector<Image> inc;
@@ -361,7 +408,8 @@ static void build_scatter(const Geometry &g, Schedules &out)
             fill.assign(count.begin(), count.end() - 1);
         }
         for (int a = 0; a < g.n_angles; ++a)
-            for (int k = 0; k < g.n_det; ++k) {
+            for (int k = 0; k < k_end; ++k) {
+                if (!scatter_k_valid(g, k)) continue;
                 int x0, y0;
                 g.base(a, k, x0, y0);
                 for (int sy = -1; sy <= 1; ++sy) {
@@ -371,13 +419,17 @@ static void build_scatter(const Geometry &g, Schedules &out)
                         const int bx = x0 + sx * G;
                         if (bx + KH < 0 || bx > G - 1) continue;
                         const int rx_lo = std::max(bx, 0) / SR_X, rx_hi = std::min(bx + KH, G - 1) / SR_X;
-                        const int ry_lo = std::max(by, 0) / SR_Y, ry_hi = std::min(by + KH, G - 1) / SR_Y;
-                        for (int ry = ry_lo; ry <= ry_hi; ++ry)
-                            for (int rx = rx_lo; rx <= rx_hi; ++rx) {
-                                const int r = ry * nrx + rx;
-                                if (pass == 0) ++count[r + 1];
-                                else inc[fill[r]++] = Image{((uint32_t)a << 16) | (uint32_t)k, bx, by};
-                            }
+                        for (size_t sg = 0; sg < segs.size(); ++sg) {
+                            const int ylo = std::max(by, segs[sg].y0), yhi = std::min(by + KH, segs[sg].y1 - 1);
+                            if (ylo > yhi) continue;
+                            const int ry_lo = (ylo - segs[sg].y0) / SR_Y, ry_hi = (yhi - segs[sg].y0) / SR_Y;
+                            for (int ry = ry_lo; ry <= ry_hi; ++ry)
+                                for (int rx = rx_lo; rx <= rx_hi; ++rx) {
+                                    const int r = seg_first[sg] + ry * nrx + rx;
+                                    if (pass == 0) ++count[r + 1];
+                                    else inc[fill[r]++] = Image{((uint32_t)a << 16) | (uint32_t)k, bx, by};
+                                }
+                        }
                     }
                 }
             }
@@ -389,8 +441,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
     std::vector<Slot> tmp_slots;
 
     for (int r = 0; r < nrect; ++r) {
-        const int rx0 = (r % nrx) * SR_X, ry0 = (r / nrx) * SR_Y;
-        const int rw = std::min(SR_X, G - rx0), rh = std::min(SR_Y, G - ry0);
+        const int rx0 = rects[r].rx0, ry0 = rects[r].ry0, rw = rects[r].rw, rh = rects[r].rh;
         const int nsx = (rw + ST_X - 1) / ST_X, nsy = (rh + ST_Y - 1) / ST_Y;
         const uint32_t lo = count[r], hi = count[r + 1];
 
@@ -470,9 +521,10 @@ static void build_scatter(const Geometry &g, Schedules &out)
     for (auto &p : ctas) out.scatter_ctas.push_back(p.cta);
 }
 
-void build_schedules(const Geometry &g, Schedules &out)
+void build_schedules(const Geometry &g, Schedules &out, bool half)
 {
     out = Schedules();
+    out.half = half;
     build_gather(g, out);
     build_scatter(g, out);
 }
@@ -489,7 +541,12 @@ long long check_schedules(const Geometry &g, const Schedules &s)
 {
     long long bad = 0;
     const int G = g.G;
-    const long long M = (long long)g.n_angles * g.n_det;
+    const bool half = s.half;
+    const int kg0 = half ? half_k_begin(g) : 0, kg1 = half ? half_k_end(g) : g.n_det;   // gather samples
+    const int ks1 = scatter_k_end(g, half);                                              // scatter samples
+    const int nkg = kg1 - kg0;
+    const long long M = (long long)g.n_angles * nkg;
+    auto row_needed = [&](int cy) { return !half || cy == 0 || cy >= G / 2; };
 
     // Pairwise (brute force, independent of the builder's bitmap): bank pairs distinct per
     // half-warp; for the scatter, no two lanes of a round with the same base row and base
@@ -512,7 +569,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
     // gather: every sample exactly once, at the right place
     std::vector<uint8_t> seen(M, 0);
     for (const GatherCta &c : s.gather_ctas) {
-        if (c.tx0 % GT_X || c.ty0 % GT_Y || c.tx0 < 0 || c.ty0 < 0 || c.tx0 >= G || c.ty0 >= G) ++bad;
+        if (c.tx0 % GT_X || c.tx0 < 0 || c.ty0 < 0 || c.tx0 >= G || c.ty0 >= G) ++bad;
         if (c.round_count < 1 || c.round_count > GATHER_ROUND_CAP) ++bad;
         for (int r = 0; r < c.round_count; ++r) {
             const Slot *lanes = &s.gather_slots[(size_t)(c.round_begin + r) * 32];
@@ -520,13 +577,13 @@ long long check_schedules(const Geometry &g, const Schedules &s)
             for (int l = 0; l < 32; ++l) {
                 if (lanes[l].ak == SLOT_EMPTY) continue;
                 const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;
-                if (a >= g.n_angles || k >= g.n_det) { ++bad; continue; }
+                if (a >= g.n_angles || k < kg0 || k >= kg1) { ++bad; continue; }
                 int x0, y0;
                 g.base(a, k, x0, y0);
                 const int lx = lanes[l].lxy & 0xffff, ly = lanes[l].lxy >> 16;
                 if (lx >= GT_X || ly >= GT_Y) ++bad;
                 if (posmod(c.tx0 + lx - x0, G) != 0 || posmod(c.ty0 + ly - y0, G) != 0) ++bad;
-                if (seen[(size_t)a * g.n_det + k]++) ++bad;
+                if (seen[(size_t)a * nkg + (k - kg0)]++) ++bad;
             }
         }
     }
@@ -536,13 +593,16 @@ long long check_schedules(const Geometry &g, const Schedules &s)
     std::vector<uint64_t> expect((size_t)G * G, 0), got((size_t)G * G, 0);
     std::vector<uint8_t> written((size_t)G * G, 0);
     for (int a = 0; a < g.n_angles; ++a)
-        for (int k = 0; k < g.n_det; ++k) {
+        for (int k = 0; k < ks1; ++k) {
+            if (!scatter_k_valid(g, k)) continue;
             int x0, y0;
             g.base(a, k, x0, y0);
             const uint32_t ak = ((uint32_t)a << 16) | (uint32_t)k;
             for (int ty = 0; ty < KW; ++ty)
-                for (int tx = 0; tx < KW; ++tx)
-                    expect[(size_t)posmod(y0 + ty, G) * G + posmod(x0 + tx, G)] += tap_hash(ak, tx, ty);
+                for (int tx = 0; tx < KW; ++tx) {
+                    const int cy = (int)posmod(y0 + ty, G);
+                    if (row_needed(cy)) expect[(size_t)cy * G + posmod(x0 + tx, G)] += tap_hash(ak, tx, ty);
+                }
         }
     std::vector<int> slot_owner(s.n_partial_slots, 0);
     for (const ScatterCta &c : s.scatter_ctas) {
@@ -577,7 +637,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
                 for (int l = 0; l < 32; ++l) {
                     if (lanes[l].ak == SLOT_EMPTY) continue;
                     const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;
-                    if (a >= g.n_angles || k >= g.n_det) { ++bad; continue; }
+                    if (a >= g.n_angles || k >= ks1 || !scatter_k_valid(g, k)) { ++bad; continue; }
                     int x0, y0;
                     g.base(a, k, x0, y0);
                     const int bx = ax0 - KH + (int)(lanes[l].lxy & 0xffff), by = ay0 - KH + (int)(lanes[l].lxy >> 16);
@@ -599,7 +659,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
             for (int x = 0; x < mj.rw; ++x) ++written[(size_t)(mj.ry0 + y) * G + mj.rx0 + x];
     }
     for (size_t i = 0; i < (size_t)G * G; ++i) {
-        if (written[i] != 1) ++bad;
+        if (written[i] != (row_needed((int)(i / (size_t)G)) ? 1 : 0)) ++bad;
         if (got[i] != expect[i]) ++bad;
     }
     return bad;

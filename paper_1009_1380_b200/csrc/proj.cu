@@ -27,7 +27,7 @@ template <int L, bool INV>
 __global__ void __launch_bounds__(ProjCfg<L>::THREADS)
 proj_kernel(const float *__restrict__ in, float *__restrict__ out,
             const float2 *__restrict__ ta, const float2 *__restrict__ tb,
-            const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows)
+            const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows, int half)
 {
     extern __shared__ __align__(16) float2 s_fft[];
     using C = ProjCfg<L>;
@@ -45,7 +45,11 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
         if (live && sidx < n) {
             const float2 a = __ldg(&ta[sidx]);
             if (INV) {
-                const float2 p = __ldg(&reinterpret_cast<const float2 *>(in)[(size_t)row * n + sidx]);
+                // half: the row holds k >= n/2 (and k = 0 for even n); P[c - j] = conj P[c + j]
+                const int c = n >> 1;
+                const bool mir = half && sidx < c && !(sidx == 0 && (n & 1) == 0);
+                float2 p = __ldg(&reinterpret_cast<const float2 *>(in)[(size_t)row * n + (mir ? 2 * c - sidx : sidx)]);
+                if (mir) p.y = -p.y;
                 v[i] = make_float2(p.x * a.x + p.y * a.y, p.x * a.y - p.y * a.x);   // conj(p) * a
             } else {
                 const float y = __ldg(&in[(size_t)row * n + sidx]);
@@ -73,24 +77,24 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
 }
 
 template <int L>
-static int proj_launch(bool inv, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
+static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
 {
     using C = ProjCfg<L>;
     const int blocks = (p.n_angles + C::NF - 1) / C::NF;
     if (inv) {
         if (set_smem(proj_kernel<L, true>, C::SMEM)) return -1;
-        proj_kernel<L, true><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles);
+        proj_kernel<L, true><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);
     } else {
         if (set_smem(proj_kernel<L, false>, C::SMEM)) return -1;
-        proj_kernel<L, false><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles);
+        proj_kernel<L, false><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);
     }
     count_launch();
     return 0;
 }
 
-int launch_proj(bool inv, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
 {
-    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, p, in, out, st);)
+    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, half, p, in, out, st);)
     return -1;
 }
 

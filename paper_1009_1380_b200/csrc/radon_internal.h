@@ -123,10 +123,13 @@ struct Schedules {
     std::vector<ScatterCta> scatter_ctas;
     std::vector<MergeJob> merge_jobs;
     int n_partial_slots = 0;
+    bool half = false;
     long long gather_filled = 0, scatter_filled = 0;
 };
 
-void build_schedules(const Geometry &g, Schedules &out);
+// half == false: every sample, the whole grid (arbitrary complex data: the test hooks).
+// half == true:  Hermitian half for real images / sinograms (radon_forward, radon_adjoint).
+void build_schedules(const Geometry &g, Schedules &out, bool half);
 // Returns the number of violated invariants (0 = schedules are valid).
 long long check_schedules(const Geometry &g, const Schedules &s);
 
