@@ -34,14 +34,24 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def stage_bytes(N, G, M):
-    """Algorithmic bytes per launch of each stage."""
+def stage_bytes(N, G, M, n_angles, W=6):
+    """Algorithmic bytes per launch of each stage of radon_forward / radon_adjoint (DESIGN.md
+    section 7).  Image and sinogram are real, so the path moves the HERMITIAN HALF of the
+    spectrum: grid rows ky = 0..G/2 (+ W halo rows for the gather), T = (G/2+1) x N, polar
+    samples j >= 0 in the forward direction.  These are half of SURVEY.md 8(d)'s full-complex
+    figures (kept for the bare gridding kernels, see gridding_bytes)."""
+    H = G // 2 + 1
     return {
-        "F1_colfft": 4 * N * N + 8 * G * N, "F2_rowfft": 8 * G * N + 8 * G * G,
-        "F3_gather": 8 * G * G + 8 * M, "F4_proj_ifft": 8 * M + 4 * M,
-        "A1_proj_fft": 4 * M + 8 * M, "A2_scatter": 8 * M + 8 * G * G,
-        "A3_rowifft": 8 * G * G + 8 * G * N, "A4_colifft": 8 * G * N + 4 * N * N,
+        "F1_colfft": 4 * N * N + 8 * H * N, "F2_rowfft": 8 * H * N + 8 * (H + W) * G,
+        "F3_gather": 8 * (H + W) * G + 8 * (M // 2 + n_angles), "F4_proj_ifft": 8 * (M // 2 + n_angles) + 4 * M,
+        "A1_proj_fft": 4 * M + 8 * M, "A2_scatter": 8 * M + 8 * H * G,
+        "A3_rowifft": 8 * H * G + 8 * H * N, "A4_colifft": 8 * H * N + 4 * N * N,
     }
+
+
+def gridding_bytes(G, M):
+    """bare gridding / inverse gridding on arbitrary complex data."""
+    return 8 * G * G + 8 * M
 
 
 class ClockSampler:
@@ -58,7 +68,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -66,9 +76,16 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def wait_first(self, timeout=5.0):
+        """nvidia-smi takes a moment to start: block until its first sample arrives."""
+        t0 = time.perf_counter()
+        while self.proc and not self.lines and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+
+    def stop(self, t_begin=None, t_end=None):
+        """Samples taken in [t_begin, t_end] (host clock); all samples if the window is None."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -78,7 +95,9 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        for ts, ln in self.lines:
+            if t_begin is not None and not (t_begin <= ts <= t_end):
+                continue
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -199,11 +218,13 @@ def main():
 
     sampler = ClockSampler(local_rank)
     sampler.start()
+    sampler.wait_first()
     stream = torch.cuda.current_stream()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     plan.stage_timing(True)
     rdist.barrier(); torch.cuda.synchronize()
     n0 = rb.kernel_launch_count()
+    t_host0 = time.perf_counter()
     ev0.record(stream)
     for _ in range(args.steps):
         step()
@@ -212,7 +233,14 @@ def main():
     launches = rb.kernel_launch_count() - n0
     plan.stage_timing(False)
     stages = plan.stage_times()
-    clocks = sampler.stop()
+    # the timed region is tens of ms: keep the GPU under the identical load a little longer so
+    # that nvidia-smi (20 ms period) sees the clocks this workload runs at
+    t_load_end = time.perf_counter() + 0.5
+    while time.perf_counter() < t_load_end:
+        step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop(t_host0, time.perf_counter())
+    clocks["window"] = "timed region + 0.5 s of identical untimed steps, nvidia-smi -lms 20"
     t_ms = rdist.max_over_ranks(ev0.elapsed_time(ev1), dev)
     pairs = world * B * args.steps
     value = pairs / (t_ms * 1e-3)
@@ -243,7 +271,7 @@ def main():
 
     # ---- roofline of the dominant kernel (stage with the largest device time) -----------
     peak, peak_src = measured_peaks()
-    sbytes = stage_bytes(cfg.N, plan.G, cfg.M)
+    sbytes = stage_bytes(cfg.N, plan.G, cfg.M, cfg.n_angles)
     per_stage = {}
     for k, (ms, n) in stages.items():
         if n:
@@ -266,6 +294,34 @@ def main():
                     "algorithmic_bytes_per_launch": sbytes[dom],
                     "us_per_launch": per_stage[dom]["us_per_launch"]}
 
+    # ---- the bare gridding kernels on arbitrary complex data (north_star: >= 50 % of the HBM
+    #      roofline at this config): radon_interp_only (F3) and radon_grid_only (A2 + merge + dc),
+    #      full grid / every sample, timed alone with CUDA events on the launching stream -----
+    gk = {}
+    gen = torch.Generator(device=dev); gen.manual_seed(1234 + rank)
+    cgrid = torch.view_as_complex(torch.randn((plan.G, plan.G, 2), device=dev, generator=gen))
+    cpol = torch.view_as_complex(torch.randn((cfg.n_angles, cfg.n_det, 2), device=dev, generator=gen))
+    ogrid, opol = torch.empty_like(cgrid), torch.empty_like(cpol)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    gbytes = gridding_bytes(plan.G, cfg.M)
+    for name, fn in (("interp_only", lambda: plan.radon_interp_only(cgrid, opol)),
+                     ("grid_only", lambda: plan.radon_grid_only(cpol, ogrid))):
+        for _ in range(3):
+            fn()
+        tot, reps = 0.0, 5
+        for _ in range(reps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream)
+            torch.cuda.synchronize()
+            tot += e0.elapsed_time(e1)
+        us = tot / reps * 1e3
+        gk[name] = {"us_per_call": round(us, 2), "algorithmic_MB": round(gbytes / 1e6, 1),
+                    "GBps": round(gbytes / (us * 1e-6) / 1e9, 1),
+                    "frac_of_hbm_peak": round(gbytes / (us * 1e-6) / 1e9 / peak, 4),
+                    "samples_per_s": cfg.M / (us * 1e-6), "l2": "flushed (256 MB memset) before every call"}
+    del cgrid, cpol, ogrid, opol, flush
+
     if rank != 0:
         return 0
     cpu_baseline = None
@@ -283,7 +339,7 @@ def main():
                    "l2": f"inputs {B * cfg.N * cfg.N * 4 / 1e6:.0f} MB/step cycle through HBM (> 126 MB L2); per-slice grid 134 MB > L2"},
         "samples_per_s": 2.0 * cfg.M * value, "us_per_pair": t_pair_us,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": roofline, "stages": per_stage, "cpu_baseline": cpu_baseline,
+        "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line))
     return 0

@@ -21,10 +21,12 @@ struct ProjCfg {
     static constexpr int THREADS = NF * TF;
     static constexpr int PADLEN = fft_padded_len(L);
     static constexpr size_t SMEM = (size_t)NF * PADLEN * sizeof(float2);
+    static constexpr int MIN_CTAS = 1024 / THREADS;      // <= 64 registers per thread
 };
 
-template <int L, bool INV>
-__global__ void __launch_bounds__(ProjCfg<L>::THREADS)
+// BLUE: Bluestein form (two FFTs); false: n == L is a power of two, one FFT.
+template <int L, bool INV, bool BLUE>
+__global__ void __launch_bounds__(ProjCfg<L>::THREADS, BLUE ? 1 : ProjCfg<L>::MIN_CTAS)
 proj_kernel(const float *__restrict__ in, float *__restrict__ out,
             const float2 *__restrict__ ta, const float2 *__restrict__ tb,
             const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows, int half)
@@ -58,7 +60,7 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
         }
     }
     fft_reg<L, -1>(v, s, tw, t);
-    if (hf != nullptr) {
+    if constexpr (BLUE) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], __ldg(&hf[t + i * TF]));
         __syncthreads();
@@ -81,13 +83,18 @@ static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in
 {
     using C = ProjCfg<L>;
     const int blocks = (p.n_angles + C::NF - 1) / C::NF;
-    if (inv) {
-        if (set_smem(proj_kernel<L, true>, C::SMEM)) return -1;
-        proj_kernel<L, true><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);
-    } else {
-        if (set_smem(proj_kernel<L, false>, C::SMEM)) return -1;
-        proj_kernel<L, false><<<blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);
+#define RADON_PROJ(INV_, BLUE_)                                                                          \
+    {                                                                                                    \
+        if (set_smem(proj_kernel<L, INV_, BLUE_>, C::SMEM)) return -1;                                   \
+        proj_kernel<L, INV_, BLUE_><<<blocks, C::THREADS, C::SMEM, st>>>(                                \
+            in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);       \
     }
+    const bool blue = p.chirp_hf != nullptr;
+    if (inv && blue) RADON_PROJ(true, true)
+    else if (inv) RADON_PROJ(true, false)
+    else if (blue) RADON_PROJ(false, true)
+    else RADON_PROJ(false, false)
+#undef RADON_PROJ
     count_launch();
     return 0;
 }
