@@ -127,6 +127,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     p->M = (long long)n_angles * n_det;
     DevicePlan &d = p->dev;
     d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det;
+    d.n_sm = prop.multiProcessorCount;
     const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
     d.LP = pow2 ? n_det : std::max(16, next_pow2(2 * n_det - 1));
 

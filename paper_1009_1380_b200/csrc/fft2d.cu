@@ -18,7 +18,10 @@
 // 8 G^2-byte grid is a contiguous row.  T = (G/2+1) x N c64 (33.6 MB at config 4) is written
 // and read back within one call and stays L2-resident.
 #include "kernels.h"
+
+#include <algorithm>
 #include "fft_device.cuh"
+#include "async_copy.cuh"
 
 namespace radon {
 
@@ -188,6 +191,71 @@ rowpass_inv_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
     }
 }
 
+// ---- first half of A3, Hermitian-half form: grid rows ky = 0..L/2 as they are -> T ------------
+// Persistent CTAs; the copy engine fetches the NEXT group of rows (one bulk copy per row)
+// into a staging buffer while the warps transform the current one, so the DRAM latency of
+// the row reads is off the critical path (ncu, round 1b: the per-thread-load version issued
+// on 32 % of cycles, waiting on its 16 loads per thread).
+template <int L>
+struct RowStageCfg {
+    using C = FftCfg<L>;
+    static constexpr size_t STAGE_BYTES = (size_t)C::NF * L * sizeof(float2);
+    static constexpr size_t SMEM = C::SMEM + STAGE_BYTES;
+};
+
+template <int L>
+__global__ void __launch_bounds__(FftCfg<L>::THREADS)
+rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
+                          const float2 *__restrict__ tw, int N, int n_groups)
+{
+    extern __shared__ __align__(128) float2 s_fft[];
+    using C = FftCfg<L>;
+    constexpr int TF = C::TF, NF = C::NF;
+    __shared__ __align__(8) uint64_t bar;
+    float2 *stage = s_fft + NF * C::PADLEN;                 // NF rows of L, 16-byte aligned
+    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
+    float2 *s = s_fft + f * C::PADLEN;
+    const int c = N / 2;
+
+    auto fetch = [&](int g) {                               // one thread: rows of group g -> stage
+        int n_live = 0;
+        for (int q = 0; q < NF; ++q) n_live += (g * NF + q <= L / 2) ? 1 : 0;
+        mbar_expect_tx(&bar, (uint32_t)(n_live * L * sizeof(float2)));
+        for (int q = 0; q < NF; ++q) {
+            const int ky = g * NF + q;
+            if (ky > L / 2) break;
+            const int cy = (ky + L / 2) & (L - 1);
+            bulk_g2s(stage + q * L, grid + (size_t)cy * L, (uint32_t)(L * sizeof(float2)), &bar);
+        }
+    };
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        if ((int)blockIdx.x < n_groups) fetch(blockIdx.x);
+    }
+    __syncthreads();
+    uint32_t parity = 0;
+    for (int g = blockIdx.x; g < n_groups; g += gridDim.x) {
+        const int ky = g * NF + f;
+        const bool live = ky <= L / 2;
+        mbar_wait(&bar, parity);
+        parity ^= 1u;
+        float2 v[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            v[i] = live ? stage[f * L + ((t + i * TF + L / 2) & (L - 1))] : make_float2(0.f, 0.f);
+        __syncthreads();                                    // stage is free; s is free (previous FFT done)
+        if (threadIdx.x == 0 && g + (int)gridDim.x < n_groups) fetch(g + gridDim.x);
+        fft_reg<L, +1>(v, s, tw, t);
+        if (live) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const int ix = (t + i * TF + c) & (L - 1);
+                if (ix < N) T[(size_t)ky * N + ix] = v[i];
+            }
+        }
+    }
+}
+
 // ---- second half of A3 + A4: column pairs of T -> image ---------------------------------------
 template <int L>
 __global__ void __launch_bounds__(ColCfg<L>::THREADS)
@@ -262,8 +330,16 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
         rowpass_fwd_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
         break;
     case 2:
-        if (set_smem(rowpass_inv_kernel<L>, C::SMEM)) return -1;
-        rowpass_inv_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+        if (flag) {
+            if (set_smem(rowpass_inv_kernel<L>, C::SMEM)) return -1;
+            rowpass_inv_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+        } else {
+            using RS = RowStageCfg<L>;
+            if (set_smem(rowpass_inv_staged_kernel<L>, RS::SMEM)) return -1;
+            const int per_sm = std::max(1, std::min(8, (int)((220u << 10) / (RS::SMEM + 1024))));
+            const int ctas = std::min(row_blocks, p.n_sm * per_sm);
+            rowpass_inv_staged_kernel<L><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+        }
         break;
     case 3:
         if (set_smem(colpass_inv_kernel<L>, CC::SMEM)) return -1;

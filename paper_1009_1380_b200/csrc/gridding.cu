@@ -6,6 +6,7 @@
 //   colpass/rowpass  F1+F2 / A3+A4  de-apodise + zero-pad + 2-D FFT, and the transposed chain
 //   proj kernels     F4 / A1  centred 1-D DFTs along the projections (Bluestein for any n_det)
 #include "kernels.h"
+#include "async_copy.cuh"
 
 #include <atomic>
 
@@ -72,39 +73,6 @@ __device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__re
     const float4 *src = reinterpret_cast<const float4 *>(g_lut);
     float4 *dst = reinterpret_cast<float4 *>(s_lut);
     for (int i = threadIdx.x; i < LUT_S * LUT_ROW / 4; i += blockDim.x) dst[i] = __ldg(&src[i]);
-}
-
-// =====================================================================================
-// Bulk asynchronous copies (TMA engine, sm_90+): global -> shared, completion on an mbarrier
-// =====================================================================================
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// 16-byte aligned src/dst, bytes a multiple of 16
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
 // =====================================================================================

@@ -8,6 +8,7 @@ namespace radon {
 
 struct DevicePlan {
     int N = 0, G = 0, n_angles = 0, n_det = 0, LP = 0;   // LP: FFT length of the projection DFT
+    int n_sm = 148;               // multiprocessors of the device (persistent grids)
     // tables
     double2 *cs = nullptr;        // per angle (G/n)(cos, sin), fp64
     float *lut = nullptr;         // LUT_S x LUT_ROW (only with RADON_KB_LUT)
