@@ -49,6 +49,14 @@ def stage_bytes(N, G, M, n_angles, W=6):
     }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 4, from the ncu --set full
+# captures summarised in profiles/r01c_hermitian_half_kernels.md (A2 = scatter + merge + dc).
+NCU_DRAM_BYTES = {
+    "F1_colfft": 16.87e6, "F2_rowfft": 45.46e6, "F3_gather": 67.98e6, "F4_proj_ifft": 8.59e6,
+    "A1_proj_fft": 8.46e6, "A2_scatter": 48.83e6, "A3_rowifft": 74.34e6, "A4_colifft": 33.68e6,
+}
+
+
 def gridding_bytes(G, M):
     """bare gridding / inverse gridding on arbitrary complex data."""
     return 8 * G * G + 8 * M
@@ -175,6 +183,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=512)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-clock-load", action="store_true",
+                    help="skip the 0.5 s of untimed identical steps that give nvidia-smi time to sample "
+                         "(profiling runs: keeps the kernel launch list short and deterministic)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -236,7 +247,7 @@ def main():
     # the timed region is tens of ms: keep the GPU under the identical load a little longer so
     # that nvidia-smi (20 ms period) sees the clocks this workload runs at
     t_load_end = time.perf_counter() + 0.5
-    while time.perf_counter() < t_load_end:
+    while not args.no_clock_load and time.perf_counter() < t_load_end:
         step()
         torch.cuda.synchronize()
     clocks = sampler.stop(t_host0, time.perf_counter())
@@ -281,11 +292,7 @@ def main():
                             "GBps": round(sbytes[k] / (us * 1e-6) / 1e9, 1),
                             "frac_of_hbm_peak": round(sbytes[k] / (us * 1e-6) / 1e9 / peak, 4)}
     dom = max(per_stage, key=lambda k: per_stage[k]["us_per_launch"] * per_stage[k]["launches_timed"]) if per_stage else None
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_dram_traffic.json")
-    if dom and os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(dom, {}).get("dram_bytes_per_launch")
+    traffic = NCU_DRAM_BYTES.get(dom) if (dom and cfg.N == 2048) else None
     roofline = None
     if dom:
         ach = per_stage[dom]["GBps"]
