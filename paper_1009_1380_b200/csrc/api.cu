@@ -101,7 +101,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     cudaFree(d.cs); cudaFree(d.lut); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
     cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
     for (auto &q : d.sched) {
-        cudaFree(q.gather_ctas); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
+        cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
         cudaFree(q.merge_jobs); cudaFree(q.scratch);
     }
     for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.img); cudaFree(w.sino); }
@@ -154,7 +154,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     // P3: schedules
     for (int h = 0; h < 2; ++h) {
         Schedules sch;
-        build_schedules(p->geo, sch, h == 1);
+        build_schedules(p->geo, sch, h == 1, d.n_sm);
         DevicePlan::Sched &q = d.sched[h];
         p->gather_slots[h] = (long long)sch.gather_slots.size(); p->gather_filled[h] = sch.gather_filled;
         p->scatter_slots[h] = (long long)sch.scatter_slots.size(); p->scatter_filled[h] = sch.scatter_filled;
@@ -162,6 +162,8 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         q.n_scatter_ctas = (int)sch.scatter_ctas.size();
         q.n_merge_jobs = (int)sch.merge_jobs.size();
         if ((rc = dev_upload(p, &q.gather_ctas, sch.gather_ctas))) return rc;
+        q.n_gather_workers = (int)sch.gather_worker_begin.size() - 1;
+        if ((rc = dev_upload(p, &q.gather_worker_begin, sch.gather_worker_begin))) return rc;
         if ((rc = dev_upload(p, &q.gather_slots, sch.gather_slots))) return rc;
         if ((rc = dev_upload(p, &q.scatter_ctas, sch.scatter_ctas))) return rc;
         if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;

@@ -43,7 +43,10 @@ struct FftCfg {
 template <int L>
 struct ColCfg {
     static constexpr int TF = L / 16;
-    static constexpr int NFC_WANT = (128 / TF > 4) ? 128 / TF : 4;
+#ifndef RADON_COL_NFC
+#define RADON_COL_NFC 4
+#endif
+    static constexpr int NFC_WANT = (128 / TF > RADON_COL_NFC) ? 128 / TF : RADON_COL_NFC;
     static constexpr int NFC = (NFC_WANT * TF > 1024) ? 1024 / TF : NFC_WANT;   // column pairs per CTA
     static constexpr int THREADS = NFC * TF;
     static constexpr int SKEW = (16 / NFC > 1) ? 16 / NFC : 1;   // pairs start in distinct bank pairs
@@ -204,7 +207,7 @@ struct RowStageCfg {
 };
 
 template <int L>
-__global__ void __launch_bounds__(FftCfg<L>::THREADS)
+__global__ void __launch_bounds__(FftCfg<L>::THREADS, (FftCfg<L>::THREADS <= 256) ? 3 : 1)
 rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
                           const float2 *__restrict__ tw, int N, int n_groups)
 {
@@ -243,6 +246,10 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
 #pragma unroll
         for (int i = 0; i < 16; ++i)
             v[i] = live ? stage[f * L + ((t + i * TF + L / 2) & (L - 1))] : make_float2(0.f, 0.f);
+        // The staging buffer is read through the generic proxy and refilled through the async
+        // proxy: without this fence the refill can overtake reads still in flight (observed:
+        // run-to-run differences of 2 % in the adjoint).
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();                                    // stage is free; s is free (previous FFT done)
         if (threadIdx.x == 0 && g + (int)gridDim.x < n_groups) fetch(g + gridDim.x);
         fft_reg<L, +1>(v, s, tw, t);

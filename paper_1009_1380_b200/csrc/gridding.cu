@@ -78,91 +78,139 @@ __device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__re
 // =====================================================================================
 // F3: inverse gridding (gather)
 // =====================================================================================
-// One CTA = one GT_X x GT_Y tile of the grid (+KH halo up/right) and up to GATHER_ROUND_CAP
-// rounds of 32 samples whose footprints start inside the tile.  The tile is staged by the
-// copy engine (one bulk copy per tile row, rows and columns wrapped mod G) while the warps
-// already fetch their first slots and evaluate the Kaiser-Bessel weights; the 36 taps of a
-// sample are 64-bit shared-memory loads that the plan-time schedule made conflict free.
-constexpr int GATHER_THREADS = GATHER_WARPS * 32;
+// Persistent CTAs, one per multiprocessor.  A work item = one GT_X x GT_Y tile of the grid
+// (+KH halo up/right) and up to GATHER_ROUND_CAP rounds of 32 samples whose footprints start
+// inside the tile; the plan assigns items to CTAs (longest first onto the least loaded).
+// A producer warp keeps GATHER_STAGES tiles in flight through the copy engine (one bulk copy
+// per tile row, rows and columns wrapped mod G; "full" mbarriers count the bytes), so the HBM
+// reads never wait for the interpolation; GATHER_WARPS consumer warps take the rounds of the
+// CTA's items round-robin (balanced whatever the item sizes) and hand a tile back through an
+// "empty" mbarrier.  The 36 taps of a sample are 64-bit shared-memory loads that the
+// plan-time schedule made conflict free; slots are fetched two rounds ahead, ray directions one.
+constexpr int GATHER_THREADS = (GATHER_WARPS + 1) * 32;
 constexpr size_t LUT_SMEM = RADON_KB_LUT ? (size_t)LUT_S * LUT_ROW * sizeof(float) : 0;
 constexpr size_t GATHER_TILE_BYTES = (size_t)GT_ROWS * GT_PITCH * sizeof(float2);
-constexpr size_t GATHER_SMEM = GATHER_TILE_BYTES + LUT_SMEM;
+constexpr size_t GATHER_SMEM = GATHER_STAGES * GATHER_TILE_BYTES + LUT_SMEM;
 static_assert((GT_PITCH * sizeof(float2)) % 16 == 0 && GT_X % 2 == 0, "bulk copies need 16-byte rows");
+static_assert(GATHER_TILE_BYTES % 16 == 0, "stage buffers stay 16-byte aligned");
 
-__global__ void __launch_bounds__(GATHER_THREADS, GATHER_CTAS_PER_SM)
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+__global__ void __launch_bounds__(GATHER_THREADS, 1)
 gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
-              const GatherCta *__restrict__ ctas, const Slot *__restrict__ slots,
+              const GatherCta *__restrict__ items, const int *__restrict__ worker_begin,
+              const Slot *__restrict__ slots,
               const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
               int G, int n_det)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2 *tile = reinterpret_cast<float2 *>(smem_raw);
-    float *s_lut = reinterpret_cast<float *>(smem_raw + GATHER_TILE_BYTES);
-    __shared__ __align__(8) uint64_t bar;
+    float *s_lut = reinterpret_cast<float *>(smem_raw + GATHER_STAGES * GATHER_TILE_BYTES);
+    __shared__ __align__(8) uint64_t full[GATHER_STAGES], empty[GATHER_STAGES];
 
-    const GatherCta cta = ctas[blockIdx.x];
+    const int it_begin = worker_begin[blockIdx.x], it_end = worker_begin[blockIdx.x + 1];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < GATHER_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], GATHER_WARPS); }
+    }
     load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
-    if (warp == 0) {
-        if (lane == 0) mbar_expect_tx(&bar, (uint32_t)GATHER_TILE_BYTES);
-        __syncwarp();
-        for (int ly = lane; ly < GT_ROWS; ly += 32) {
-            const float2 *src = grid + (size_t)((cta.ty0 + ly) % G) * G;
-            float2 *dst = tile + ly * GT_PITCH;
-            int gx = cta.tx0, done = 0;                       // tx0 is even, G is even
-            while (done < GT_PITCH) {
-                const int n = min(GT_PITCH - done, G - gx);
-                bulk_g2s(dst + done, src + gx, (uint32_t)(n * sizeof(float2)), &bar);
-                done += n;
-                gx = 0;
+
+    if (warp == GATHER_WARPS) {
+        // ---- producer: stage the tiles of this CTA's items, GATHER_STAGES ahead ----
+        for (int it = it_begin; it < it_end; ++it) {
+            const int q = it - it_begin, st = q % GATHER_STAGES;
+            const GatherCta item = items[it];
+            if (lane == 0) {
+                if (q >= GATHER_STAGES) mbar_wait(&empty[st], (uint32_t)((q / GATHER_STAGES - 1) & 1));
+                mbar_expect_tx(&full[st], (uint32_t)GATHER_TILE_BYTES);
+            }
+            __syncwarp();
+            float2 *tile = reinterpret_cast<float2 *>(smem_raw + st * GATHER_TILE_BYTES);
+            for (int ly = lane; ly < GT_ROWS; ly += 32) {
+                const float2 *src = grid + (size_t)((item.ty0 + ly) % G) * G;
+                float2 *dst = tile + ly * GT_PITCH;
+                int gx = item.tx0, done = 0;                   // tx0 is even, G is even
+                while (done < GT_PITCH) {
+                    const int n = min(GT_PITCH - done, G - gx);
+                    bulk_g2s(dst + done, src + gx, (uint32_t)(n * sizeof(float2)), &full[st]);
+                    done += n;
+                    gx = 0;
+                }
             }
         }
+        return;   // every copy is consumed (waited on) by the consumer warps before the CTA ends
     }
 
+    // ---- consumers ----
     const int cd = n_det / 2;
     const double halfG = 0.5 * (double)G;
-    const Slot *my = slots + (size_t)cta.round_begin * 32 + lane;
-    int r = warp;
-    Slot sl;
-    sl.ak = SLOT_EMPTY; sl.lxy = 0;
-    if (r < cta.round_count) sl = my[(size_t)r * 32];
-    bool staged = false;
-    while (r < cta.round_count) {
-        const int rn = r + GATHER_WARPS;
-        Slot nx;
-        nx.ak = SLOT_EMPTY; nx.lxy = 0;
-        if (rn < cta.round_count) nx = my[(size_t)rn * 32];
-        const bool act = sl.ak != SLOT_EMPTY;
-        const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
-        Taps tp;
-        sample_taps(cs, s_lut, kp, a, k, cd, halfG, tp);
-        if (!staged) { mbar_wait(&bar, 0); staged = true; }
-        if (act) {
-            const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
-            float accr = 0.f, acci = 0.f;
-#pragma unroll
-            for (int ly = 0; ly < KW; ++ly) {
-                float rr = 0.f, ri = 0.f;
-#pragma unroll
-                for (int lx = 0; lx < KW; ++lx) {
-                    const float2 v = base[ly * GT_PITCH + lx];
-                    rr = fmaf(v.x, tp.wx[lx], rr);
-                    ri = fmaf(v.y, tp.wx[lx], ri);
-                }
-                accr = fmaf(rr, tp.wy[ly], accr);
-                acci = fmaf(ri, tp.wy[ly], acci);
-            }
-            // ghost k = n_det (Hermitian-half schedule, even n): F[a, j = -n/2] = conj F[a, j = +n/2]
-            if (k == n_det) polar[(size_t)a * n_det] = make_float2(accr, -acci);
-            else polar[(size_t)a * n_det + k] = make_float2(accr, acci);
+    // position in the concatenated round sequence of this CTA's items
+    struct Pos { int it, r; };
+    auto norm = [&](Pos p) {
+        while (p.it < it_end) {
+            const int rc = __ldg(&items[p.it].round_count);
+            if (p.r < rc) break;
+            p.r -= rc;
+            ++p.it;
         }
-        sl = nx;
-        r = rn;
+        return p;
+    };
+    auto load_slot = [&](const Pos &p) {
+        Slot s;
+        s.ak = SLOT_EMPTY; s.lxy = 0;
+        if (p.it < it_end) s = slots[((size_t)__ldg(&items[p.it].round_begin) + p.r) * 32 + lane];
+        return s;
+    };
+    auto load_dir = [&](const Slot &s) {
+        return s.ak != SLOT_EMPTY ? __ldg(&cs[s.ak >> 16]) : make_double2(0.0, 0.0);
+    };
+    Pos cur = norm(Pos{it_begin, warp});
+    Pos p1 = norm(Pos{cur.it, cur.r + GATHER_WARPS});
+    Pos p2 = norm(Pos{p1.it, p1.r + GATHER_WARPS});
+    Slot sl = load_slot(cur), nx = load_slot(p1);
+    double2 d = load_dir(sl);
+    for (int it = it_begin; it < it_end; ++it) {
+        const int q = it - it_begin, st = q % GATHER_STAGES;
+        const float2 *tile = reinterpret_cast<const float2 *>(smem_raw + st * GATHER_TILE_BYTES);
+        mbar_wait(&full[st], (uint32_t)((q / GATHER_STAGES) & 1));
+        while (cur.it == it) {
+            const Slot nn = load_slot(p2);
+            const double2 dn = load_dir(nx);
+            const bool act = sl.ak != SLOT_EMPTY;
+            const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
+            Taps tp;
+            sample_taps_dir(d, s_lut, kp, k, cd, halfG, tp);
+            if (act) {
+                const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
+                float accr = 0.f, acci = 0.f;
+#pragma unroll
+                for (int ly = 0; ly < KW; ++ly) {
+                    float rr = 0.f, ri = 0.f;
+#pragma unroll
+                    for (int lx = 0; lx < KW; ++lx) {
+                        const float2 v = base[ly * GT_PITCH + lx];
+                        rr = fmaf(v.x, tp.wx[lx], rr);
+                        ri = fmaf(v.y, tp.wx[lx], ri);
+                    }
+                    accr = fmaf(rr, tp.wy[ly], accr);
+                    acci = fmaf(ri, tp.wy[ly], acci);
+                }
+                // ghost k = n_det (Hermitian-half schedule, even n): F[a, j = -n/2] = conj F[a, j = +n/2]
+                if (k == n_det) polar[(size_t)a * n_det] = make_float2(accr, -acci);
+                else polar[(size_t)a * n_det + k] = make_float2(accr, acci);
+            }
+            cur = p1; p1 = p2;
+            p2 = norm(Pos{p2.it, p2.r + GATHER_WARPS});
+            sl = nx; nx = nn; d = dn;
+        }
+        // generic-proxy reads of the tile must be ordered before the async-proxy refill
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();                       // every lane has read its taps of this tile
+        if (lane == 0) mbar_arrive(&empty[st]);
     }
-    // a CTA must not exit while bulk copies into its shared memory are in flight
-    if (!staged) mbar_wait(&bar, 0);
 }
 
 // =====================================================================================
@@ -411,8 +459,8 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     if (q.n_gather_ctas == 0) return 0;
-    gather_kernel<<<q.n_gather_ctas, GATHER_THREADS, GATHER_SMEM, st>>>(
-        grid, polar, q.gather_ctas, q.gather_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
+    gather_kernel<<<q.n_gather_workers, GATHER_THREADS, GATHER_SMEM, st>>>(
+        grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
     count_launch();
     return 0;
 }

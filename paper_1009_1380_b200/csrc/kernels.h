@@ -20,7 +20,8 @@ struct DevicePlan {
     // schedules: [0] every sample / whole grid (arbitrary complex data: the test hooks),
     //            [1] Hermitian half (real image / real sinogram: radon_forward, radon_adjoint)
     struct Sched {
-        GatherCta *gather_ctas = nullptr;   int n_gather_ctas = 0;
+        GatherCta *gather_ctas = nullptr;   int n_gather_ctas = 0;      // work items
+        int *gather_worker_begin = nullptr; int n_gather_workers = 0;   // persistent CTAs
         Slot *gather_slots = nullptr;
         ScatterCta *scatter_ctas = nullptr; int n_scatter_ctas = 0;
         Slot *scatter_slots = nullptr;

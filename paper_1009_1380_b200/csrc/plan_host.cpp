@@ -310,7 +310,7 @@ static inline int half_k_end(const Geometry &g) { return g.n_det + ((g.n_det & 1
 static inline int scatter_k_end(const Geometry &g, bool half) { return half ? half_k_end(g) : g.n_det; }
 static inline bool scatter_k_valid(const Geometry &g, int k) { return k != g.n_det / 2; }
 
-static void build_gather(const Geometry &g, Schedules &out)
+static void build_gather(const Geometry &g, Schedules &out, int n_workers)
 {
     const int G = g.G;
     const bool half = out.half;
@@ -358,6 +358,23 @@ static void build_gather(const Geometry &g, Schedules &out)
     }
     std::stable_sort(out.gather_ctas.begin(), out.gather_ctas.end(),
                      [](const GatherCta &x, const GatherCta &y) { return x.round_count > y.round_count; });
+    // Items -> persistent CTAs: longest processing time first onto the least loaded worker
+    // (deterministic: ties go to the lowest worker index), then grouped by worker.
+    const int P = std::max(1, n_workers);
+    std::vector<long long> load(P, 0);
+    std::vector<std::vector<GatherCta>> mine(P);
+    for (const GatherCta &c : out.gather_ctas) {
+        int w = 0;
+        for (int q = 1; q < P; ++q) if (load[q] < load[w]) w = q;
+        load[w] += c.round_count + GATHER_ITEM_COST;
+        mine[w].push_back(c);
+    }
+    out.gather_ctas.clear();
+    out.gather_worker_begin.assign(1, 0);
+    for (int w = 0; w < P; ++w) {
+        for (const GatherCta &c : mine[w]) out.gather_ctas.push_back(c);
+        out.gather_worker_begin.push_back((int)out.gather_ctas.size());
+    }
 }
 
 // ---------------------------------------------------------------- scatter --------
@@ -521,11 +538,11 @@ static void build_scatter(const Geometry &g, Schedules &out)
     for (auto &p : ctas) out.scatter_ctas.push_back(p.cta);
 }
 
-void build_schedules(const Geometry &g, Schedules &out, bool half)
+void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers)
 {
     out = Schedules();
     out.half = half;
-    build_gather(g, out);
+    build_gather(g, out, n_workers);
     build_scatter(g, out);
 }
 
@@ -566,6 +583,11 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         }
     };
 
+    // gather: the worker partition covers every item once, in order
+    if (s.gather_worker_begin.empty() || s.gather_worker_begin.front() != 0 ||
+        s.gather_worker_begin.back() != (int)s.gather_ctas.size()) ++bad;
+    for (size_t w = 1; w < s.gather_worker_begin.size(); ++w)
+        if (s.gather_worker_begin[w] < s.gather_worker_begin[w - 1]) ++bad;
     // gather: every sample exactly once, at the right place
     std::vector<uint8_t> seen(M, 0);
     for (const GatherCta &c : s.gather_ctas) {

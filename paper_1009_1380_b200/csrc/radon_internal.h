@@ -58,8 +58,9 @@ constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, 
 constexpr int GT_X = 128, GT_Y = 64;
 constexpr int GT_PITCH = GT_X + KH + 1;   // 134 complex per smem row: 16-byte multiple for the bulk copies
 constexpr int GT_ROWS = GT_Y + KH;    // 69
-constexpr int GATHER_WARPS = 8;
-constexpr int GATHER_CTAS_PER_SM = 3;
+constexpr int GATHER_WARPS = 24;      // consumer warps of the persistent gather CTA (+1 producer warp)
+constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : 3;   // tiles in flight per CTA (74 KB each)
+constexpr int GATHER_ITEM_COST = 16;  // load balancing: an item costs its rounds + this (tile staging)
 constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
 
 // Scatter (gridding): a CTA accumulates one SR_X x SR_Y output rectangle in shared memory;
@@ -82,7 +83,7 @@ struct Slot {
 };
 constexpr uint32_t SLOT_EMPTY = 0xFFFFFFFFu;
 
-struct GatherCta {
+struct GatherCta {              // one work item of the gather: a staged tile and some of its rounds
     int tx0, ty0;               // tile origin (cells, centred layout)
     int round_begin, round_count;
 };
@@ -118,7 +119,8 @@ struct Geometry {
 
 struct Schedules {
     std::vector<Slot> gather_slots;         // 32 per round
-    std::vector<GatherCta> gather_ctas;
+    std::vector<GatherCta> gather_ctas;     // work items, grouped by persistent CTA
+    std::vector<int> gather_worker_begin;   // persistent CTA w owns items [begin[w], begin[w+1])
     std::vector<Slot> scatter_slots;
     std::vector<ScatterCta> scatter_ctas;
     std::vector<MergeJob> merge_jobs;
@@ -129,7 +131,8 @@ struct Schedules {
 
 // half == false: every sample, the whole grid (arbitrary complex data: the test hooks).
 // half == true:  Hermitian half for real images / sinograms (radon_forward, radon_adjoint).
-void build_schedules(const Geometry &g, Schedules &out, bool half);
+// n_workers: persistent CTAs of the gather (one per multiprocessor).
+void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers = 148);
 // Returns the number of violated invariants (0 = schedules are valid).
 long long check_schedules(const Geometry &g, const Schedules &s);
 

@@ -141,6 +141,27 @@ def test_full_size_configs_on_sampled_outputs(rb, cfg_id, n_sub):
     assert e_f < G1 and e_a < G1, (cfg_id, e_f, e_a)
 
 
+@pytest.mark.parametrize("cfg_id", [2, 3])
+def test_repeated_calls_are_bitwise_identical(rb, cfg_id):
+    """No atomics and a fixed order of every addition: forward, adjoint and the bare gridding
+    kernels are bitwise reproducible from call to call (also guards the staged kernels'
+    buffer reuse: a missing proxy fence showed up here as run-to-run differences)."""
+    cfg = workloads.get_config(cfg_id)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    rng = np.random.default_rng(40 + cfg_id)
+    x = dev(rng.standard_normal((cfg.N, cfg.N)), torch.float32)
+    y = dev(rng.standard_normal((cfg.n_angles, cfg.n_det)), torch.float32)
+    pol = torch.view_as_complex(dev(rng.standard_normal((cfg.n_angles, cfg.n_det, 2)), torch.float32))
+    grd = torch.view_as_complex(dev(rng.standard_normal((plan.G, plan.G, 2)), torch.float32))
+    ref = [plan.radon_forward(x).clone(), plan.radon_adjoint(y).clone(),
+           plan.radon_grid_only(pol).clone(), plan.radon_interp_only(grd).clone()]
+    for _ in range(12):
+        assert torch.equal(plan.radon_forward(x), ref[0])
+        assert torch.equal(plan.radon_adjoint(y), ref[1])
+        assert torch.equal(plan.radon_grid_only(pol), ref[2])
+        assert torch.equal(plan.radon_interp_only(grd), ref[3])
+
+
 def test_batch_and_host_entry_points_match_single_calls(rb):
     N, na, nd = 128, 50, 181
     plan = rb.RadonPlan(N, na, nd)
