@@ -118,7 +118,11 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
 
+#ifndef RADON_GDBG
+#define RADON_GDBG 0
+#endif
     if (warp == GATHER_WARPS) {
+        if (RADON_GDBG == 2) return;
         // ---- producer: stage the tiles of this CTA's items, GATHER_STAGES ahead ----
         for (int it = it_begin; it < it_end; ++it) {
             const int q = it - it_begin, st = q % GATHER_STAGES;
@@ -175,7 +179,9 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     for (int it = it_begin; it < it_end; ++it) {
         const int q = it - it_begin, st = q % GATHER_STAGES;
         const float2 *tile = reinterpret_cast<const float2 *>(smem_raw + st * GATHER_TILE_BYTES);
+#if RADON_GDBG != 2
         mbar_wait(&full[st], (uint32_t)((q / GATHER_STAGES) & 1));
+#endif
         while (cur.it == it) {
             const Slot nn = load_slot(p2);
             const double2 dn = load_dir(nx);
@@ -183,7 +189,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
             Taps tp;
             sample_taps_dir(d, s_lut, kp, k, cd, halfG, tp);
-            if (act) {
+            if (act && RADON_GDBG != 1) {
                 const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
                 float accr = 0.f, acci = 0.f;
 #pragma unroll
@@ -273,6 +279,54 @@ __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float 
         "f"(wx[0]), "f"(wx[1]), "f"(wx[2]), "f"(wx[3]), "f"(wx[4]), "f"(wx[5]) : "memory");
 }
 
+// A whole unclipped footprint of one sample (fast rounds: every tap lies inside the quadrant, so
+// there are no tap predicates, only `act` for idle lanes).  Row by row: W 64-bit loads, W packed
+// FMAs (fma.rn.f32x2: re and im of a cell in one instruction, same rounding as two scalar FMAs),
+// W stores, warp barrier.  vrow[ly] = (vr, vi) * wy[ly] packed, w2[lx] = (wx[lx], wx[lx]) packed.
+#define RADON_ROW_FAST(OFF, V)                                                                        \
+    "@p ld.shared.b64 c0, [%0+" #OFF "+0];\n @p ld.shared.b64 c1, [%0+" #OFF "+8];\n"                 \
+    "@p ld.shared.b64 c2, [%0+" #OFF "+16];\n @p ld.shared.b64 c3, [%0+" #OFF "+24];\n"               \
+    "@p ld.shared.b64 c4, [%0+" #OFF "+32];\n @p ld.shared.b64 c5, [%0+" #OFF "+40];\n"               \
+    "fma.rn.f32x2 c0, " V ", %8, c0;\n fma.rn.f32x2 c1, " V ", %9, c1;\n"                              \
+    "fma.rn.f32x2 c2, " V ", %10, c2;\n fma.rn.f32x2 c3, " V ", %11, c3;\n"                            \
+    "fma.rn.f32x2 c4, " V ", %12, c4;\n fma.rn.f32x2 c5, " V ", %13, c5;\n"                            \
+    "@p st.shared.b64 [%0+" #OFF "+0], c0;\n @p st.shared.b64 [%0+" #OFF "+8], c1;\n"                 \
+    "@p st.shared.b64 [%0+" #OFF "+16], c2;\n @p st.shared.b64 [%0+" #OFF "+24], c3;\n"               \
+    "@p st.shared.b64 [%0+" #OFF "+32], c4;\n @p st.shared.b64 [%0+" #OFF "+40], c5;\n"               \
+    "bar.warp.sync 0xffffffff;\n"
+
+__device__ __forceinline__ uint64_t pack2(float a, float b)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+
+__device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, float vr, float vi, const Taps &tp)
+{
+    static_assert(KW == 6 && ACC_PITCH * sizeof(float2) == 1040, "row offsets below are written for W = 6, pitch 130");
+    uint64_t v[KW], w[KW];
+#pragma unroll
+    for (int l = 0; l < KW; ++l) {
+        v[l] = pack2(vr * tp.wy[l], vi * tp.wy[l]);
+        w[l] = pack2(tp.wx[l], tp.wx[l]);
+    }
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        ".reg .b64 c0, c1, c2, c3, c4, c5;\n"
+        "setp.ne.b32 p, %1, 0;\n"
+        "mov.b64 c0, 0;\n mov.b64 c1, 0;\n mov.b64 c2, 0;\n mov.b64 c3, 0;\n mov.b64 c4, 0;\n mov.b64 c5, 0;\n"
+        RADON_ROW_FAST(0, "%2")
+        RADON_ROW_FAST(1040, "%3")
+        RADON_ROW_FAST(2080, "%4")
+        RADON_ROW_FAST(3120, "%5")
+        RADON_ROW_FAST(4160, "%6")
+        RADON_ROW_FAST(5200, "%7")
+        "}\n" ::"r"(addr), "r"(act), "l"(v[0]), "l"(v[1]), "l"(v[2]), "l"(v[3]), "l"(v[4]), "l"(v[5]),
+        "l"(w[0]), "l"(w[1]), "l"(w[2]), "l"(w[3]), "l"(w[4]), "l"(w[5]) : "memory");
+}
+
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
@@ -310,9 +364,6 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
             const int k = (int)(s.ak & 0xffff);
             v = __ldg(&polar[(size_t)(s.ak >> 16) * n_det + (k == n_det ? 0 : k)]);
             d = __ldg(&cs[s.ak >> 16]);
-            // Hermitian-half schedule, even n: the unpaired Nyquist sample k = 0 (j = -n/2) and
-            // its ghost k = n (j = +n/2) carry half the value each, the ghost conjugated
-            if (nyq_split && (k == 0 || k == n_det)) v = make_float2(0.5f * v.x, k == 0 ? 0.5f * v.y : -0.5f * v.y);
         }
     };
     Slot s0 = load_slot(0), s1 = load_slot(1), s2 = load_slot(2), s3 = load_slot(3);
@@ -335,10 +386,18 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         double2 d2;
         load_value(s2, v2, d2);
         const bool act = s0.ak != SLOT_EMPTY;
+        const int k0 = (int)(s0.ak & 0xffff);
+        // Hermitian-half schedule, even n: the unpaired Nyquist sample k = 0 (j = -n/2) and its
+        // ghost k = n (j = +n/2) carry half the value each, the ghost conjugated.  Applied here,
+        // at the point of use, so that the prefetched load stays off the critical path.
+        if (nyq_split && (k0 == 0 || k0 == n_det)) v0 = make_float2(0.5f * v0.x, k0 == 0 ? 0.5f * v0.y : -0.5f * v0.y);
         Taps tp;
-        sample_taps_dir(d0, s_lut, kp, (int)(s0.ak & 0xffff), cd, halfG, tp);
+        sample_taps_dir(d0, s_lut, kp, k0, cd, halfG, tp);
         const int bx = (int)(s0.lxy & 0xffff), by = (int)(s0.lxy >> 16);   // biased by KH
         const uint32_t base = origin + (uint32_t)((by * ACC_PITCH + bx) * (int)sizeof(float2));
+        if (RADON_SC_FAST && r < item.fast_count) {   // warp-uniform: footprints wholly inside the quadrant
+            scatter_footprint_fast(base, act ? 1 : 0, v0.x, v0.y, tp);
+        } else {
         // taps inside the quadrant: KH <= bx + lx < KH + sw, likewise rows -> bit masks
         const int xlo = min(max(KH - bx, 0), KW), xhi = min(max(KH + item.sw - bx, 0), KW);
         const int ylo = min(max(KH - by, 0), KW), yhi = min(max(KH + item.sh - by, 0), KW);
@@ -350,6 +409,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
             scatter_row(base + (uint32_t)(ly * ACC_PITCH * (int)sizeof(float2)), m,
                         v0.x * tp.wy[ly], v0.y * tp.wy[ly], tp.wx);
             __syncwarp();   // row steps of different lanes may touch the same cells
+        }
         }
         s0 = s1; s1 = s2; s2 = s3; s3 = s4;
         v0 = v1; v1 = v2; d0 = d1; d1 = d2;

@@ -372,7 +372,14 @@ static void build_gather(const Geometry &g, Schedules &out, int n_workers)
     out.gather_ctas.clear();
     out.gather_worker_begin.assign(1, 0);
     for (int w = 0; w < P; ++w) {
-        for (const GatherCta &c : mine[w]) out.gather_ctas.push_back(c);
+        // a worker's items arrive heaviest first; interleave them heavy, light, heavy, ... so
+        // that the interpolation of a dense tile overlaps the staging of sparse ones (the
+        // copy engine runs GATHER_STAGES items ahead)
+        const std::vector<GatherCta> &m = mine[w];
+        for (size_t lo = 0, hi = m.size(); lo < hi;) {
+            out.gather_ctas.push_back(m[lo++]);
+            if (lo < hi) out.gather_ctas.push_back(m[--hi]);
+        }
         out.gather_worker_begin.push_back((int)out.gather_ctas.size());
     }
 }
@@ -470,7 +477,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
         for (auto &v : quad) v.clear();
         for (int iy = 0; iy < nsy; ++iy)
             for (int ix = 0; ix < nsx; ++ix) {
-                ScatterItem &I = geom[iy * 2 + ix];
+                ScatterItem &I = geom[iy * SQ_X + ix];
                 I.sx0 = ix * ST_X; I.sy0 = iy * ST_Y;
                 I.sw = std::min(ST_X, rw - I.sx0); I.sh = std::min(ST_Y, rh - I.sy0);
                 const int ax0 = rx0 + I.sx0, ay0 = ry0 + I.sy0;          // absolute origin
@@ -481,7 +488,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
                     c.ak = im.ak;
                     c.lx = (int16_t)(im.bx - (ax0 - KH));
                     c.ly = (int16_t)(im.by - (ay0 - KH));
-                    quad[iy * 2 + ix].push_back(c);
+                    quad[iy * SQ_X + ix].push_back(c);
                 }
             }
 
@@ -489,19 +496,42 @@ static void build_scatter(const Geometry &g, Schedules &out)
         size_t biggest = 0;
         for (auto &v : quad) biggest = std::max(biggest, v.size());
         int K = std::max<int>(1, (int)((biggest + (size_t)24 * SCATTER_ROUND_MAX - 1) / ((size_t)24 * SCATTER_ROUND_MAX)));
-        std::vector<Cand> part;
-        std::vector<int> rb, rc;
+        // Rounds of a warp: first the footprints wholly inside its quadrant (no clipping: the
+        // kernel runs them without tap predicates), then the clipped ones.
+        std::vector<Cand> part, part_clip;
+        std::vector<int> rb, rc, rf;
         long long f = 0;
         for (int attempt = 0; attempt < 8; ++attempt) {
             tmp_slots.clear(); f = 0;
             rb.assign((size_t)K * SCATTER_ITEMS, 0); rc.assign((size_t)K * SCATTER_ITEMS, 0);
+            rf.assign((size_t)K * SCATTER_ITEMS, 0);
             int mr = 0;
             for (int kk = 0; kk < K; ++kk)
                 for (int it = 0; it < SCATTER_ITEMS; ++it) {
-                    part.clear();
-                    for (size_t q = kk; q < quad[it].size(); q += K) part.push_back(quad[it][q]);
+                    part.clear(); part_clip.clear();
+                    for (size_t q = kk; q < quad[it].size(); q += K) {
+                        const Cand &c = quad[it][q];
+                        const bool inside = c.lx >= KH && c.lx <= geom[it].sw - 1 && c.ly >= KH && c.ly <= geom[it].sh - 1;
+                        (inside ? part : part_clip).push_back(c);
+                    }
                     rb[kk * SCATTER_ITEMS + it] = (int)(tmp_slots.size() / 32);
-                    rc[kk * SCATTER_ITEMS + it] = build_rounds(part, true, ACC_PITCH, tmp_slots, f);
+                    // one greedy packing over "inside first, clipped after": the leading rounds
+                    // come out all-inside, one round mixes, the rest is clipped
+                    part.insert(part.end(), part_clip.begin(), part_clip.end());
+                    const int nr = build_rounds(part, true, ACC_PITCH, tmp_slots, f);
+                    rc[kk * SCATTER_ITEMS + it] = nr;
+                    int nf = 0;
+                    for (; nf < nr; ++nf) {
+                        const Slot *lanes = &tmp_slots[((size_t)rb[kk * SCATTER_ITEMS + it] + nf) * 32];
+                        bool all_in = true;
+                        for (int l = 0; l < 32 && all_in; ++l) {
+                            if (lanes[l].ak == SLOT_EMPTY) continue;
+                            const int lx = (int)(lanes[l].lxy & 0xffff), ly = (int)(lanes[l].lxy >> 16);
+                            all_in = lx >= KH && lx <= geom[it].sw - 1 && ly >= KH && ly <= geom[it].sh - 1;
+                        }
+                        if (!all_in) break;
+                    }
+                    rf[kk * SCATTER_ITEMS + it] = RADON_SC_FAST ? nf : 0;
                     mr = std::max(mr, rc[kk * SCATTER_ITEMS + it]);
                 }
             if (mr <= SCATTER_ROUND_MAX || attempt == 7) break;
@@ -527,6 +557,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
                 p.cta.items[it] = geom[it];
                 p.cta.items[it].round_begin = base + rb[kk * SCATTER_ITEMS + it];
                 p.cta.items[it].round_count = rc[kk * SCATTER_ITEMS + it];
+                p.cta.items[it].fast_count = rf[kk * SCATTER_ITEMS + it];
                 p.work = std::max<long long>(p.work, rc[kk * SCATTER_ITEMS + it]);
             }
             ctas.push_back(p);
@@ -652,6 +683,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         for (int it = 0; it < SCATTER_ITEMS; ++it) {
             const ScatterItem &I = c.items[it];
             if (I.round_count > SCATTER_ROUND_MAX * 2) ++bad;
+            if (I.fast_count < 0 || I.fast_count > I.round_count) ++bad;
             const int ax0 = c.rx0 + I.sx0, ay0 = c.ry0 + I.sy0;
             for (int r = 0; r < I.round_count; ++r) {
                 const Slot *lanes = &s.scatter_slots[(size_t)(I.round_begin + r) * 32];
@@ -664,6 +696,8 @@ long long check_schedules(const Geometry &g, const Schedules &s)
                     g.base(a, k, x0, y0);
                     const int bx = ax0 - KH + (int)(lanes[l].lxy & 0xffff), by = ay0 - KH + (int)(lanes[l].lxy >> 16);
                     if (posmod(bx - x0, G) != 0 || posmod(by - y0, G) != 0) ++bad;
+                    // fast rounds run without tap predicates: the footprint must lie inside the quadrant
+                    if (r < I.fast_count && (bx < ax0 || bx + KH >= ax0 + I.sw || by < ay0 || by + KH >= ay0 + I.sh)) ++bad;
                     for (int ty = 0; ty < KW; ++ty)
                         for (int tx = 0; tx < KW; ++tx) {
                             const int cx = bx + tx, cy = by + ty;       // the kernel clips to the quadrant

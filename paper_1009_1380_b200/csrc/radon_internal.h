@@ -54,12 +54,20 @@ RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
 constexpr int LUT_S = 256;            // (RADON_KB_LUT) rows per grid unit, linear interpolation
 constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, slope) per tap
 
-// Gather (inverse gridding): one CTA stages a GT_X x GT_Y tile of the grid (+halo).
-constexpr int GT_X = 128, GT_Y = 64;
-constexpr int GT_PITCH = GT_X + KH + 1;   // 134 complex per smem row: 16-byte multiple for the bulk copies
+// Gather (inverse gridding): a work item is a GT_X x GT_Y tile of the grid (+halo), staged by
+// one bulk copy per tile row.  Wide, flat tiles: the copy engine spends ~65 cycles per copy
+// whatever its size (measured: 1 KB copies reach 4.5 TB/s over 148 SMs, >= 2 KB copies the HBM
+// rate), so a row of 4 KB is worth the larger halo (21/16 rows).
+#ifndef RADON_GT_X
+#define RADON_GT_X 512
+#define RADON_GT_Y 16
+#define RADON_GSTAGES 2
+#endif
+constexpr int GT_X = RADON_GT_X, GT_Y = RADON_GT_Y;
+constexpr int GT_PITCH = GT_X + KH + 1;   // complex per smem row: 16-byte multiple for the bulk copies
 constexpr int GT_ROWS = GT_Y + KH;    // 69
 constexpr int GATHER_WARPS = 24;      // consumer warps of the persistent gather CTA (+1 producer warp)
-constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : 3;   // tiles in flight per CTA (74 KB each)
+constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : RADON_GSTAGES;   // tiles in flight per CTA (74 KB each)
 constexpr int GATHER_ITEM_COST = 16;  // load balancing: an item costs its rounds + this (tile staging)
 constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
 
@@ -67,13 +75,24 @@ constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier
 // each of its warps owns one ST_X x ST_Y quadrant of it and processes every sample whose
 // footprint intersects that quadrant, taps clipped to the quadrant (so warps never share a
 // cell, and the accumulator needs no margins).
-constexpr int ST_X = 64, ST_Y = 32;
-constexpr int SR_X = 2 * ST_X, SR_Y = 2 * ST_Y;   // CTA output rectangle: 2 x 2 quadrants
-constexpr int SCATTER_ITEMS = 4;      // warps per CTA
+#ifndef RADON_SC_FAST
+#define RADON_SC_FAST 1               // unclipped footprints first, run without tap predicates
+#endif
+#ifndef RADON_ST_X
+#define RADON_ST_X 64
+#define RADON_ST_Y 32
+#define RADON_SQ_X 2
+#define RADON_SQ_Y 2
+#define RADON_SC_CTAS 3
+#endif
+constexpr int ST_X = RADON_ST_X, ST_Y = RADON_ST_Y;
+constexpr int SQ_X = RADON_SQ_X, SQ_Y = RADON_SQ_Y;   // quadrants per rectangle
+constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
+constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
 constexpr int SB_W = ST_X + KH, SB_H = ST_Y + KH;   // range of biased base coordinates in a quadrant
 constexpr int SCATTER_ROUND_MAX = 48; // rounds per warp before a rectangle's samples are split over CTAs
-constexpr int SCATTER_CTAS_PER_SM = 3;
+constexpr int SCATTER_CTAS_PER_SM = RADON_SC_CTAS;
 
 // One lane's work in one round: which polar sample, and where its W x W footprint
 // starts inside the staged tile (gather) or the warp-private accumulator (scatter).
@@ -91,6 +110,8 @@ struct GatherCta {              // one work item of the gather: a staged tile an
 struct ScatterItem {            // one warp: quadrant (relative to the rectangle) and its rounds
     int sx0, sy0, sw, sh;       // slot coordinates are relative to (sx0 - KH, sy0 - KH)
     int round_begin, round_count;
+    int fast_count;             // the first fast_count rounds hold only footprints wholly inside the quadrant
+    int pad;
 };
 
 struct ScatterCta {
