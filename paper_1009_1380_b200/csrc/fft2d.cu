@@ -71,13 +71,28 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
         if (ix < N) {
             const bool has_b = ix + 1 < N;
             const float da = __ldg(&deapod[ix]), db = has_b ? __ldg(&deapod[ix + 1]) : 0.f;
-            for (int iy = threadIdx.x / NFC; iy < N; iy += C::THREADS / NFC) {
-                const float dy = __ldg(&deapod[iy]);
-                const float *row = x + (size_t)iy * N + ix;
-                float2 v;
-                if (even) v = __ldg(reinterpret_cast<const float2 *>(row));
-                else { v.x = __ldg(row); v.y = has_b ? __ldg(row + 1) : 0.f; }
-                sf[FFT_PAD((iy - c) & (L - 1))] = make_float2(v.x * da * dy, v.y * db * dy);
+            // batches of 8 rows: all loads of a batch are in flight before the first is used
+            constexpr int RS = C::THREADS / NFC;
+            for (int iy0 = threadIdx.x / NFC; iy0 < N; iy0 += 8 * RS) {
+                float2 v[8];
+                float dy[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const int iy = iy0 + q * RS;
+                    v[q] = make_float2(0.f, 0.f);
+                    dy[q] = 0.f;
+                    if (iy < N) {
+                        dy[q] = __ldg(&deapod[iy]);
+                        const float *row = x + (size_t)iy * N + ix;
+                        if (even) v[q] = __ldg(reinterpret_cast<const float2 *>(row));
+                        else { v[q].x = __ldg(row); v[q].y = has_b ? __ldg(row + 1) : 0.f; }
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const int iy = iy0 + q * RS;
+                    if (iy < N) sf[FFT_PAD((iy - c) & (L - 1))] = make_float2(v[q].x * da * dy[q], v[q].y * db * dy[q]);
+                }
             }
         }
     }
@@ -278,15 +293,28 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
     float2 *sf = s_fft + fc * C::STRIDE;
     if (ixc < N) {   // cooperative load: thread -> (ky, pair fc); pack Z = A + i B, Z[-k] = conj A + i conj B
         const bool has_b = ixc + 1 < N;
-        for (int k = threadIdx.x / NFC; k <= L / 2; k += C::THREADS / NFC) {
-            const float2 *src = T + (size_t)k * N + ixc;
-            float2 A, B;
-            if (even) { const float4 q = __ldg(reinterpret_cast<const float4 *>(src)); A = make_float2(q.x, q.y); B = make_float2(q.z, q.w); }
-            else { A = __ldg(src); B = has_b ? __ldg(src + 1) : make_float2(0.f, 0.f); }
-            if (k == 0 || k == L / 2) sf[FFT_PAD(k)] = make_float2(A.x, B.x);        // real by symmetry
-            else {
-                sf[FFT_PAD(k)] = make_float2(A.x - B.y, A.y + B.x);
-                sf[FFT_PAD(L - k)] = make_float2(A.x + B.y, B.x - A.y);
+        constexpr int RS = C::THREADS / NFC;
+        for (int k0 = threadIdx.x / NFC; k0 <= L / 2; k0 += 8 * RS) {
+            float2 A[8], B[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {       // 8 loads in flight
+                const int k = k0 + q * RS;
+                A[q] = B[q] = make_float2(0.f, 0.f);
+                if (k <= L / 2) {
+                    const float2 *src = T + (size_t)k * N + ixc;
+                    if (even) { const float4 w = __ldg(reinterpret_cast<const float4 *>(src)); A[q] = make_float2(w.x, w.y); B[q] = make_float2(w.z, w.w); }
+                    else { A[q] = __ldg(src); if (has_b) B[q] = __ldg(src + 1); }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int k = k0 + q * RS;
+                if (k > L / 2) continue;
+                if (k == 0 || k == L / 2) sf[FFT_PAD(k)] = make_float2(A[q].x, B[q].x);        // real by symmetry
+                else {
+                    sf[FFT_PAD(k)] = make_float2(A[q].x - B[q].y, A[q].y + B[q].x);
+                    sf[FFT_PAD(L - k)] = make_float2(A[q].x + B[q].y, B[q].x - A[q].y);
+                }
             }
         }
     }
