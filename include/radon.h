@@ -154,9 +154,9 @@ int radon_plan_schedule_stats(const radon_plan *p, int half,
  * the gather and scatter schedules for the geometry and verifies that every
  * sample is issued exactly once by the gather, that the scatter issues every
  * (sample, wrap image, output rectangle) incidence exactly once, that no two
- * samples issued to one warp in the same round have overlapping W x W footprints
- * (write-conflict freedom without atomics) and that the 16 lanes of every
- * half-warp start in distinct shared-memory bank pairs.  Returns RADON_OK or
+ * samples issued to one warp in the same round touch the same cell within a row
+ * step (write-conflict freedom without atomics) and that at most two lanes of a
+ * half-warp start in the same shared-memory bank pair.  Returns RADON_OK or
  * RADON_EINVAL; *n_violations (may be NULL) receives the number of violations. */
 int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W, int half,
                              long long *n_violations);

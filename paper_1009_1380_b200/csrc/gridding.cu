@@ -283,17 +283,26 @@ __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float 
 // there are no tap predicates, only `act` for idle lanes).  Row by row: W 64-bit loads, W packed
 // FMAs (fma.rn.f32x2: re and im of a cell in one instruction, same rounding as two scalar FMAs),
 // W stores, warp barrier.  vrow[ly] = (vr, vi) * wy[ly] packed, w2[lx] = (wx[lx], wx[lx]) packed.
-#define RADON_ROW_FAST(OFF, V)                                                                        \
-    "@p ld.shared.b64 c0, [%0+" #OFF "+0];\n @p ld.shared.b64 c1, [%0+" #OFF "+8];\n"                 \
-    "@p ld.shared.b64 c2, [%0+" #OFF "+16];\n @p ld.shared.b64 c3, [%0+" #OFF "+24];\n"               \
-    "@p ld.shared.b64 c4, [%0+" #OFF "+32];\n @p ld.shared.b64 c5, [%0+" #OFF "+40];\n"               \
-    "fma.rn.f32x2 c0, " V ", %8, c0;\n fma.rn.f32x2 c1, " V ", %9, c1;\n"                              \
-    "fma.rn.f32x2 c2, " V ", %10, c2;\n fma.rn.f32x2 c3, " V ", %11, c3;\n"                            \
-    "fma.rn.f32x2 c4, " V ", %12, c4;\n fma.rn.f32x2 c5, " V ", %13, c5;\n"                            \
-    "@p st.shared.b64 [%0+" #OFF "+0], c0;\n @p st.shared.b64 [%0+" #OFF "+8], c1;\n"                 \
-    "@p st.shared.b64 [%0+" #OFF "+16], c2;\n @p st.shared.b64 [%0+" #OFF "+24], c3;\n"               \
-    "@p st.shared.b64 [%0+" #OFF "+32], c4;\n @p st.shared.b64 [%0+" #OFF "+40], c5;\n"               \
-    "bar.warp.sync 0xffffffff;\n"
+#define RADON_ROW_LD(OFF, R)                                                                          \
+    "@p ld.shared.b64 " #R "0, [%0+" #OFF "+0];\n @p ld.shared.b64 " #R "1, [%0+" #OFF "+8];\n"       \
+    "@p ld.shared.b64 " #R "2, [%0+" #OFF "+16];\n @p ld.shared.b64 " #R "3, [%0+" #OFF "+24];\n"     \
+    "@p ld.shared.b64 " #R "4, [%0+" #OFF "+32];\n @p ld.shared.b64 " #R "5, [%0+" #OFF "+40];\n"
+#define RADON_ROW_FMA(V, R)                                                                           \
+    "fma.rn.f32x2 " #R "0, " V ", %8, " #R "0;\n fma.rn.f32x2 " #R "1, " V ", %9, " #R "1;\n"          \
+    "fma.rn.f32x2 " #R "2, " V ", %10, " #R "2;\n fma.rn.f32x2 " #R "3, " V ", %11, " #R "3;\n"        \
+    "fma.rn.f32x2 " #R "4, " V ", %12, " #R "4;\n fma.rn.f32x2 " #R "5, " V ", %13, " #R "5;\n"
+#define RADON_ROW_ST(OFF, R)                                                                          \
+    "@p st.shared.b64 [%0+" #OFF "+0], " #R "0;\n @p st.shared.b64 [%0+" #OFF "+8], " #R "1;\n"       \
+    "@p st.shared.b64 [%0+" #OFF "+16], " #R "2;\n @p st.shared.b64 [%0+" #OFF "+24], " #R "3;\n"     \
+    "@p st.shared.b64 [%0+" #OFF "+32], " #R "4;\n @p st.shared.b64 [%0+" #OFF "+40], " #R "5;\n"
+#define RADON_WARP_BAR "bar.warp.sync 0xffffffff;\n"
+#define RADON_STEP1(O0, V0) RADON_ROW_LD(O0, c) RADON_ROW_FMA(V0, c) RADON_ROW_ST(O0, c) RADON_WARP_BAR
+#define RADON_STEP2(O0, V0, O1, V1)                                                                   \
+    RADON_ROW_LD(O0, c) RADON_ROW_LD(O1, d) RADON_ROW_FMA(V0, c) RADON_ROW_FMA(V1, d)                 \
+    RADON_ROW_ST(O0, c) RADON_ROW_ST(O1, d) RADON_WARP_BAR
+#define RADON_STEP3(O0, V0, O1, V1, O2, V2)                                                           \
+    RADON_ROW_LD(O0, c) RADON_ROW_LD(O1, d) RADON_ROW_LD(O2, e) RADON_ROW_FMA(V0, c) RADON_ROW_FMA(V1, d) \
+    RADON_ROW_FMA(V2, e) RADON_ROW_ST(O0, c) RADON_ROW_ST(O1, d) RADON_ROW_ST(O2, e) RADON_WARP_BAR
 
 __device__ __forceinline__ uint64_t pack2(float a, float b)
 {
@@ -314,15 +323,19 @@ __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, f
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        ".reg .b64 c0, c1, c2, c3, c4, c5;\n"
+        ".reg .b64 c0, c1, c2, c3, c4, c5, d0, d1, d2, d3, d4, d5, e0, e1, e2, e3, e4, e5;\n"
         "setp.ne.b32 p, %1, 0;\n"
         "mov.b64 c0, 0;\n mov.b64 c1, 0;\n mov.b64 c2, 0;\n mov.b64 c3, 0;\n mov.b64 c4, 0;\n mov.b64 c5, 0;\n"
-        RADON_ROW_FAST(0, "%2")
-        RADON_ROW_FAST(1040, "%3")
-        RADON_ROW_FAST(2080, "%4")
-        RADON_ROW_FAST(3120, "%5")
-        RADON_ROW_FAST(4160, "%6")
-        RADON_ROW_FAST(5200, "%7")
+        "mov.b64 d0, 0;\n mov.b64 d1, 0;\n mov.b64 d2, 0;\n mov.b64 d3, 0;\n mov.b64 d4, 0;\n mov.b64 d5, 0;\n"
+        "mov.b64 e0, 0;\n mov.b64 e1, 0;\n mov.b64 e2, 0;\n mov.b64 e3, 0;\n mov.b64 e4, 0;\n mov.b64 e5, 0;\n"
+#if RADON_SC_STEP_ROWS == 1
+        RADON_STEP1(0, "%2") RADON_STEP1(1040, "%3") RADON_STEP1(2080, "%4")
+        RADON_STEP1(3120, "%5") RADON_STEP1(4160, "%6") RADON_STEP1(5200, "%7")
+#elif RADON_SC_STEP_ROWS == 2
+        RADON_STEP2(0, "%2", 1040, "%3") RADON_STEP2(2080, "%4", 3120, "%5") RADON_STEP2(4160, "%6", 5200, "%7")
+#else
+        RADON_STEP3(0, "%2", 1040, "%3", 2080, "%4") RADON_STEP3(3120, "%5", 4160, "%6", 5200, "%7")
+#endif
         "}\n" ::"r"(addr), "r"(act), "l"(v[0]), "l"(v[1]), "l"(v[2]), "l"(v[3]), "l"(v[4]), "l"(v[5]),
         "l"(w[0]), "l"(w[1]), "l"(w[2]), "l"(w[3]), "l"(w[4]), "l"(w[5]) : "memory");
 }

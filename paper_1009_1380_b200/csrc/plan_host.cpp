@@ -8,12 +8,14 @@
 // samples, in which order they accumulate) is taken here once:
 //   * samples are binned into grid tiles by a counting sort;
 //   * inside a tile they are packed into ROUNDS of 32 (one per lane of a warp) such that
-//       - the 16 lanes of each half-warp start in 16 distinct shared-memory bank pairs, so
-//         every 64-bit tap access of the round is conflict free (all lanes add the same
-//         tap offset to their base), and
-//       - (scatter only) no two footprints of a round overlap, so the warp can accumulate
-//         with plain load/add/store into its private accumulator: no atomics, and the order
-//         of every floating-point addition is fixed -> bitwise reproducible;
+//       - the lanes of each half-warp start in distinct shared-memory bank pairs, so every
+//         64-bit tap access of the round is conflict free (all lanes add the same tap offset
+//         to their base); lanes that would otherwise stay idle may share a bank pair with one
+//         other lane (2-way conflict: one extra wavefront instead of another round), and
+//       - (scatter only) no two lanes of a round touch the same cell within a row step (same
+//         base row, base columns closer than W), so the warp can accumulate with plain
+//         load/add/store: no atomics, and the order of every floating-point addition is
+//         fixed -> bitwise reproducible;
 //   * tiles whose sample count (polar sampling is ~1/r dense: PAPER.md:57's imbalance) would
 //     make one block run long are split over several warps / blocks by dealing their samples
 //     round-robin; partial rectangles are summed in a fixed order by a merge kernel.
@@ -251,7 +253,12 @@ struct Occupancy {          // one bitmap row per base row, up to 128 base colum
     {
         const int lo = std::max(lx - KH, 0), hi = std::min(lx + KH, 127);
         unsigned __int128 m = ((((unsigned __int128)1) << (hi - lo + 1)) - 1) << lo;
-        rows[ly][0] |= (uint64_t)m; rows[ly][1] |= (uint64_t)(m >> 64);
+        constexpr int NR = (int)(sizeof(rows) / sizeof(rows[0]));
+        // a step covers SC_STEP_ROWS rows from each lane's own base row: base rows closer than
+        // that share a row within a step
+        for (int y = std::max(ly - (SC_STEP_ROWS - 1), 0); y <= std::min(ly + (SC_STEP_ROWS - 1), NR - 1); ++y) {
+            rows[y][0] |= (uint64_t)m; rows[y][1] |= (uint64_t)(m >> 64);
+        }
     }
 };
 
@@ -287,6 +294,29 @@ static int build_rounds(std::vector<Cand> &cands, bool disjoint, int pitch,
             s.lxy = (uint32_t)c.lx | ((uint32_t)c.ly << 16);
         }
         for (; i < cands.size(); ++i) next.push_back(cands[i]);
+        // Second pass: lanes still idle take candidates whose bank pair is already used ONCE in
+        // their half-warp (a 2-way conflict costs that half-warp one extra wavefront per access;
+        // an idle lane costs the whole round again later).  Footprint disjointness still holds.
+        if (cnt[0] + cnt[1] < 32 && !next.empty()) {
+            uint32_t twice[2] = {0u, 0u};
+            size_t w = 0;
+            for (size_t q = 0; q < next.size(); ++q) {
+                const Cand &c = next[q];
+                const uint32_t res = 1u << ((c.ly * pitch + c.lx) & 15);
+                int h = -1;
+                if (cnt[0] + cnt[1] < 32 && !(disjoint && occ.overlaps(c.lx, c.ly))) {
+                    if (cnt[0] < 16 && !(twice[0] & res)) h = 0;
+                    else if (cnt[1] < 16 && !(twice[1] & res)) h = 1;
+                }
+                if (h < 0) { next[w++] = c; continue; }
+                if (disjoint) occ.mark(c.lx, c.ly);
+                if (mask[h] & res) twice[h] |= res; else mask[h] |= res;
+                Slot &sl = lanes[h * 16 + cnt[h]++];
+                sl.ak = c.ak;
+                sl.lxy = (uint32_t)c.lx | ((uint32_t)c.ly << 16);
+            }
+            next.resize(w);
+        }
         filled += cnt[0] + cnt[1];
         out.insert(out.end(), lanes, lanes + 32);
         cands.swap(next);
@@ -415,6 +445,8 @@ static void build_scatter(const Geometry &g, Schedules &out)
     const int G = g.G;
     const bool half = out.half;
     const int k_end = scatter_k_end(g, half);
+    // measured at config 4: 48 is best for the half schedule (66 vs 79 us), 96 for the full one (108 vs 118 us)
+    const int round_max = half ? SCATTER_ROUND_MAX / 2 : SCATTER_ROUND_MAX;
     const int nrx = (G + SR_X - 1) / SR_X;
     std::vector<RowSeg> segs;
     std::vector<RectGeom> rects;
@@ -495,7 +527,7 @@ static void build_scatter(const Geometry &g, Schedules &out)
         // K CTAs share the rectangle: each quadrant's samples are dealt round-robin over them
         size_t biggest = 0;
         for (auto &v : quad) biggest = std::max(biggest, v.size());
-        int K = std::max<int>(1, (int)((biggest + (size_t)24 * SCATTER_ROUND_MAX - 1) / ((size_t)24 * SCATTER_ROUND_MAX)));
+        int K = std::max<int>(1, (int)((biggest + (size_t)24 * round_max - 1) / ((size_t)24 * round_max)));
         // Rounds of a warp: first the footprints wholly inside its quadrant (no clipping: the
         // kernel runs them without tap predicates), then the clipped ones.
         std::vector<Cand> part, part_clip;
@@ -534,8 +566,8 @@ static void build_scatter(const Geometry &g, Schedules &out)
                     rf[kk * SCATTER_ITEMS + it] = RADON_SC_FAST ? nf : 0;
                     mr = std::max(mr, rc[kk * SCATTER_ITEMS + it]);
                 }
-            if (mr <= SCATTER_ROUND_MAX || attempt == 7) break;
-            K = (int)std::ceil(K * (double)mr / SCATTER_ROUND_MAX * 1.1) + (attempt > 2);
+            if (mr <= round_max || attempt == 7) break;
+            K = (int)std::ceil(K * (double)mr / round_max * 1.1) + (attempt > 2);
         }
         const int base = (int)(out.scatter_slots.size() / 32);
         out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
@@ -596,8 +628,8 @@ long long check_schedules(const Geometry &g, const Schedules &s)
     const long long M = (long long)g.n_angles * nkg;
     auto row_needed = [&](int cy) { return !half || cy == 0 || cy >= G / 2; };
 
-    // Pairwise (brute force, independent of the builder's bitmap): bank pairs distinct per
-    // half-warp; for the scatter, no two lanes of a round with the same base row and base
+    // Pairwise (brute force, independent of the builder's bitmap): at most two lanes of a
+    // half-warp per bank pair; for the scatter, no two lanes of a round with the same base row and base
     // columns closer than W (the kernel's row-step rule), and every footprint inside the
     // accumulator.
     auto check_round = [&](const Slot *lanes, int pitch, bool disjoint) {
@@ -605,11 +637,15 @@ long long check_schedules(const Geometry &g, const Schedules &s)
             if (lanes[i].ak == SLOT_EMPTY) continue;
             const int xi = lanes[i].lxy & 0xffff, yi = lanes[i].lxy >> 16;
             if (disjoint && (xi >= SB_W || yi >= SB_H)) ++bad;
+            int same_bank = 0;      // lanes of this half-warp in the same bank pair: at most 2-way
+            for (int j = 0; j < 32; ++j)
+                if (j != i && lanes[j].ak != SLOT_EMPTY && (i >> 4) == (j >> 4) &&
+                    ((yi * pitch + xi) & 15) == ((int)((lanes[j].lxy >> 16) * pitch + (lanes[j].lxy & 0xffff)) & 15)) ++same_bank;
+            if (same_bank > 1) ++bad;
             for (int j = i + 1; j < 32; ++j) {
                 if (lanes[j].ak == SLOT_EMPTY) continue;
                 const int xj = lanes[j].lxy & 0xffff, yj = lanes[j].lxy >> 16;
-                if ((i >> 4) == (j >> 4) && ((yi * pitch + xi) & 15) == ((yj * pitch + xj) & 15)) ++bad;
-                if (disjoint && yi == yj && std::abs(xi - xj) < KW) ++bad;
+                if (disjoint && std::abs(yi - yj) < SC_STEP_ROWS && std::abs(xi - xj) < KW) ++bad;
             }
         }
     };

@@ -78,6 +78,11 @@ constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier
 #ifndef RADON_SC_FAST
 #define RADON_SC_FAST 1               // unclipped footprints first, run without tap predicates
 #endif
+#ifndef RADON_SC_STEP_ROWS
+#define RADON_SC_STEP_ROWS 1          // footprint rows a lane adds between two warp barriers (fast rounds)
+#endif
+constexpr int SC_STEP_ROWS = RADON_SC_STEP_ROWS;
+static_assert(SC_STEP_ROWS == 1 || SC_STEP_ROWS == 2 || SC_STEP_ROWS == 3, "6 rows in steps of 1, 2 or 3");
 #ifndef RADON_ST_X
 #define RADON_ST_X 64
 #define RADON_ST_Y 32
@@ -91,7 +96,8 @@ constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
 constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
 constexpr int SB_W = ST_X + KH, SB_H = ST_Y + KH;   // range of biased base coordinates in a quadrant
-constexpr int SCATTER_ROUND_MAX = 48; // rounds per warp before a rectangle's samples are split over CTAs
+constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a rectangle's samples are split over CTAs
+                                      // (full schedule; the Hermitian-half one, with half the CTAs, splits at 48)
 constexpr int SCATTER_CTAS_PER_SM = RADON_SC_CTAS;
 
 // One lane's work in one round: which polar sample, and where its W x W footprint

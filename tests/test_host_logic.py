@@ -51,8 +51,8 @@ def test_strerror_and_validation_without_gpu():
                                    (256, 100, 256)])
 def test_schedule_invariants(shape, half):
     """Every sample issued exactly once by the gather; every (sample, wrap image, tap, cell)
-    incidence accumulated exactly once by the scatter; footprints of a round disjoint; bank
-    pairs distinct per half-warp; every grid cell written exactly once.  half: the Hermitian
+    incidence accumulated exactly once by the scatter; footprints of a round disjoint per row
+    step; at most two lanes of a half-warp per bank pair; every grid cell written exactly once.  half: the Hermitian
     half schedules of radon_forward / radon_adjoint (samples j >= 0 plus the Nyquist ghost for
     even n_det; grid rows ky = 0 .. G/2 only, every other row untouched)."""
     rc, bad = rb.schedule_selfcheck(*shape, half=half)
@@ -66,11 +66,12 @@ def test_schedule_stats_config2_shape():
     assert st["scatter_filled"] >= M                       # owner-computes duplicates at tile borders
     assert st["scatter_filled"] < 1.3 * M
     assert st["gather_filled"] / st["gather_slots"] > 0.8  # lane utilisation of the gather rounds
-    assert st["scatter_max_rounds"] <= 64 and st["gather_max_rounds"] <= 64
+    assert st["scatter_max_rounds"] <= 96 and st["gather_max_rounds"] <= 64   # full schedule splits at 96
     # Hermitian half: j >= 0 of every ray plus the ghost (n even) or nothing (n odd: 725)
     sh = rb.schedule_host_stats(512, 360, 725, half=True)
     assert sh["gather_filled"] == 360 * (725 - 725 // 2)
     assert 0.5 * M <= sh["scatter_filled"] < 0.7 * M
+    assert sh["scatter_max_rounds"] <= 48                                      # half schedule splits at 48
     se = rb.schedule_host_stats(512, 90, 512, half=True)
     assert se["gather_filled"] == 90 * (512 // 2 + 1)
 
