@@ -179,3 +179,121 @@ def test_batch_and_host_entry_points_match_single_calls(rb):
     plan.radon_adjoint_host(hs, hb)
     assert torch.equal(hb, back.cpu())
     assert rb.kernel_launch_count() > 0
+
+
+# --------------------------------------------------------------- edge cases -----
+@pytest.mark.parametrize("N,na,nd", [(8, 1, 2), (8, 3, 5), (16, 2, 64), (32, 5, 16), (64, 7, 256), (16, 1, 33)])
+def test_degenerate_and_ragged_geometries(rb, N, na, nd):
+    """Smallest sizes the ABI accepts (N = 8, one angle, two detector bins), detector rows much
+    longer or shorter than the image, tiles and rounds that are mostly ragged tails.  Gate G2
+    (arbitrary input) for the pair, full O-direct."""
+    plan = rb.RadonPlan(N, na, nd)
+    rng = np.random.default_rng(N * 1000 + na * 10 + nd)
+    x = rng.standard_normal((N, N))
+    y = rng.standard_normal((na, nd))
+    S = plan.radon_forward(dev(x, torch.float32)).cpu().numpy()
+    A = plan.radon_adjoint(dev(y, torch.float32)).cpu().numpy()
+    assert rel(S, oracle.forward(x.astype(np.float32), na, nd)) < G2
+    assert rel(A, oracle.adjoint(y.astype(np.float32), N)) < G2
+
+
+def test_zero_input_gives_exact_zeros_and_delta_gives_dirichlet_kernel(rb):
+    N, na, nd = 64, 12, 91
+    plan = rb.RadonPlan(N, na, nd)
+    z = plan.radon_forward(torch.zeros((N, N), device="cuda"))
+    assert torch.count_nonzero(z) == 0
+    assert torch.count_nonzero(plan.radon_adjoint(torch.zeros((na, nd), device="cuda"))) == 0
+    x = np.zeros((N, N), dtype=np.float32)
+    x[N // 2 + 9, N // 2 - 13] = 1.0                      # corner-ish pixel: the hardest input (SURVEY H1)
+    S = plan.radon_forward(dev(x, torch.float32)).cpu().numpy()
+    assert rel(S, oracle.dirichlet_forward(x, na, nd)) < G2    # pin C1's closed form, through the GPU
+
+
+def test_invalid_arguments_are_refused_with_error_codes(rb):
+    import ctypes
+    L = rb.lib()
+    h = ctypes.c_void_p()
+    assert L.radon_plan_create(ctypes.byref(h), 4, 4, 8, ctypes.c_float(2.0), 6) == -1        # N < 8
+    assert L.radon_plan_create(ctypes.byref(h), 64, 0, 8, ctypes.c_float(2.0), 6) == -1       # no angles
+    assert L.radon_plan_create(ctypes.byref(h), 64, 4, 1, ctypes.c_float(2.0), 6) == -1       # n_det < 2
+    assert L.radon_plan_create(ctypes.byref(h), 64, 4, 8, ctypes.c_float(2.0), 4) != 0        # W != 6: unsupported build
+    assert L.radon_plan_create(ctypes.byref(h), 96, 4, 8, ctypes.c_float(2.0), 6) != 0        # sigma*N not a power of two
+    assert not h.value
+    plan = rb.RadonPlan(16, 3, 9)
+    assert L.radon_forward(plan._h, None, None, None) == -1
+    assert L.radon_adjoint(plan._h, None, None, None) == -1
+
+
+def test_largest_grid_on_sampled_outputs(rb):
+    """G = 8192 (the largest FFT length of this build), N = 4096; oracle on a seeded subset."""
+    N, na, nd = 4096, 96, 4096
+    plan = rb.RadonPlan(N, na, nd)
+    x = workloads.make_batch_slice(3, N)
+    rng = np.random.default_rng(8192)
+    idx = rng.choice(na * nd, 96, replace=False)
+    S = plan.radon_forward(dev(x, torch.float32))
+    ref = oracle.dirichlet_forward_subset(x, na, nd, idx)
+    assert rel(S.cpu().numpy().ravel()[idx], ref) < G1
+    y = S.cpu().numpy()
+    pix = rng.choice(N * N, 96, replace=False)
+    A = plan.radon_adjoint(dev(y, torch.float32)).cpu().numpy()
+    assert rel(A.ravel()[pix], oracle.dirichlet_adjoint(y, N, pix=pix)) < G1
+
+
+# --------------------------------------------------------------- configs 3 and 5 as workloads ----
+def test_config3_solver_loop_200_alternating_calls(rb):
+    """BASELINE.json configs[2]: 200 alternating forward / adjoint calls as in a basis-pursuit
+    solver loop (x_{k+1} = x_k - alpha A^T (A x_k - b), b = A x_true).  Parity on
+    the inputs of the first and of the last call, each handed to the oracle as the GPU saw it."""
+    cfg = workloads.get_config(3)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    x_true = dev(workloads.make_image(3), torch.float32)
+    b = plan.radon_forward(x_true).clone()
+    v = torch.ones_like(x_true)
+    for _ in range(10):                                    # power iteration: ||A^T A||
+        w = plan.radon_adjoint(plan.radon_forward(v)).clone()
+        lam = float(w.norm() / v.norm())
+        v = w / w.norm()
+    alpha = 1.0 / lam
+    rng = np.random.default_rng(303)
+    idx = rng.choice(cfg.M, 256, replace=False)
+    pix = rng.choice(cfg.N * cfg.N, 256, replace=False)
+    x = torch.zeros_like(x_true)
+    res0 = None
+    for k in range(100):                                   # 100 iterations = 200 operator calls
+        Ax = plan.radon_forward(x)
+        r = Ax - b
+        if k in (0, 99):
+            xin = x.cpu().numpy(); rin = r.cpu().numpy()
+            if k == 0:
+                assert torch.count_nonzero(Ax) == 0        # x_0 = 0
+            else:
+                assert rel(Ax.cpu().numpy().ravel()[idx],
+                           oracle.dirichlet_forward_subset(xin, cfg.n_angles, cfg.n_det, idx)) < G1
+        g = plan.radon_adjoint(r)
+        if k in (0, 99):
+            assert rel(g.cpu().numpy().ravel()[pix], oracle.dirichlet_adjoint(rin, cfg.N, pix=pix)) < G2
+        if res0 is None:
+            res0 = float(r.norm())
+        x = x - alpha * g
+    assert float((plan.radon_forward(x) - b).norm()) < 0.5 * res0      # the iteration descends
+
+
+def test_config5_batched_volume_matches_single_slice_calls(rb):
+    """BASELINE.json configs[4]: 32 slices of 2048^2 sharing one plan, batched entry points."""
+    cfg = workloads.get_config(4)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    B = 32
+    uniq = [torch.from_numpy(workloads.make_batch_slice(i, cfg.N)) for i in range(4)]
+    hx = torch.stack([uniq[i % 4] * (1.0 + 0.01 * (i // 4)) for i in range(B)]).float()
+    x = hx.cuda()
+    S = plan.radon_forward_batch(x)
+    for i in (0, 13, 31):
+        assert torch.equal(S[i], plan.radon_forward(x[i]))
+    X = plan.radon_adjoint_batch(S)
+    for i in (0, 13, 31):
+        assert torch.equal(X[i], plan.radon_adjoint(S[i]))
+    rng = np.random.default_rng(55)
+    idx = rng.choice(cfg.M, 192, replace=False)
+    ref = oracle.dirichlet_forward_subset(hx[13].numpy(), cfg.n_angles, cfg.n_det, idx)
+    assert rel(S[13].cpu().numpy().ravel()[idx], ref) < G1
