@@ -50,10 +50,10 @@ def stage_bytes(N, G, M, n_angles, W=6):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 4, from the ncu --set full
-# captures summarised in profiles/r01c_hermitian_half_kernels.md (A2 = scatter + merge + dc).
+# captures summarised in profiles/r01d_end_of_round1_kernels.md (A2 = scatter + merge + dc).
 NCU_DRAM_BYTES = {
-    "F1_colfft": 16.87e6, "F2_rowfft": 45.46e6, "F3_gather": 67.98e6, "F4_proj_ifft": 8.59e6,
-    "A1_proj_fft": 8.46e6, "A2_scatter": 48.83e6, "A3_rowifft": 74.34e6, "A4_colifft": 33.68e6,
+    "F1_colfft": 16.99e6, "F2_rowfft": 45.03e6, "F3_gather": 69.34e6, "F4_proj_ifft": 8.59e6,
+    "A1_proj_fft": 8.46e6, "A2_scatter": 47.15e6, "A3_rowifft": 71.55e6, "A4_colifft": 33.73e6,
 }
 
 
