@@ -94,6 +94,16 @@ constexpr size_t GATHER_SMEM = GATHER_STAGES * GATHER_TILE_BYTES + LUT_SMEM;
 static_assert((GT_PITCH * sizeof(float2)) % 16 == 0 && GT_X % 2 == 0, "bulk copies need 16-byte rows");
 static_assert(GATHER_TILE_BYTES % 16 == 0, "stage buffers stay 16-byte aligned");
 
+#ifndef RADON_GATHER_PACKED
+#define RADON_GATHER_PACKED 1
+#endif
+__device__ __forceinline__ uint64_t pack2(float a, float b)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -191,6 +201,26 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             sample_taps_dir(d, s_lut, kp, k, cd, halfG, tp);
             if (act && RADON_GDBG != 1) {
                 const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
+#if RADON_GATHER_PACKED
+                // packed FMAs (fma.rn.f32x2): re and im of a cell in one instruction, same rounding
+                // as two scalar FMAs, half the issue slots of the tap loop
+                uint64_t wx2[KW], acc2 = 0ull;
+#pragma unroll
+                for (int lx = 0; lx < KW; ++lx) wx2[lx] = pack2(tp.wx[lx], tp.wx[lx]);
+#pragma unroll
+                for (int ly = 0; ly < KW; ++ly) {
+                    uint64_t row2 = 0ull;
+#pragma unroll
+                    for (int lx = 0; lx < KW; ++lx) {
+                        const uint64_t v = *reinterpret_cast<const uint64_t *>(&base[ly * GT_PITCH + lx]);
+                        asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(row2) : "l"(v), "l"(wx2[lx]));
+                    }
+                    const uint64_t wy2 = pack2(tp.wy[ly], tp.wy[ly]);
+                    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2) : "l"(row2), "l"(wy2));
+                }
+                float accr, acci;
+                asm("mov.b64 {%0, %1}, %2;" : "=f"(accr), "=f"(acci) : "l"(acc2));
+#else
                 float accr = 0.f, acci = 0.f;
 #pragma unroll
                 for (int ly = 0; ly < KW; ++ly) {
@@ -204,6 +234,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
                     accr = fmaf(rr, tp.wy[ly], accr);
                     acci = fmaf(ri, tp.wy[ly], acci);
                 }
+#endif
                 // ghost k = n_det (Hermitian-half schedule, even n): F[a, j = -n/2] = conj F[a, j = +n/2]
                 if (k == n_det) polar[(size_t)a * n_det] = make_float2(accr, -acci);
                 else polar[(size_t)a * n_det + k] = make_float2(accr, acci);
@@ -303,13 +334,6 @@ __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float 
 #define RADON_STEP3(O0, V0, O1, V1, O2, V2)                                                           \
     RADON_ROW_LD(O0, c) RADON_ROW_LD(O1, d) RADON_ROW_LD(O2, e) RADON_ROW_FMA(V0, c) RADON_ROW_FMA(V1, d) \
     RADON_ROW_FMA(V2, e) RADON_ROW_ST(O0, c) RADON_ROW_ST(O1, d) RADON_ROW_ST(O2, e) RADON_WARP_BAR
-
-__device__ __forceinline__ uint64_t pack2(float a, float b)
-{
-    uint64_t r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
-    return r;
-}
 
 __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, float vr, float vi, const Taps &tp)
 {

@@ -57,19 +57,29 @@ constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, 
 // Gather (inverse gridding): a work item is a GT_X x GT_Y tile of the grid (+halo), staged by
 // one bulk copy per tile row.  Wide, flat tiles: the copy engine spends ~65 cycles per copy
 // whatever its size (measured: 1 KB copies reach 4.5 TB/s over 148 SMs, >= 2 KB copies the HBM
-// rate), so a row of 4 KB is worth the larger halo (21/16 rows).
+// rate), so a row of 3 KB is worth the larger halo (21/16 rows); three tiles in flight per CTA
+// (measured at config 4, bare kernel: 128 x 64 x 3 stages 62 us, 512 x 16 x 2 55 us, 384 x 16 x 3 49 us).
 #ifndef RADON_GT_X
-#define RADON_GT_X 512
+#define RADON_GT_X 384
 #define RADON_GT_Y 16
-#define RADON_GSTAGES 2
+#define RADON_GSTAGES 3
 #endif
 constexpr int GT_X = RADON_GT_X, GT_Y = RADON_GT_Y;
 constexpr int GT_PITCH = GT_X + KH + 1;   // complex per smem row: 16-byte multiple for the bulk copies
 constexpr int GT_ROWS = GT_Y + KH;    // 69
-constexpr int GATHER_WARPS = 24;      // consumer warps of the persistent gather CTA (+1 producer warp)
+#ifndef RADON_GWARPS
+#define RADON_GWARPS 24
+#endif
+constexpr int GATHER_WARPS = RADON_GWARPS;      // consumer warps of the persistent gather CTA (+1 producer warp)
 constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : RADON_GSTAGES;   // tiles in flight per CTA (74 KB each)
-constexpr int GATHER_ITEM_COST = 16;  // load balancing: an item costs its rounds + this (tile staging)
-constexpr int GATHER_ROUND_CAP = 64;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
+#ifndef RADON_GCOST
+#define RADON_GCOST 16
+#endif
+constexpr int GATHER_ITEM_COST = RADON_GCOST;  // load balancing: an item costs its rounds + this (tile staging)
+#ifndef RADON_GCAP
+#define RADON_GCAP 64
+#endif
+constexpr int GATHER_ROUND_CAP = RADON_GCAP;  // rounds (of 32 samples) per CTA; heavier tiles get more CTAs
 
 // Scatter (gridding): a CTA accumulates one SR_X x SR_Y output rectangle in shared memory;
 // each of its warps owns one ST_X x ST_Y quadrant of it and processes every sample whose
