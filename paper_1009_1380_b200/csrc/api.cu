@@ -26,9 +26,12 @@ struct Workspace {
     float2 *T = nullptr;       // (G/2+1) x N Hermitian-half intermediate of the 2-D FFT
     float2 *grid = nullptr;    // G x G oversampled spectrum (centred)
     float2 *polar = nullptr;   // M polar samples
+    float2 *scratch = nullptr; // partial rectangles of the scatter's split tiles (per workspace:
+                               // two slices may be gridded at the same time on different streams)
     float *img = nullptr;      // N x N   (host-buffer entry points only)
     float *sino = nullptr;     // M       (host-buffer entry points only)
 };
+constexpr int NWS = 4;         // workspaces = slices in flight of the host-buffer entry points
 
 // Optional stage timing: one CUDA event at every stage boundary of forward / adjoint.
 struct StageTimer {
@@ -45,12 +48,13 @@ struct radon_plan {
     StageTimer timer;
     Geometry geo;
     DevicePlan dev;
-    Workspace ws[2];
+    Workspace ws[NWS];
     long long M = 0;
+    int n_partial = 0;         // scratch slots a workspace needs (max over the two schedule sets)
     size_t device_bytes = 0;
     long long gather_slots[2] = {0, 0}, gather_filled[2] = {0, 0}, scatter_slots[2] = {0, 0}, scatter_filled[2] = {0, 0};
-    cudaStream_t hstream[2] = {nullptr, nullptr};
-    cudaEvent_t hevent[2] = {nullptr, nullptr};
+    cudaStream_t hstream[NWS] = {};
+    cudaEvent_t hevent[NWS] = {};
 };
 
 template <typename T>
@@ -102,11 +106,11 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
     for (auto &q : d.sched) {
         cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
-        cudaFree(q.merge_jobs); cudaFree(q.scratch);
+        cudaFree(q.merge_jobs);
     }
-    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.img); cudaFree(w.sino); }
+    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < NWS; ++i) {
         if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
     }
@@ -152,6 +156,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if ((rc = dev_upload(p, &d.chirp_b, cb))) return rc;
     if (!hf.empty() && (rc = dev_upload(p, &d.chirp_hf, hf))) return rc;
     // P3: schedules
+    int n_partial = 0;
     for (int h = 0; h < 2; ++h) {
         Schedules sch;
         build_schedules(p->geo, sch, h == 1, d.n_sm);
@@ -168,14 +173,18 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         if ((rc = dev_upload(p, &q.scatter_ctas, sch.scatter_ctas))) return rc;
         if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;
         if ((rc = dev_upload(p, &q.merge_jobs, sch.merge_jobs))) return rc;
-        if ((rc = dev_alloc(p, &q.scratch, (size_t)sch.n_partial_slots * SR_X * SR_Y))) return rc;
+        n_partial = std::max(n_partial, sch.n_partial_slots);
     }
-    // workspace (two sets: the host-buffer entry points overlap copies with kernels)
-    for (auto &w : p->ws) {
+    // workspaces: the first serves the device-pointer calls, all of them the host-buffer entry
+    // points (copies and kernels of NWS slices overlap); allocated on first use beyond the first
+    for (int i = 0; i < 1; ++i) {
+        Workspace &w = p->ws[i];
         if ((rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
         if ((rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
         if ((rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
+        if ((rc = dev_alloc(p, &w.scratch, (size_t)std::max(n_partial, 1) * SR_X * SR_Y))) return rc;
     }
+    p->n_partial = n_partial;
     return RADON_OK;
 }
 
@@ -238,7 +247,7 @@ static int nufft2_ws(radon_plan *p, Workspace &w, bool half, const float *d_x, f
 static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st)
 {
     mark(p, st, 5);
-    if (launch_scatter(p->dev, half, d_polar, w.grid, st)) return RADON_ECUDA;             // A2
+    if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, st)) return RADON_ECUDA;             // A2
     mark(p, st, 6);
     if (launch_fft2d_pass(2, p->dev, w.grid, w.T, half ? 0 : 1, st)) return RADON_ECUDA;   // A3 (rows)
     mark(p, st, 7);
@@ -339,10 +348,16 @@ extern "C" int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_
 // ---- host-buffer entry points: two streams, copies of slice b+1 overlap kernels of slice b
 static int host_setup(radon_plan *p)
 {
-    for (int i = 0; i < 2; ++i) {
+    const int G = p->dev.G, N = p->dev.N;
+    for (int i = 0; i < NWS; ++i) {
         if (!p->hstream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
         if (!p->hevent[i]) CUDA_TRY(cudaEventCreateWithFlags(&p->hevent[i], cudaEventDisableTiming));
         int rc;
+        Workspace &w = p->ws[i];
+        if (!w.T && (rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
+        if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
+        if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
+        if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
         if (!p->ws[i].img && (rc = dev_alloc(p, &p->ws[i].img, (size_t)p->dev.N * p->dev.N))) return rc;
         if (!p->ws[i].sino && (rc = dev_alloc(p, &p->ws[i].sino, (size_t)p->M))) return rc;
     }
@@ -357,7 +372,7 @@ static int host_run(radon_plan *p, bool fwd, const float *h_in, float *h_out, in
     const size_t nx = (size_t)p->dev.N * p->dev.N, ns = (size_t)p->M;
     const size_t n_in = fwd ? nx : ns, n_out = fwd ? ns : nx;
     for (int b = 0; b < batch; ++b) {
-        const int i = b & 1;
+        const int i = b % NWS;
         cudaStream_t st = p->hstream[i];
         Workspace &w = p->ws[i];
         float *d_in = fwd ? w.img : w.sino, *d_out = fwd ? w.sino : w.img;
@@ -366,8 +381,7 @@ static int host_run(radon_plan *p, bool fwd, const float *h_in, float *h_out, in
         if (rc) return rc;
         CUDA_TRY(cudaMemcpyAsync(h_out + b * n_out, d_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st));
     }
-    CUDA_TRY(cudaStreamSynchronize(p->hstream[0]));
-    CUDA_TRY(cudaStreamSynchronize(p->hstream[1]));
+    for (int i = 0; i < NWS; ++i) CUDA_TRY(cudaStreamSynchronize(p->hstream[i]));
     return RADON_OK;
 }
 
@@ -408,7 +422,7 @@ extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_po
 extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
-    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 

@@ -562,14 +562,14 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
     return 0;
 }
 
-int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, cudaStream_t st)
+int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch, cudaStream_t st)
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     scatter_kernel<<<q.n_scatter_ctas, SCATTER_THREADS, SCATTER_SMEM, st>>>(
-        polar, grid, q.scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, (half && (p.n_det & 1) == 0) ? 1 : 0);
+        polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, (half && (p.n_det & 1) == 0) ? 1 : 0);
     count_launch();
     if (q.n_merge_jobs > 0) {
-        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(q.scratch, grid, q.merge_jobs, p.G);
+        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(scratch, grid, q.merge_jobs, p.G);
         count_launch();
     }
     dc_kernel<<<1, DC_THREADS, 0, st>>>(polar, grid, p.lut, p.kb, p.G, p.n_det, p.n_angles, half ? 1 : 0);

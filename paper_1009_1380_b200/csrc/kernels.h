@@ -26,7 +26,6 @@ struct DevicePlan {
         ScatterCta *scatter_ctas = nullptr; int n_scatter_ctas = 0;
         Slot *scatter_slots = nullptr;
         MergeJob *merge_jobs = nullptr;     int n_merge_jobs = 0;
-        float2 *scratch = nullptr;          // partial rectangles of split tiles
     } sched[2];
 };
 
@@ -67,7 +66,8 @@ static inline int set_smem(F kernel, size_t bytes)
 // is written (plus k = 0 for even n, from the ghost sample); scatter: only grid rows
 // [G/2, G) and row 0 are written.
 int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *polar, cudaStream_t st);
-int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, cudaStream_t st);
+// scratch: room for the partial rectangles of the schedule's split tiles (one set per stream in flight)
+int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch, cudaStream_t st);
 // which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid; flag 1: also write every mirrored row,
 // flag 2: only the mirrored rows the half gather reads, |ky| <= W/2 and |ky - G/2| <= W/2),
 // 2 rowpass_inv (grid -> T; flag: fold the mirrored rows in), 3 colpass_inv (T -> x).

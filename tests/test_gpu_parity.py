@@ -297,3 +297,23 @@ def test_config5_batched_volume_matches_single_slice_calls(rb):
     idx = rng.choice(cfg.M, 192, replace=False)
     ref = oracle.dirichlet_forward_subset(hx[13].numpy(), cfg.n_angles, cfg.n_det, idx)
     assert rel(S[13].cpu().numpy().ravel()[idx], ref) < G1
+
+
+def test_host_entry_points_with_slices_in_flight_on_several_streams(rb):
+    """The host-buffer calls keep several slices in flight on their own streams and workspaces;
+    at this size the scatter splits its centre rectangles (partial rectangles + merge), so a
+    scratch buffer shared between streams would show up here as a mismatch."""
+    cfg = workloads.get_config(2)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    assert rb.schedule_host_stats(cfg.N, cfg.n_angles, cfg.n_det, half=True)["merge_jobs"] > 0
+    B = 9
+    rng = np.random.default_rng(77)
+    hy = torch.from_numpy(rng.standard_normal((B, cfg.n_angles, cfg.n_det)).astype(np.float32)).pin_memory()
+    hx = torch.empty((B, cfg.N, cfg.N), dtype=torch.float32).pin_memory()
+    hs = torch.empty_like(hy).pin_memory()
+    for _ in range(3):
+        plan.radon_adjoint_host(hy, hx)
+        plan.radon_forward_host(hx, hs)
+        for i in (0, 4, 8):
+            assert torch.equal(hx[i], plan.radon_adjoint(hy[i].cuda()).cpu())
+            assert torch.equal(hs[i], plan.radon_forward(hx[i].cuda()).cpu())
