@@ -55,6 +55,7 @@ struct radon_plan {
     long long gather_slots[2] = {0, 0}, gather_filled[2] = {0, 0}, scatter_slots[2] = {0, 0}, scatter_filled[2] = {0, 0};
     cudaStream_t hstream[NWS] = {};
     cudaEvent_t hevent[NWS] = {};
+    cudaEvent_t fork_event = nullptr;
 };
 
 template <typename T>
@@ -110,6 +111,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     }
     for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
+    if (p->fork_event) cudaEventDestroy(p->fork_event);
     for (int i = 0; i < NWS; ++i) {
         if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
@@ -323,26 +325,60 @@ extern "C" int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, voi
     return adjoint_ws(p, p->ws[0], d_sino, d_x, (cudaStream_t)stream);
 }
 
-extern "C" int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream)
+// ---- batched device-pointer calls ------------------------------------------------------
+// Slices are independent.  Consecutive slices go to BATCH_LANES internal streams
+// with a workspace each, forked from and joined back into the caller's stream by events, so
+// that the tail of one slice's kernel (most kernels leave part of the 148 SMs idle in their
+// last wave) overlaps the head of the other slice's.  While stage timing is on the slices run
+// one after the other on the caller's stream, so that the stage events mean what they say.
+#ifndef RADON_BATCH_LANES
+#define RADON_BATCH_LANES 4
+#endif
+constexpr int BATCH_LANES = RADON_BATCH_LANES;
+static_assert(BATCH_LANES >= 1 && BATCH_LANES <= NWS, "one workspace per lane");
+
+static int host_setup(radon_plan *p);
+
+static int batch_run(radon_plan *p, bool fwd, const float *d_in, float *d_out, int batch, cudaStream_t user)
 {
-    if (!p || !d_x || !d_sino || batch < 0) return RADON_EINVAL;
-    const size_t nx = (size_t)p->dev.N * p->dev.N;
+    if (!p || !d_in || !d_out || batch < 0) return RADON_EINVAL;
+    const size_t nx = (size_t)p->dev.N * p->dev.N, ns = (size_t)p->M;
+    const size_t n_in = fwd ? nx : ns, n_out = fwd ? ns : nx;
+    const int lanes = (p->timer.enabled || batch < 2) ? 1 : BATCH_LANES;
+    if (lanes == 1) {
+        for (int b = 0; b < batch; ++b) {
+            int rc = fwd ? forward_ws(p, p->ws[0], d_in + b * n_in, d_out + b * n_out, user)
+                         : adjoint_ws(p, p->ws[0], d_in + b * n_in, d_out + b * n_out, user);
+            if (rc) return rc;
+        }
+        return RADON_OK;
+    }
+    int rc = host_setup(p);                                 // streams, events, further workspaces
+    if (rc) return rc;
+    if (!p->fork_event) CUDA_TRY(cudaEventCreateWithFlags(&p->fork_event, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventRecord(p->fork_event, user));
+    for (int l = 0; l < lanes; ++l) CUDA_TRY(cudaStreamWaitEvent(p->hstream[l], p->fork_event, 0));
     for (int b = 0; b < batch; ++b) {
-        int rc = forward_ws(p, p->ws[0], d_x + b * nx, d_sino + (size_t)b * p->M, (cudaStream_t)stream);
+        const int l = b % lanes;
+        rc = fwd ? forward_ws(p, p->ws[l], d_in + b * n_in, d_out + b * n_out, p->hstream[l])
+                 : adjoint_ws(p, p->ws[l], d_in + b * n_in, d_out + b * n_out, p->hstream[l]);
         if (rc) return rc;
+    }
+    for (int l = 0; l < lanes; ++l) {
+        CUDA_TRY(cudaEventRecord(p->hevent[l], p->hstream[l]));
+        CUDA_TRY(cudaStreamWaitEvent(user, p->hevent[l], 0));
     }
     return RADON_OK;
 }
 
+extern "C" int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream)
+{
+    return batch_run(p, true, d_x, d_sino, batch, (cudaStream_t)stream);
+}
+
 extern "C" int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batch, void *stream)
 {
-    if (!p || !d_x || !d_sino || batch < 0) return RADON_EINVAL;
-    const size_t nx = (size_t)p->dev.N * p->dev.N;
-    for (int b = 0; b < batch; ++b) {
-        int rc = adjoint_ws(p, p->ws[0], d_sino + (size_t)b * p->M, d_x + b * nx, (cudaStream_t)stream);
-        if (rc) return rc;
-    }
-    return RADON_OK;
+    return batch_run(p, false, d_sino, d_x, batch, (cudaStream_t)stream);
 }
 
 // ---- host-buffer entry points: two streams, copies of slice b+1 overlap kernels of slice b
