@@ -364,6 +364,20 @@ def main():
                               "note": "working set fits the 126 MB L2; 180 x 1024 samples, sigma=2, W=6"}
         del pp
 
+    # ---- the density-compensated inverse Radon transform at this config ----
+    xi = torch.empty((cfg.N, cfg.N), dtype=torch.float32, device=dev)
+    plan.radon_inverse(sino[0], xi)                       # builds D (host, fp64) on first use
+    for _ in range(3):
+        plan.radon_inverse(sino[0], xi)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(20):
+        plan.radon_inverse(sino[i % B], xi)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    next_rows = {"radon_inverse_us_per_call": round(e0.elapsed_time(e1) / 20 * 1e3, 1),
+                 "note": "A1 with density weights (PAPER.md:89) + A2-A4; one slice at a time"}
+
     if rank != 0:
         return 0
     cpu_baseline = None
@@ -381,7 +395,7 @@ def main():
                    "l2": f"inputs {B * cfg.N * cfg.N * 4 / 1e6:.0f} MB/step cycle through HBM (> 126 MB L2); per-slice grid 134 MB > L2"},
         "samples_per_s": 2.0 * cfg.M * value, "us_per_pair": t_pair_us,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "paper_shape": paper_shape,
+        "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "paper_shape": paper_shape, "next_rows": next_rows,
         "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line))

@@ -136,6 +136,26 @@ int radon_plan_stage_times(radon_plan *p, double total_ms[8], long long launches
 int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_det,
                     long long *M, size_t *workspace_bytes);
 
+/* ---- inverse Radon transform ("Fast Radon and inverse Radon transforms"; Fig. 5
+ * equations :85 and :89) -------------------------------------------------------------------
+ * x = scale * Re{ sum_{a,k} D[a,k] Yhat[a,k] exp(+i (2 pi j/n)(X cos theta_a + Y sin theta_a)) },
+ * Yhat = the centred 1-D DFT of every projection (as in radon_adjoint), computed by gridding
+ * (eq. :85) WITH the density compensation D(x_i,y_i) = 1 / sum_j K(x_i - x_j, y_i - y_j) of
+ * eq. :89 (sum over all polar samples, K the Kaiser-Bessel kernel on the oversampled grid),
+ * followed by the 2-D inverse FFT, crop and de-apodisation.  scale = n_det phihat(0)^2 / G^2
+ * turns D into an area element of the Fourier plane.  D is a plan
+ * constant, derived in fp64 on the host at the first call (a second or two at 2048^2).
+ * d_sino: n_angles*n_det fp32 (device), d_x: N*N fp32 (device, written).  Asynchronous on
+ * `stream` after the first call.  Returns RADON_OK or a negative code as radon_adjoint. */
+int radon_inverse(radon_plan *p, const float *d_sino, float *d_x, void *cuda_stream);
+
+/* D * scale as the plan uses it (M = n_angles*n_det floats, HOST pointer, may be NULL) and
+ * scale (may be NULL).  Builds D if the plan has not done so yet. */
+int radon_plan_density(radon_plan *p, float *h_density, double *scale);
+
+/* The same table without a plan or a GPU (host only; used by the CPU tests). */
+int radon_density_host(int N, int n_angles, int n_det, float sigma, int W, float *h_density, double *scale);
+
 /* A plan holds two schedule sets.  half = 0: every polar sample and the whole grid (arbitrary
  * complex data: radon_nufft2/1, radon_interp_only, radon_grid_only).  half = 1: the Hermitian
  * half used by radon_forward / radon_adjoint, whose image and sinogram are real: the polar

@@ -24,6 +24,10 @@ Functions (each cites the passage it follows; details in radon_oracle.c):
   used to separate algorithmic error from fp32 round-off.  Gated against
   O-direct in the pins before it is trusted.
 
+* ``density`` / ``inverse``  O-density: D(x_i,y_i) = 1/sum_j K(x_i-x_j, y_i-y_j)
+   and the density-compensated inverse Radon transform (PAPER.md:51,
+  :85): weights times the exact adjoint NDFT.
+
 All pinned in tests/test_oracle_pins.py; nothing here is
 "parity unpinned".
 """
@@ -61,6 +65,7 @@ def _load():
         lib.okb_phihat.argtypes = [DBL, I, DBL]; lib.okb_phihat.restype = DBL
         lib.ogrid_interp.argtypes = [D, D, I, I, I, I, DBL, D, D]
         lib.ogrid_grid.argtypes = [D, D, I, I, I, I, DBL, D, D]
+        lib.odensity.argtypes = [I, I, I, I, DBL, I, D]
         _lib = lib
     return _lib
 
@@ -287,3 +292,35 @@ def fast_adjoint(y, N, W=6, sigma=2.0):
     E = _centered_dft_matrix(n_det, -1)        # [k, s]
     Yh = (y @ E.T) / n_det
     return np.real(fast_nufft1(Yh, N, W, sigma))
+
+
+# ---- O-density / inverse Radon ---------------
+
+def density(n_angles, n_det, G, W=6, sigma=2.0, brute=False):
+    """D(x_i,y_i) = 1 / sum_j K(x_i - x_j, y_i - y_j) over all polar samples."""
+    lib = _load()
+    D = np.empty(n_angles * n_det)
+    lib.odensity(n_angles, n_det, G, W, kb_beta(W, sigma), int(bool(brute)), _d(D))
+    return D.reshape(n_angles, n_det)
+
+
+def inverse_scale(n_det, G, W=6, sigma=2.0):
+    """Quadrature weight that turns D into an area element of the image's Fourier plane:
+    sum_j K ~ (samples per grid cell) * (integral of K) = rho * phihat(0)^2, so a sample owns
+    D * phihat(0)^2 grid cells = D * phihat(0)^2 (2 pi / G)^2 (rad/pixel)^2, and the inverse
+    Fourier integral (1/4 pi^2) int xhat e^{i w.X} d^2 w over samples xhat = n * Yhat becomes
+    sum_m Yhat_m e^{...} D_m * n phihat(0)^2 / G^2."""
+    ph0 = float(kb_phihat(0.0, W, kb_beta(W, sigma)))
+    return n_det * ph0 * ph0 / float(G * G)
+
+
+def inverse(y, N, sigma=2.0, W=6, pix=None):
+    """Density-compensated inverse Radon transform ("inverse Radon", eq. :85 with
+    the D of eq. :89): 1-D DFT of every projection, weights D, exact adjoint NDFT, real part."""
+    y = _f64(y)
+    n_angles, n_det = y.shape
+    G = int(round(sigma * N))
+    E = _centered_dft_matrix(n_det, -1)
+    Yh = (y @ E.T) / n_det
+    D = density(n_angles, n_det, G, W, sigma)
+    return np.real(ndft1(Yh * D, N, pix=pix)) * inverse_scale(n_det, G, W, sigma)

@@ -41,6 +41,7 @@
 #include <math.h>
 #include <stddef.h>
 #include <stdlib.h>
+#include <string.h>
 #ifdef _OPENMP
 #include <omp.h>
 #endif
@@ -476,4 +477,64 @@ void ogrid_grid(const double *pr, const double *pi, int G, int n_angles, int n_d
                 gi[cell] += pi[m] * K;
             }
     }
+}
+
+/* ------------------------------------------------------------------------- */
+/* O-density: the density compensation printed with Fig. 5,     */
+/*   D(x_i,y_i) = 1 / sum_j K(x_i - x_j, y_i - y_j),                          */
+/* the sum running over ALL polar samples j (j = i included: K(0,0) = 1), with */
+/* the same separable Kaiser-Bessel kernel K(dx,dy) = phi(dx) phi(dy) on the   */
+/* oversampled grid's coordinates (kappa, polar_kappa above).  */
+/* is a garbled duplicate of the same formula (reading S11).                   */
+/* brute != 0: the double sum exactly as printed, O(M^2).  brute == 0: the    */
+/* same sum with the samples bucketed by integer cell so that only cells within*/
+/* the kernel's support are visited (identical terms, other order).            */
+void odensity(int n_angles, int n_det, int G, int W, double beta, int brute, double *D)
+{
+    const long long M = (long long)n_angles * n_det;
+    double *kx = (double *)malloc(sizeof(double) * (size_t)M), *ky = (double *)malloc(sizeof(double) * (size_t)M);
+    for (long long m = 0; m < M; ++m)
+        polar_kappa((int)(m / n_det), (int)(m % n_det), n_angles, n_det, G, &kx[m], &ky[m]);
+    if (brute) {
+#pragma omp parallel for schedule(dynamic, 64)
+        for (long long i = 0; i < M; ++i) {
+            double s = 0.0;
+            for (long long j = 0; j < M; ++j)
+                s += okb_phi(kx[i] - kx[j], W, beta) * okb_phi(ky[i] - ky[j], W, beta);
+            D[i] = 1.0 / s;
+        }
+    } else {
+        /* buckets: cell (cx,cy) = floor(kappa) + G/2 + 1 in a (G+3)^2 array (kappa in [-G/2, G/2]) */
+        const int B = G + 3, R = W / 2 + 1;
+        long long *start = (long long *)calloc((size_t)B * B + 1, sizeof(long long));
+        long long *order = (long long *)malloc(sizeof(long long) * (size_t)M);
+        int *cell = (int *)malloc(sizeof(int) * (size_t)M);
+        for (long long m = 0; m < M; ++m) {
+            const int cx = (int)floor(kx[m]) + G / 2 + 1, cy = (int)floor(ky[m]) + G / 2 + 1;
+            cell[m] = cy * B + cx;
+            ++start[cell[m] + 1];
+        }
+        for (size_t c = 0; c < (size_t)B * B; ++c) start[c + 1] += start[c];
+        long long *fill = (long long *)malloc(sizeof(long long) * (size_t)B * B);
+        memcpy(fill, start, sizeof(long long) * (size_t)B * B);
+        for (long long m = 0; m < M; ++m) order[fill[cell[m]]++] = m;
+#pragma omp parallel for schedule(dynamic, 64)
+        for (long long i = 0; i < M; ++i) {
+            const int cx = cell[i] % B, cy = cell[i] / B;
+            double s = 0.0;
+            for (int y = cy - R; y <= cy + R; ++y) {
+                if (y < 0 || y >= B) continue;
+                for (int x = cx - R; x <= cx + R; ++x) {
+                    if (x < 0 || x >= B) continue;
+                    for (long long q = start[y * B + x]; q < start[y * B + x + 1]; ++q) {
+                        const long long j = order[q];
+                        s += okb_phi(kx[i] - kx[j], W, beta) * okb_phi(ky[i] - ky[j], W, beta);
+                    }
+                }
+            }
+            D[i] = 1.0 / s;
+        }
+        free(start); free(order); free(cell); free(fill);
+    }
+    free(kx); free(ky);
 }

@@ -33,6 +33,9 @@ _SIGNATURES = {
     "radon_schedule_selfcheck": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_schedule_host_stats": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_kb_weights_host": (c_int, [c_int, c_float, c_float, P(c_float)]),
+    "radon_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_plan_density": (c_int, [c_void_p, c_void_p, P(ctypes.c_double)]),
+    "radon_density_host": (c_int, [c_int, c_int, c_int, c_float, c_int, c_void_p, P(ctypes.c_double)]),
     "radon_kernel_launch_count": (c_ll, []),
     "radon_strerror": (ctypes.c_char_p, [c_int]),
     "radon_last_cuda_error": (ctypes.c_char_p, []),
@@ -73,6 +76,17 @@ def lib():
 def _check(code, where):
     if code != 0:
         raise RadonError(code, where)
+
+
+def density_host(N, n_angles, n_det, sigma=2.0, W=6):
+    """Host-only density table of radon_inverse: (numpy float32 (n_angles, n_det) = D * scale, scale)."""
+    import numpy as np
+
+    out = np.empty((n_angles, n_det), dtype=np.float32)
+    sc = ctypes.c_double()
+    _check(lib().radon_density_host(N, n_angles, n_det, sigma, W, out.ctypes.data_as(c_void_p), ctypes.byref(sc)),
+           "radon_density_host")
+    return out, float(sc.value)
 
 
 def kernel_launch_count() -> int:
@@ -188,6 +202,24 @@ class RadonPlan:
         self._chk(x, torch.float32, self.N * self.N, "x")
         _check(lib().radon_adjoint(self._h, _ptr(sino), _ptr(x), self._stream()), "radon_adjoint")
         return x
+
+    def radon_inverse(self, sino, x=None):
+        import torch
+
+        self._chk(sino, torch.float32, self.M, "sino")
+        x = self._new((self.N, self.N), torch.float32) if x is None else x
+        self._chk(x, torch.float32, self.N * self.N, "x")
+        _check(lib().radon_inverse(self._h, _ptr(sino), _ptr(x), self._stream()), "radon_inverse")
+        return x
+
+    def density(self):
+        """(D * scale as a CPU float32 tensor of shape (n_angles, n_det), scale)."""
+        import torch
+
+        d = torch.empty((self.n_angles, self.n_det), dtype=torch.float32)
+        sc = ctypes.c_double()
+        _check(lib().radon_plan_density(self._h, _ptr(d), ctypes.byref(sc)), "radon_plan_density")
+        return d, float(sc.value)
 
     def radon_forward_batch(self, x, sino=None):
         import torch

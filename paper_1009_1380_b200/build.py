@@ -10,7 +10,7 @@ SOURCES = ["api.cu", "gridding.cu", "fft2d.cu", "proj.cu", "plan_host.cpp"]
 HEADERS = ["kernels.h", "radon_internal.h", "fft_device.cuh", "async_copy.cuh", os.path.join("..", "..", "include", "radon.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",
-    "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+    "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-lpthread",
 ]
 
 

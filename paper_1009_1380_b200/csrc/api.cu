@@ -56,6 +56,8 @@ struct radon_plan {
     cudaStream_t hstream[NWS] = {};
     cudaEvent_t hevent[NWS] = {};
     cudaEvent_t fork_event = nullptr;
+    float *dev_density = nullptr;   // D of PAPER.md:89 times the quadrature scale (built on first radon_inverse)
+    double density_scale = 0.0;
 };
 
 template <typename T>
@@ -112,6 +114,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     if (p->fork_event) cudaEventDestroy(p->fork_event);
+    cudaFree(p->dev_density);
     for (int i = 0; i < NWS; ++i) {
         if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
@@ -262,15 +265,18 @@ static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_si
     int rc = nufft2_ws(p, w, true, d_x, w.polar, st);
     if (rc) return rc;
     mark(p, st, 3);
-    if (launch_proj(true, true, p->dev, (const float *)w.polar, d_sino, st)) return RADON_ECUDA;   // F4
+    if (launch_proj(true, true, p->dev, (const float *)w.polar, d_sino, nullptr, st)) return RADON_ECUDA;   // F4
     mark(p, st, -1);
     return check_launch();
 }
 
-static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st)
+// dens == nullptr: the exact transpose of forward_ws (D == 1, reading S11); else the inverse
+// Radon transform of PAPER.md:51 / :85 with the density compensation D of :89
+static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st,
+                      const float *dens = nullptr)
 {
     mark(p, st, 4);
-    if (launch_proj(false, false, p->dev, d_sino, (float *)w.polar, st)) return RADON_ECUDA;        // A1
+    if (launch_proj(false, false, p->dev, d_sino, (float *)w.polar, dens, st)) return RADON_ECUDA;  // A1
     int rc = check_launch();
     if (rc) return rc;
     rc = nufft1_ws(p, w, true, w.polar, d_x, st);
@@ -323,6 +329,56 @@ extern "C" int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, voi
 {
     if (!p || !d_x || !d_sino) return RADON_EINVAL;
     return adjoint_ws(p, p->ws[0], d_sino, d_x, (cudaStream_t)stream);
+}
+
+// ---- inverse Radon transform ---------------------------------------
+static int density_setup(radon_plan *p)
+{
+    if (p->dev_density) return RADON_OK;
+    std::vector<float> D;
+    try {
+        build_density(p->geo, D, &p->density_scale);
+    } catch (const std::bad_alloc &) {
+        return RADON_ENOMEM;
+    }
+    return dev_upload(p, &p->dev_density, D);
+}
+
+extern "C" int radon_inverse(radon_plan *p, const float *d_sino, float *d_x, void *stream)
+{
+    if (!p || !d_x || !d_sino) return RADON_EINVAL;
+    int rc = density_setup(p);
+    if (rc) return rc;
+    return adjoint_ws(p, p->ws[0], d_sino, d_x, (cudaStream_t)stream, p->dev_density);
+}
+
+extern "C" int radon_plan_density(radon_plan *p, float *h_density, double *scale)
+{
+    if (!p) return RADON_EINVAL;
+    int rc = density_setup(p);
+    if (rc) return rc;
+    if (scale) *scale = p->density_scale;
+    if (h_density)
+        CUDA_TRY(cudaMemcpy(h_density, p->dev_density, (size_t)p->M * sizeof(float), cudaMemcpyDeviceToHost));
+    return RADON_OK;
+}
+
+extern "C" int radon_density_host(int N, int n_angles, int n_det, float sigma, int W, float *h_density, double *scale)
+{
+    if (!h_density) return RADON_EINVAL;
+    int G = 0;
+    int rc = validate(N, n_angles, n_det, sigma, W, &G);
+    if (rc) return rc;
+    try {
+        Geometry geo;
+        geo.init(N, n_angles, n_det, (double)sigma, W);
+        std::vector<float> D;
+        build_density(geo, D, scale);
+        std::memcpy(h_density, D.data(), D.size() * sizeof(float));
+    } catch (...) {
+        return RADON_ENOMEM;
+    }
+    return RADON_OK;
 }
 
 // ---- batched device-pointer calls ------------------------------------------------------
@@ -465,14 +521,14 @@ extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_gri
 extern "C" int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream)
 {
     if (!p || !d_polar || !d_sino) return RADON_EINVAL;
-    if (launch_proj(true, false, p->dev, d_polar, d_sino, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_proj(true, false, p->dev, d_polar, d_sino, nullptr, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
 extern "C" int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *stream)
 {
     if (!p || !d_polar || !d_sino) return RADON_EINVAL;
-    if (launch_proj(false, false, p->dev, d_sino, d_polar, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_proj(false, false, p->dev, d_sino, d_polar, nullptr, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 

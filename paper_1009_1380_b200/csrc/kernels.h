@@ -75,6 +75,7 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
 int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st);
 // inv == false: sinogram -> polar (A1); inv == true: polar -> sinogram (F4).  half (F4 only):
 // the polar rows hold k >= n/2 (and k = 0 for even n); the rest is their conjugate mirror.
-int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st);
+// dens (A1 only, may be null): per-sample density weights multiplied into the output (radon_inverse).
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st);
 
 }  // namespace radon

@@ -29,7 +29,8 @@ template <int L, bool INV, bool BLUE>
 __global__ void __launch_bounds__(ProjCfg<L>::THREADS, BLUE ? 1 : ProjCfg<L>::MIN_CTAS)
 proj_kernel(const float *__restrict__ in, float *__restrict__ out,
             const float2 *__restrict__ ta, const float2 *__restrict__ tb,
-            const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows, int half)
+            const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows, int half,
+            const float *__restrict__ dens)
 {
     extern __shared__ __align__(16) float2 s_fft[];
     using C = ProjCfg<L>;
@@ -71,15 +72,19 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
     for (int i = 0; i < 16; ++i) {
         const int k = t + i * TF;
         if (k < n) {
-            const float2 r = cmul(v[i], __ldg(&tb[k]));
+            float2 r = cmul(v[i], __ldg(&tb[k]));
             if (INV) out[(size_t)row * n + k] = r.x;
-            else reinterpret_cast<float2 *>(out)[(size_t)row * n + k] = r;
+            else {
+                // radon_inverse: density compensation D applied to the sample
+                if (dens != nullptr) { const float w = __ldg(&dens[(size_t)row * n + k]); r.x *= w; r.y *= w; }
+                reinterpret_cast<float2 *>(out)[(size_t)row * n + k] = r;
+            }
         }
     }
 }
 
 template <int L>
-static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
+static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st)
 {
     using C = ProjCfg<L>;
     const int blocks = (p.n_angles + C::NF - 1) / C::NF;
@@ -87,7 +92,7 @@ static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in
     {                                                                                                    \
         if (set_smem(proj_kernel<L, INV_, BLUE_>, C::SMEM)) return -1;                                   \
         proj_kernel<L, INV_, BLUE_><<<blocks, C::THREADS, C::SMEM, st>>>(                                \
-            in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0);       \
+            in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0, dens); \
     }
     const bool blue = p.chirp_hf != nullptr;
     if (inv && blue) RADON_PROJ(true, true)
@@ -99,9 +104,9 @@ static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in
     return 0;
 }
 
-int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, cudaStream_t st)
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st)
 {
-    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, half, p, in, out, st);)
+    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, half, p, in, out, dens, st);)
     return -1;
 }
 

@@ -184,5 +184,8 @@ void build_twiddles(int L, std::vector<float> &tw);                            /
 // L == n when n is a power of two: then hf is empty and a/b are the centring phases).
 void build_chirp(int n, int L, std::vector<float> &a, std::vector<float> &b, std::vector<float> &hf);
 int next_pow2(int v);
+// Density compensation of the inverse Radon transform: D_i = 1 / sum_j K(x_i - x_j, y_i - y_j)
+// over all polar samples, times the quadrature scale n phihat(0)^2 / G^2; fp64, stored fp32.
+void build_density(const Geometry &g, std::vector<float> &D, double *scale_out);
 
 }  // namespace radon

@@ -317,3 +317,32 @@ def test_host_entry_points_with_slices_in_flight_on_several_streams(rb):
         for i in (0, 4, 8):
             assert torch.equal(hx[i], plan.radon_adjoint(hy[i].cuda()).cpu())
             assert torch.equal(hs[i], plan.radon_forward(hx[i].cuda()).cpu())
+
+
+# --------------------------------------------------------------- inverse Radon ----
+def test_inverse_radon_matches_oracle_and_recovers_the_phantom(rb):
+    """radon_inverse (gridding with the density compensation of PAPER.md:89) against the
+    oracle's exact weighted adjoint NDFT: gate G1 on config 1 (full) and config 2 (pixel subset)."""
+    cfg = workloads.get_config(1)
+    x = workloads.make_image(1)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    y = oracle.forward(x, cfg.n_angles, cfg.n_det).astype(np.float32)
+    X = plan.radon_inverse(dev(y, torch.float32)).cpu().numpy()
+    ref = oracle.inverse(y, cfg.N)
+    assert rel(X, ref) < G1
+    D, scale = plan.density()
+    assert abs(scale / oracle.inverse_scale(cfg.n_det, plan.G) - 1) < 1e-12
+    assert np.max(np.abs(D.numpy() / (oracle.density(cfg.n_angles, cfg.n_det, plan.G) * scale) - 1)) < 2e-7
+    # the operator pair is unchanged by building D (radon_adjoint keeps D == 1)
+    assert rel(plan.radon_adjoint(dev(y, torch.float32)).cpu().numpy(), oracle.adjoint(y, cfg.N)) < G1
+    # filtered-back-projection quality on a smooth object
+    g = workloads.gaussian_blob(cfg.N, 5.0, -7.0, 4.0)
+    S = plan.radon_forward(dev(g, torch.float32))
+    assert rel(plan.radon_inverse(S).cpu().numpy(), g) < 0.10
+
+    cfg = workloads.get_config(2)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    y = plan.radon_forward(dev(workloads.make_image(2), torch.float32)).cpu().numpy()
+    pix = np.random.default_rng(12).choice(cfg.N * cfg.N, 512, replace=False)
+    X = plan.radon_inverse(dev(y, torch.float32)).cpu().numpy()
+    assert rel(X.ravel()[pix], oracle.inverse(y, cfg.N, pix=pix)) < G1

@@ -4,6 +4,7 @@ import ctypes
 import os
 import re
 
+import numpy as np
 import pytest
 
 import paper_1009_1380_b200 as rb
@@ -88,3 +89,15 @@ def test_kb_polynomial_weights_match_oracle_kernel():
         ref = oracle.kb_phi(np.float32(delta).astype(np.float64) - 3.0 + np.arange(6))
         worst = max(worst, float(np.abs(w - ref).max()))
     assert worst < 3e-7, worst
+
+
+@pytest.mark.parametrize("shape", [(64, 90, 91), (32, 17, 48), (16, 3, 64)])
+def test_density_table_of_the_library_matches_the_oracle(shape):
+    """radon_inverse's plan constant (host fp64 -> fp32) against O-density."""
+    import oracle
+
+    N, na, nd = shape
+    D, scale = rb.density_host(N, na, nd)
+    assert abs(scale / oracle.inverse_scale(nd, 2 * N) - 1) < 1e-12
+    ref = oracle.density(na, nd, 2 * N) * scale
+    assert np.max(np.abs(D / ref - 1)) < 2e-7

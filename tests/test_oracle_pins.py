@@ -331,3 +331,42 @@ def test_golden_regression_fixture():
     got = make_golden.compute()
     assert ref.shape == got.shape
     assert np.abs(ref - got).max() < 1e-12 * np.abs(ref).max()
+
+
+# ---- O-density / inverse Radon -----------------
+def test_density_bucketed_sum_equals_the_double_sum_as_printed():
+    """PAPER.md:89 written out as the O(M^2) double sum against the bucketed evaluation."""
+    for (na, nd, G) in [(12, 21, 32), (9, 16, 16), (5, 33, 64)]:
+        Db = oracle.density(na, nd, G, brute=True)
+        Df = oracle.density(na, nd, G)
+        assert np.max(np.abs(Db / Df - 1)) < 1e-13
+
+
+def test_density_special_values_and_ramp():
+    """All n_angles samples with j = 0 coincide at kappa = 0 and see the same neighbourhood, so
+    they share one D <= 1/n_angles (K(0,0) = 1 for each of them); an isolated sample has D = 1;
+    between DC and the band edge D follows the polar area element, D ~ |j| (the ramp filter)."""
+    na, nd, G = 90, 91, 128
+    D = oracle.density(na, nd, G)
+    c = nd // 2
+    assert np.ptp(D[:, c]) < 1e-12 * D[0, c] and D[0, c] < 1.0 / na
+    assert abs(oracle.density(1, 2, 64)[0, 1] - 1.0) < 1e-12          # two samples 32 cells apart
+    j = np.arange(8, 33)
+    ratio = D[10, c + j] / j
+    assert np.max(np.abs(ratio / ratio.mean() - 1)) < 0.01
+    assert np.allclose(D[:, c + j], D[:, c - j], rtol=1e-9)            # point symmetry of the sample set
+
+
+def test_inverse_recovers_a_gaussian_blob():
+    """inverse(forward(x)) ~ x for a band-limited blob (filtered-back-projection quality: the
+    kernel-smoothed density of eq. :89 is not the exact ramp near DC)."""
+    N, na, nd = 64, 90, 91
+    x = workloads.gaussian_blob(N, 5.0, -7.0, 4.0)
+    xr = oracle.inverse(oracle.forward(x, na, nd), N)
+    assert rel(xr, x) < 0.10
+    assert abs(xr.max() / x.max() - 1) < 0.03
+    iy, ix = np.unravel_index(np.argmax(xr), xr.shape)
+    assert (iy, ix) == (N // 2 - 7, N // 2 + 5)
+    # a pixel subset is exact (independent sums)
+    pix = np.array([5, 77, N * N - 1, (N // 2 - 7) * N + N // 2 + 5])
+    assert np.allclose(oracle.inverse(oracle.forward(x, na, nd), N, pix=pix), xr.ravel()[pix], rtol=1e-12, atol=1e-14)
