@@ -3,8 +3,8 @@
 //   gather_kernel    F3  inverse gridding, PAPER.md:87 (regular grid -> polar samples)
 //   scatter_kernel   A2  gridding, PAPER.md:85 with D == 1 (polar samples -> regular grid)
 //   merge_kernel         fixed-order sum of the partial rectangles of split tiles
-//   colpass/rowpass  F1+F2 / A3+A4  de-apodise + zero-pad + 2-D FFT, and the transposed chain
-//   proj kernels     F4 / A1  centred 1-D DFTs along the projections (Bluestein for any n_det)
+//   dc_kernel            the j = 0 samples of all angles, summed and gridded once (DESIGN.md R-tie)
+// (the FFT passes live in fft2d.cu, the projection DFTs in proj.cu)
 #include "kernels.h"
 #include "async_copy.cuh"
 
@@ -128,11 +128,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
 
-#ifndef RADON_GDBG
-#define RADON_GDBG 0
-#endif
     if (warp == GATHER_WARPS) {
-        if (RADON_GDBG == 2) return;
         // ---- producer: stage the tiles of this CTA's items, GATHER_STAGES ahead ----
         for (int it = it_begin; it < it_end; ++it) {
             const int q = it - it_begin, st = q % GATHER_STAGES;
@@ -189,9 +185,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     for (int it = it_begin; it < it_end; ++it) {
         const int q = it - it_begin, st = q % GATHER_STAGES;
         const float2 *tile = reinterpret_cast<const float2 *>(smem_raw + st * GATHER_TILE_BYTES);
-#if RADON_GDBG != 2
         mbar_wait(&full[st], (uint32_t)((q / GATHER_STAGES) & 1));
-#endif
         while (cur.it == it) {
             const Slot nn = load_slot(p2);
             const double2 dn = load_dir(nx);
@@ -199,7 +193,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
             Taps tp;
             sample_taps_dir(d, s_lut, kp, k, cd, halfG, tp);
-            if (act && RADON_GDBG != 1) {
+            if (act) {
                 const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
 #if RADON_GATHER_PACKED
                 // packed FMAs (fma.rn.f32x2): re and im of a cell in one instruction, same rounding
