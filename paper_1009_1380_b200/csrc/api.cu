@@ -26,6 +26,7 @@ struct Workspace {
     float2 *T = nullptr;       // (G/2+1) x N Hermitian-half intermediate of the 2-D FFT
     float2 *grid = nullptr;    // G x G oversampled spectrum (centred)
     float2 *polar = nullptr;   // M polar samples
+    float2 *dcbuf = nullptr;   // (W+1)^2 values: the summed j = 0 samples on the centre window
     float2 *scratch = nullptr; // partial rectangles of the scatter's split tiles (per workspace:
                                // two slices may be gridded at the same time on different streams)
     float *img = nullptr;      // N x N   (host-buffer entry points only)
@@ -111,7 +112,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
         cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
         cudaFree(q.merge_jobs);
     }
-    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.img); cudaFree(w.sino); }
+    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.dcbuf); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     if (p->fork_event) cudaEventDestroy(p->fork_event);
     cudaFree(p->dev_density);
@@ -171,6 +172,18 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         q.n_gather_ctas = (int)sch.gather_ctas.size();
         q.n_scatter_ctas = (int)sch.scatter_ctas.size();
         q.n_merge_jobs = (int)sch.merge_jobs.size();
+        {   // is every cell of the centre window (rows ky >= 0 only on the half grid) inside a split rectangle?
+            bool all = !sch.merge_jobs.empty();
+            for (int uy = (h == 1 ? 0 : -KW / 2); uy <= KW / 2 && all; ++uy)
+                for (int ux = -KW / 2; ux <= KW / 2 && all; ++ux) {
+                    const int cx = G / 2 + ux, cy = G / 2 + uy;
+                    bool in = false;
+                    for (const MergeJob &mj : sch.merge_jobs)
+                        in = in || (cx >= mj.rx0 && cx < mj.rx0 + mj.rw && cy >= mj.ry0 && cy < mj.ry0 + mj.rh);
+                    all = in;
+                }
+            q.dc_fused = all;
+        }
         if ((rc = dev_upload(p, &q.gather_ctas, sch.gather_ctas))) return rc;
         q.n_gather_workers = (int)sch.gather_worker_begin.size() - 1;
         if ((rc = dev_upload(p, &q.gather_worker_begin, sch.gather_worker_begin))) return rc;
@@ -188,6 +201,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         if ((rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
         if ((rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
         if ((rc = dev_alloc(p, &w.scratch, (size_t)std::max(n_partial, 1) * SR_X * SR_Y))) return rc;
+        if ((rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
     }
     p->n_partial = n_partial;
     return RADON_OK;
@@ -252,7 +266,7 @@ static int nufft2_ws(radon_plan *p, Workspace &w, bool half, const float *d_x, f
 static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st)
 {
     mark(p, st, 5);
-    if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, st)) return RADON_ECUDA;             // A2
+    if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, w.dcbuf, st)) return RADON_ECUDA;             // A2
     mark(p, st, 6);
     if (launch_fft2d_pass(2, p->dev, w.grid, w.T, half ? 0 : 1, st)) return RADON_ECUDA;   // A3 (rows)
     mark(p, st, 7);
@@ -450,6 +464,7 @@ static int host_setup(radon_plan *p)
         if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
         if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
         if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
+        if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
         if (!p->ws[i].img && (rc = dev_alloc(p, &p->ws[i].img, (size_t)p->dev.N * p->dev.N))) return rc;
         if (!p->ws[i].sino && (rc = dev_alloc(p, &p->ws[i].sino, (size_t)p->M))) return rc;
     }
@@ -514,7 +529,7 @@ extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_po
 extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
-    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, p->ws[0].dcbuf, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 

@@ -358,14 +358,96 @@ __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, f
         "l"(w[0]), "l"(w[1]), "l"(w[2]), "l"(w[3]), "l"(w[4]), "l"(w[5]) : "memory");
 }
 
+constexpr int DC_CELLS = (KW + 1) * (KW + 1);
+// NT threads of one CTA: sum the j = 0 samples (fixed order), then thread t < DC_CELLS holds the
+// value to add to window cell t (offset ux = t % (W+1) - W/2, uy = t / (W+1) - W/2 from DC);
+// returns false where nothing is to be added.  part: NT float2 of shared memory.
+template <int NT>
+__device__ __forceinline__ bool dc_compute(const float2 *__restrict__ polar, const float *__restrict__ g_lut,
+                                           const KbPoly &kp, int n_det, int n_angles, int half,
+                                           float2 *part, float2 &add, int &ux, int &uy)
+{
+    static_assert(DC_CELLS <= NT, "one thread per cell of the (W+1)^2 window");
+    const int t = threadIdx.x, cd = n_det / 2;
+    float sr = 0.f, si = 0.f;
+    for (int a0 = 0; a0 < n_angles; a0 += 8 * NT) {              // 8 independent loads in flight
+        float2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int a = a0 + q * NT + t;
+            v[q] = a < n_angles ? __ldg(&polar[(size_t)a * n_det + cd]) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { sr += v[q].x; si += v[q].y; }
+    }
+    part[t] = make_float2(sr, si);
+    __syncthreads();
+    for (int h = NT / 2; h > 0; h >>= 1) {
+        if (t < h) { part[t].x += part[t + h].x; part[t].y += part[t + h].y; }
+        __syncthreads();
+    }
+    const float2 V = part[0];
+    float wa[KW], wb[KW];
+#if RADON_KB_LUT
+    lut_weights(g_lut, 0.f, wa);
+    lut_weights(g_lut, 1.f, wb);
+#else
+    kb_poly_weights(kp, 0.f, wa);
+    kb_poly_weights(kp, 1.f, wb);
+#endif
+    add = make_float2(0.f, 0.f);
+    ux = t % (KW + 1) - KW / 2; uy = t / (KW + 1) - KW / 2;     // cell offset from DC: -W/2 .. W/2
+    if (t >= DC_CELLS) return false;
+    auto tap = [](const float (&w)[KW], int l) {
+        float r = 0.f;
+#pragma unroll
+        for (int q = 0; q < KW; ++q) r = (q == l) ? w[q] : r;
+        return r;
+    };
+    const float a2 = tap(wa, ux + KW / 2) * tap(wa, uy + KW / 2);           // taps -W/2 .. W/2-1
+    const float b2 = tap(wb, ux + KW / 2 - 1) * tap(wb, uy + KW / 2 - 1);   // taps -W/2+1 .. W/2
+    if (half) {
+        if (uy < 0) return false;
+        add = make_float2(0.5f * V.x * (a2 + b2), 0.5f * V.y * (a2 - b2));
+    } else {
+        add = make_float2(V.x * a2, V.y * a2);
+    }
+    return !(a2 == 0.f && (b2 == 0.f || !half));
+}
+
+// Stand-alone form (plans whose centre rectangles are not split: nobody else could add the
+// window after the scatter): one thread per cell adds its value to the grid, no atomics.
+constexpr int DC_THREADS = 256;
+__global__ void __launch_bounds__(DC_THREADS)
+dc_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, const float *__restrict__ g_lut,
+          const KbPoly kp, int G, int n_det, int n_angles, int half)
+{
+    __shared__ float2 part[DC_THREADS];
+    float2 add;
+    int ux, uy;
+    if (!dc_compute<DC_THREADS>(polar, g_lut, kp, n_det, n_angles, half, part, add, ux, uy)) return;
+    float2 *cell = grid + (size_t)((G / 2 + uy) & (G - 1)) * G + ((G / 2 + ux) & (G - 1));
+    const float2 c = *cell;
+    *cell = make_float2(c.x + add.x, c.y + add.y);
+}
+
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
                const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
-               int G, int n_det, int nyq_split)
+               int G, int n_det, int nyq_split, float2 *__restrict__ dcbuf, int n_angles, int half)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *acc = reinterpret_cast<float2 *>(smem_raw);
+    if (dcbuf != nullptr && blockIdx.x == gridDim.x - 1) {
+        // one extra CTA: the j = 0 samples, summed while the others grid; merge_kernel adds
+        // dcbuf to the centre window when it writes those cells (DESIGN.md R-tie)
+        float2 add;
+        int ux, uy;
+        dc_compute<SCATTER_THREADS>(polar, g_lut, kp, n_det, n_angles, half, acc, add, ux, uy);
+        if (threadIdx.x < DC_CELLS) dcbuf[threadIdx.x] = add;
+        return;
+    }
     float *s_lut = reinterpret_cast<float *>(smem_raw + SCATTER_ACC_BYTES);
     __shared__ ScatterCta cta;
 
@@ -464,7 +546,7 @@ constexpr int MERGE_THREADS = 256;
 constexpr int MERGE_CHUNKS = (SR_X * SR_Y + MERGE_THREADS - 1) / MERGE_THREADS;
 __global__ void __launch_bounds__(MERGE_THREADS)
 merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
-             const MergeJob *__restrict__ jobs, int G)
+             const MergeJob *__restrict__ jobs, int G, const float2 *__restrict__ dcbuf)
 {
     const MergeJob j = jobs[blockIdx.x / MERGE_CHUNKS];
     const int i = (blockIdx.x % MERGE_CHUNKS) * MERGE_THREADS + threadIdx.x;
@@ -478,6 +560,14 @@ merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
         sr += c.x;
         si += c.y;
     }
+    if (dcbuf != nullptr) {            // centre window: the summed j = 0 samples (dc_compute)
+        const int ux = j.rx0 + x - G / 2, uy = j.ry0 + y - G / 2;
+        if (ux >= -KW / 2 && ux <= KW / 2 && uy >= -KW / 2 && uy <= KW / 2) {
+            const float2 d = dcbuf[(uy + KW / 2) * (KW + 1) + ux + KW / 2];
+            sr += d.x;
+            si += d.y;
+        }
+    }
     grid[(size_t)(j.ry0 + y) * G + j.rx0 + x] = make_float2(sr, si);
 }
 
@@ -489,63 +579,6 @@ merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
 // part of that footprint, (V wA(kx) wA(ky) + conj(V) wB(kx) wB(ky)) / 2, wB(u) = wA(-u) the
 // mirrored taps (-W/2, W/2] (delta = 1) -- what the full gridding followed by Re{.} computes
 // (reading R-tie).
-constexpr int DC_THREADS = 256;
-static_assert((KW + 1) * (KW + 1) <= DC_THREADS, "one thread per cell of the (W+1)^2 window");
-__global__ void __launch_bounds__(DC_THREADS)
-dc_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, const float *__restrict__ g_lut,
-          const KbPoly kp, int G, int n_det, int n_angles, int half)
-{
-    __shared__ float2 part[DC_THREADS];
-    const int t = threadIdx.x, cd = n_det / 2;
-    float sr = 0.f, si = 0.f;
-    for (int a0 = 0; a0 < n_angles; a0 += 8 * DC_THREADS) {      // 8 independent loads in flight
-        float2 v[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            const int a = a0 + q * DC_THREADS + t;
-            v[q] = a < n_angles ? __ldg(&polar[(size_t)a * n_det + cd]) : make_float2(0.f, 0.f);
-        }
-#pragma unroll
-        for (int q = 0; q < 8; ++q) { sr += v[q].x; si += v[q].y; }
-    }
-    part[t] = make_float2(sr, si);
-    __syncthreads();
-    for (int h = DC_THREADS / 2; h > 0; h >>= 1) {
-        if (t < h) { part[t].x += part[t + h].x; part[t].y += part[t + h].y; }
-        __syncthreads();
-    }
-    const float2 V = part[0];
-    float wa[KW], wb[KW];
-#if RADON_KB_LUT
-    lut_weights(g_lut, 0.f, wa);
-    lut_weights(g_lut, 1.f, wb);
-#else
-    kb_poly_weights(kp, 0.f, wa);
-    kb_poly_weights(kp, 1.f, wb);
-#endif
-    if (t >= (KW + 1) * (KW + 1)) return;
-    const int ux = t % (KW + 1) - KW / 2, uy = t / (KW + 1) - KW / 2;     // cell offset from DC: -W/2 .. W/2
-    auto tap = [](const float (&w)[KW], int l) {
-        float r = 0.f;
-#pragma unroll
-        for (int q = 0; q < KW; ++q) r = (q == l) ? w[q] : r;
-        return r;
-    };
-    const float a2 = tap(wa, ux + KW / 2) * tap(wa, uy + KW / 2);           // taps -W/2 .. W/2-1
-    const float b2 = tap(wb, ux + KW / 2 - 1) * tap(wb, uy + KW / 2 - 1);   // taps -W/2+1 .. W/2
-    float2 add;
-    if (half) {
-        if (uy < 0) return;
-        add = make_float2(0.5f * V.x * (a2 + b2), 0.5f * V.y * (a2 - b2));
-    } else {
-        add = make_float2(V.x * a2, V.y * a2);
-    }
-    if (a2 == 0.f && (b2 == 0.f || !half)) return;
-    float2 *cell = grid + (size_t)((G / 2 + uy) & (G - 1)) * G + ((G / 2 + ux) & (G - 1));
-    const float2 c = *cell;
-    *cell = make_float2(c.x + add.x, c.y + add.y);
-}
-
 int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *polar, cudaStream_t st)
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
@@ -556,18 +589,26 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
     return 0;
 }
 
-int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch, cudaStream_t st)
+int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch,
+                   float2 *dcbuf, cudaStream_t st)
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
-    scatter_kernel<<<q.n_scatter_ctas, SCATTER_THREADS, SCATTER_SMEM, st>>>(
-        polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, (half && (p.n_det & 1) == 0) ? 1 : 0);
+    const int nyq = (half && (p.n_det & 1) == 0) ? 1 : 0;
+    // dc_fused: every cell of the centre window lies in a split rectangle, so merge_kernel can
+    // add the summed j = 0 samples; they are summed by one extra CTA of the scatter launch
+    float2 *dcb = q.dc_fused ? dcbuf : nullptr;
+    scatter_kernel<<<q.n_scatter_ctas + (dcb ? 1 : 0), SCATTER_THREADS, SCATTER_SMEM, st>>>(
+        polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, nyq,
+        dcb, p.n_angles, half ? 1 : 0);
     count_launch();
     if (q.n_merge_jobs > 0) {
-        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(scratch, grid, q.merge_jobs, p.G);
+        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(scratch, grid, q.merge_jobs, p.G, dcb);
         count_launch();
     }
-    dc_kernel<<<1, DC_THREADS, 0, st>>>(polar, grid, p.lut, p.kb, p.G, p.n_det, p.n_angles, half ? 1 : 0);
-    count_launch();
+    if (!dcb) {
+        dc_kernel<<<1, DC_THREADS, 0, st>>>(polar, grid, p.lut, p.kb, p.G, p.n_det, p.n_angles, half ? 1 : 0);
+        count_launch();
+    }
     return 0;
 }
 
