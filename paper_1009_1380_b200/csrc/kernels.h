@@ -1,5 +1,8 @@
 // kernels.h -- device-side view of a plan and the kernel launchers (internal).
 #pragma once
+#include <mutex>
+#include <set>
+#include <utility>
 #include <cuda_runtime.h>
 
 #include "radon_internal.h"
@@ -35,14 +38,22 @@ int init_kernel_attributes();
 long long launch_count();
 void count_launch();
 
-// Opt a kernel in to more than 48 KB of dynamic shared memory.
+// Opt a kernel in to more than 48 KB of dynamic shared memory: once per (device, kernel); the
+// attribute call costs microseconds of host time, which a batch of back-to-back launches feels.
 template <typename F>
 static inline int set_smem(F kernel, size_t bytes)
 {
-    if (bytes > 48 * 1024) {
-        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
-            return -1;
-    }
+    if (bytes <= 48 * 1024) return 0;
+    static std::mutex mu;
+    static std::set<std::pair<int, const void *>> done;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    const std::pair<int, const void *> key(dev, reinterpret_cast<const void *>(kernel));
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count(key)) return 0;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+        return -1;
+    done.insert(key);
     return 0;
 }
 

@@ -101,3 +101,38 @@ def test_density_table_of_the_library_matches_the_oracle(shape):
     assert abs(scale / oracle.inverse_scale(nd, 2 * N) - 1) < 1e-12
     ref = oracle.density(na, nd, 2 * N) * scale
     assert np.max(np.abs(D / ref - 1)) < 2e-7
+
+
+def test_product_never_touches_the_oracle_or_work_files():
+    """The CUDA path and its binding share nothing with oracle/ (and nothing committed reads
+    _work/): scan the package and the C sources for any reference."""
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    pkg = os.path.join(root, "paper_1009_1380_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if not f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
+                continue
+            text = open(os.path.join(dirpath, f)).read()
+            assert not re.search(r"^\s*(import|from)\s+oracle\b", text, re.M), f
+            assert "liboracle" not in text and "radon_oracle" not in text, f
+            assert "_work/" not in text, f
+    assert "oracle" not in open(os.path.join(root, "include", "radon.h")).read()
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` (the CPU oracle as the reference arm) prints one JSON line with
+    the contract's keys; a tiny sample keeps this to seconds."""
+    import json
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--ref-sample", "8"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-500:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                "scaling", "vs_baseline", "dtype", "data", "config", "e2e", "cpu_baseline"):
+        assert key in line, key
+    assert line["impl"] == "reference" and line["unit"] == "pairs/s" and line["value"] > 0
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["cpu_baseline"]["kind"] == "oracle"
