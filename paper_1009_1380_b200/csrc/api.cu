@@ -96,7 +96,10 @@ static int validate(int N, int n_angles, int n_det, float sigma, int W, int *G_o
     if (fabs(g - (double)G) > 1e-6 || (G & 1)) return RADON_EINVAL;
     if (W != KW) return RADON_EUNSUPPORTED;
     if (!fft_length_supported((int)G)) return RADON_EUNSUPPORTED;
-    if (2 * (long long)n_det - 1 > 8192) return RADON_EUNSUPPORTED;
+    {   // projection DFT: one FFT of length n_det when that is a power of two >= 16, else Bluestein (L >= 2n - 1)
+        const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
+        if (pow2 ? n_det > 8192 : 2 * (long long)n_det - 1 > 8192) return RADON_EUNSUPPORTED;
+    }
     *G_out = (int)G;
     return RADON_OK;
 }
@@ -644,7 +647,7 @@ extern "C" const char *radon_strerror(int code)
     case RADON_ENOMEM: return "out of memory";
     case RADON_ECUDA: return "CUDA runtime error (see radon_last_cuda_error)";
     case RADON_EARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
-    case RADON_EUNSUPPORTED: return "valid request outside this build (W != 6, or sigma*N not a power of two in [16, 8192], or 2*n_det-1 > 8192)";
+    case RADON_EUNSUPPORTED: return "valid request outside this build (W != 6, or sigma*N not a power of two in [16, 8192], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
     default: return "unknown error";
     }
 }

@@ -57,7 +57,7 @@ def test_grid_only_matches_ogrid_and_is_deterministic(rb, shape):
     assert np.array_equal(out1.view(np.uint32), out2.view(np.uint32))    # bitwise, every cell rewritten
 
 
-@pytest.mark.parametrize("nd", [16, 91, 128, 725, 1449, 2048])
+@pytest.mark.parametrize("nd", [2, 3, 16, 91, 128, 725, 1449, 2048, 2897, 4096, 8192])
 def test_projection_dfts_match_plain_dft(rb, nd):
     na = 5
     plan = rb.RadonPlan(64, na, nd)
