@@ -64,7 +64,8 @@ extern "C" {
 #define RADON_ENOMEM       -2   /* host or device allocation failed */
 #define RADON_ECUDA        -3   /* a CUDA runtime call failed (radon_last_cuda_error) */
 #define RADON_EARCH        -4   /* current device is not compute capability 10.x */
-#define RADON_EUNSUPPORTED -5   /* valid but not built: W != 6, sigma*N not a power of two */
+#define RADON_EUNSUPPORTED -5   /* valid but not built: W != 6, sigma*N not a power of two in [16, 8192],
+                                   n_det > 8192 (power of two) or 2*n_det - 1 > 8192 (otherwise) */
 
 typedef struct radon_plan radon_plan;   /* opaque, owned by the library */
 
@@ -76,8 +77,10 @@ typedef struct radon_plan radon_plan;   /* opaque, owned by the library */
  * the conflict-free gather/scatter schedules (the plan-time binning that takes
  * the place of the paper's load-balanced bins), FFT twiddles and
  * chirp tables, and the workspace.  EINVAL: N < 8, n_angles < 1, n_det < 2,
- * n_angles or n_det > 65535, sigma*N not an even integer, W outside [2,12],
- * out == NULL.  On failure *out is set to NULL. */
+ * n_angles > 65535 or n_det > 65533, sigma*N not an even integer, sigma outside (1, 8],
+ * W outside [2,12], out == NULL.  EUNSUPPORTED: see above.  On failure *out is set to NULL.
+ * Device memory: one workspace (T + grid + polar, 185 MB at N = 2048) at creation; the batched
+ * and host-buffer calls allocate three more on first use (four slices in flight). */
 int radon_plan_create(radon_plan **out, int N, int n_angles, int n_det, float sigma, int W);
 
 /* Frees everything the plan owns (synchronises the device first). NULL is OK. */
@@ -89,7 +92,9 @@ int radon_forward(radon_plan *p, const float *d_x, float *d_sino, void *stream);
 /* x~ = Radon^T{y}: exact transpose of radon_forward (PAPER.md:85 with D == 1). */
 int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, void *stream);
 
-/* `batch` contiguous slices sharing the plan (BASELINE.json configs[4]). */
+/* `batch` contiguous slices sharing the plan (BASELINE.json configs[4]).  The slices run on
+ * four internal streams forked from and joined into `stream` (asynchronous for the caller
+ * exactly like the single-slice calls); while stage timing is enabled they run one by one. */
 int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream);
 int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batch, void *stream);
 
