@@ -83,6 +83,84 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
     }
 }
 
+// ---- n_det a power of two: two projections per FFT ---------------------------------------------
+// For n = L a power of two the centring phases are real (a[s] = (-1)^s, b[k] = (-1)^k / n), so
+// real <-> Hermitian symmetry halves the work exactly as in the column passes of the 2-D FFT:
+//   A1 (INV = false): rows y0, y1 real -> one FFT of a .* (y0 + i y1) = W; the two spectra are
+//       untangled through shared memory, Y0[k] = b[k] (W[k] + conj W[-k])/2,
+//       Y1[k] = b[k] (W[k] - conj W[-k])/(2i).
+//   F4 (INV = true, Hermitian-half rows only): P0, P1 completed to Hermitian rows (the stored
+//       half, mirrored and conjugated; the self-mirrored k = n/2 and the unpaired k = 0 keep
+//       their real part: that is what Re{.} of the single-row form leaves of them), one FFT of
+//       conj(P0 + i P1) .* a, r = b .* result; S0 = r.x, S1 = -r.y.
+template <int L, bool INV>
+__global__ void __launch_bounds__(ProjCfg<L>::THREADS, ProjCfg<L>::MIN_CTAS)
+proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
+                 const float2 *__restrict__ ta, const float2 *__restrict__ tb,
+                 const float2 *__restrict__ tw, int n_rows, const float *__restrict__ dens)
+{
+    extern __shared__ __align__(16) float2 s_fft[];
+    using C = ProjCfg<L>;
+    constexpr int TF = C::TF, n = L, c = L / 2;
+    const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
+    float2 *s = s_fft + f * C::PADLEN;
+    const int r0 = 2 * (blockIdx.x * C::NF + f), r1 = r0 + 1;
+    const bool live0 = r0 < n_rows, live1 = r1 < n_rows;
+
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int sidx = t + i * TF;
+        const float a = __ldg(&ta[sidx]).x;
+        if (INV) {
+            const bool self = sidx == 0 || sidx == c;            // keep the real part only
+            const bool mir = sidx < c && sidx != 0;
+            const int src = mir ? 2 * c - sidx : sidx;
+            const float2 *P = reinterpret_cast<const float2 *>(in);
+            float2 p0 = live0 ? __ldg(&P[(size_t)r0 * n + src]) : make_float2(0.f, 0.f);
+            float2 p1 = live1 ? __ldg(&P[(size_t)r1 * n + src]) : make_float2(0.f, 0.f);
+            if (mir) { p0.y = -p0.y; p1.y = -p1.y; }
+            if (self) { p0.y = 0.f; p1.y = 0.f; }
+            // z = p0 + i p1; v = conj(z) * a
+            v[i] = make_float2((p0.x - p1.y) * a, -(p0.y + p1.x) * a);
+        } else {
+            const float y0 = live0 ? __ldg(&in[(size_t)r0 * n + sidx]) : 0.f;
+            const float y1 = live1 ? __ldg(&in[(size_t)r1 * n + sidx]) : 0.f;
+            v[i] = make_float2(y0 * a, y1 * a);
+        }
+    }
+    fft_reg<L, -1>(v, s, tw, t);
+    if (INV) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            const float b = __ldg(&tb[k]).x;
+            if (live0) out[(size_t)r0 * n + k] = v[i].x * b;
+            if (live1) out[(size_t)r1 * n + k] = -v[i].y * b;
+        }
+    } else {
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
+        __syncthreads();
+        float2 *Y = reinterpret_cast<float2 *>(out);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            const float2 wk = v[i], wm = s[FFT_PAD((L - k) & (L - 1))];
+            const float b = __ldg(&tb[k]).x;
+            float2 y0 = make_float2(0.5f * b * (wk.x + wm.x), 0.5f * b * (wk.y - wm.y));
+            float2 y1 = make_float2(0.5f * b * (wk.y + wm.y), 0.5f * b * (wm.x - wk.x));
+            if (dens != nullptr) {        // radon_inverse: density compensation
+                if (live0) { const float w = __ldg(&dens[(size_t)r0 * n + k]); y0.x *= w; y0.y *= w; }
+                if (live1) { const float w = __ldg(&dens[(size_t)r1 * n + k]); y1.x *= w; y1.y *= w; }
+            }
+            if (live0) Y[(size_t)r0 * n + k] = y0;
+            if (live1) Y[(size_t)r1 * n + k] = y1;
+        }
+    }
+}
+
 template <int L>
 static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st)
 {
@@ -95,6 +173,18 @@ static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in
             in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0, dens); \
     }
     const bool blue = p.chirp_hf != nullptr;
+    if (!blue && (!inv || half)) {        // n_det a power of two: two projections per FFT
+        const int pair_blocks = ((p.n_angles + 1) / 2 + C::NF - 1) / C::NF;
+        if (inv) {
+            if (set_smem(proj_pair_kernel<L, true>, C::SMEM)) return -1;
+            proj_pair_kernel<L, true><<<pair_blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens);
+        } else {
+            if (set_smem(proj_pair_kernel<L, false>, C::SMEM)) return -1;
+            proj_pair_kernel<L, false><<<pair_blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens);
+        }
+        count_launch();
+        return 0;
+    }
     if (inv && blue) RADON_PROJ(true, true)
     else if (inv) RADON_PROJ(true, false)
     else if (blue) RADON_PROJ(false, true)
