@@ -226,13 +226,13 @@ __global__ void __launch_bounds__(FftCfg<L>::THREADS, (FftCfg<L>::THREADS <= 256
 rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
                           const float2 *__restrict__ tw, int N, int n_groups)
 {
-    extern __shared__ __align__(128) float2 s_fft[];
+    extern __shared__ __align__(128) float2 s_rows[];   // FFT scratch, then the staged rows
     using C = FftCfg<L>;
     constexpr int TF = C::TF, NF = C::NF;
     __shared__ __align__(8) uint64_t bar;
-    float2 *stage = s_fft + NF * C::PADLEN;                 // NF rows of L, 16-byte aligned
+    float2 *stage = s_rows + NF * C::PADLEN;                 // NF rows of L, 16-byte aligned
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
-    float2 *s = s_fft + f * C::PADLEN;
+    float2 *s = s_rows + f * C::PADLEN;
     const int c = N / 2;
 
     auto fetch = [&](int g) {                               // one thread: rows of group g -> stage
