@@ -346,3 +346,26 @@ def test_inverse_radon_matches_oracle_and_recovers_the_phantom(rb):
     pix = np.random.default_rng(12).choice(cfg.N * cfg.N, 512, replace=False)
     X = plan.radon_inverse(dev(y, torch.float32)).cpu().numpy()
     assert rel(X.ravel()[pix], oracle.inverse(y, cfg.N, pix=pix)) < G1
+
+
+def test_calls_can_be_captured_in_a_cuda_graph(rb):
+    """The device-pointer calls only launch kernels on the given stream (no allocation, no
+    synchronisation after the first use), so a solver loop can capture them in a CUDA graph."""
+    cfg = workloads.get_config(2)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    x = dev(workloads.make_image(2), torch.float32)
+    s = plan.radon_forward(x)
+    xo = plan.radon_adjoint(s)
+    ref_s, ref_x = s.clone(), xo.clone()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        plan.radon_forward(x, s); plan.radon_adjoint(s, xo)       # warm up on the capture stream
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        plan.radon_forward(x, s)
+        plan.radon_adjoint(s, xo)
+    s.zero_(); xo.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(s, ref_s) and torch.equal(xo, ref_x)
