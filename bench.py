@@ -5,7 +5,11 @@ A step = one pass of the whole hot path (radon_forward_batch then radon_adjoint_
 F1-F4 and A1-A4 of SURVEY.md 8(a)) over one batch of `--slices` synthetic 2048^2 slices with
 1025 x 2048 projections (BASELINE.json configs[3] shape, batched as configs[4]).  `value` is
 whole-job pairs/s with inputs resident in HBM; `e2e` is the same metric through the host-buffer
-C-ABI calls (pinned host memory, copies inside the timed region).
+C-ABI calls (pinned host memory, copies inside the timed region).  Beside the contract's keys the
+line carries `stages` (per-stage CUDA events of a second, untimed pass), `roofline` (the dominant
+stage against the measured HBM peak), `gridding_kernels` (the bare interpolation / gridding kernels
+on complex data, SURVEY 8(d)'s 151 MB, north_star's 50 % target), `paper_shape` (PAPER.md:59's own
+180 x 1024 shape, context), `next_rows` (radon_inverse) and `cpu_baseline` (the oracle, sampled).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--slices B] [--impl reference]
   torchrun ... bench.py --gpus N ...      one rank per GPU; slice-parallel replicas (weak scaling)
