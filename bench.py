@@ -382,6 +382,41 @@ def main():
     next_rows = {"radon_inverse_us_per_call": round(e0.elapsed_time(e1) / 20 * 1e3, 1),
                  "note": "A1 with density weights (PAPER.md:89) + A2-A4; one slice at a time"}
 
+    # ---- SURVEY 8(f) item 3 / BASELINE.json configs[2]: the operator pair inside a solver loop
+    #      (iterative soft-thresholding: x <- S_tau(x - alpha A^T (A x - b)));
+    #      the vector updates are torch elementwise ops, the two operator calls are this library ----
+    c3 = workloads.get_config(3)
+    p3 = rb.RadonPlan(c3.N, c3.n_angles, c3.n_det)
+    xt3 = torch.from_numpy(workloads.make_image(3)).float().to(dev)
+    b3 = p3.radon_forward(xt3).clone()
+    v3 = torch.ones_like(xt3)
+    for _ in range(8):
+        w3 = p3.radon_adjoint(p3.radon_forward(v3)).clone()
+        lam = float(w3.norm() / v3.norm())
+        v3 = w3 / w3.norm()
+    alpha, tau = 1.0 / lam, 1e-4
+    x3 = torch.zeros_like(xt3); r3 = torch.empty_like(b3); g3 = torch.empty_like(xt3)
+
+    def ista(n_it):
+        nonlocal x3
+        for _ in range(n_it):
+            p3.radon_forward(x3, r3)
+            r3.sub_(b3)
+            p3.radon_adjoint(r3, g3)
+            x3 = torch.nn.functional.softshrink(x3 - alpha * g3, tau)
+
+    ista(10)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    ista(100)                                              # 200 alternating operator calls
+    e1.record(stream)
+    torch.cuda.synchronize()
+    res = float((p3.radon_forward(x3) - b3).norm() / b3.norm())
+    next_rows["solver_loop_config3"] = {"iterations_per_s": round(100 / (e0.elapsed_time(e1) * 1e-3), 1),
+                                        "operator_calls": 200, "relative_residual_after_110": round(res, 4),
+                                        "note": "ISTA on configs[2] (1024^2, 64 x 1449); latency bound at this size"}
+    del p3
+
     if rank != 0:
         return 0
     cpu_baseline = None
