@@ -297,7 +297,10 @@ def fast_adjoint(y, N, W=6, sigma=2.0):
 # ---- O-density / inverse Radon ---------------
 
 def density(n_angles, n_det, G, W=6, sigma=2.0, brute=False):
-    """D(x_i,y_i) = 1 / sum_j K(x_i - x_j, y_i - y_j) over all polar samples."""
+    """D(x_i,y_i) = 1 / sum_j K(x_i - x_j, y_i - y_j) over all polar samples.
+    brute=True: all M^2 terms as printed.  brute=False: the terms that are exactly zero (|dy| or
+    |dx| > W/2) are skipped by a sort on the y coordinate and a scan of the band (no cell buckets:
+    deliberately a different algorithm from the product's bucketed table)."""
     lib = _load()
     D = np.empty(n_angles * n_det)
     lib.odensity(n_angles, n_det, G, W, kb_beta(W, sigma), int(bool(brute)), _d(D))
@@ -309,12 +312,14 @@ def inverse_scale(n_det, G, W=6, sigma=2.0):
     sum_j K ~ (samples per grid cell) * (integral of K) = rho * phihat(0)^2, so a sample owns
     D * phihat(0)^2 grid cells = D * phihat(0)^2 (2 pi / G)^2 (rad/pixel)^2, and the inverse
     Fourier integral (1/4 pi^2) int xhat e^{i w.X} d^2 w over samples xhat = n * Yhat becomes
-    sum_m Yhat_m e^{...} D_m * n phihat(0)^2 / G^2."""
+    sum_m Yhat_m e^{...} D_m * n phihat(0)^2 / G^2.
+    Pinned (tests/test_oracle_pins.py) against the polar area element the same integral gives
+    directly: D * inverse_scale -> pi |j| / (n_det n_angles) in the mid band."""
     ph0 = float(kb_phihat(0.0, W, kb_beta(W, sigma)))
     return n_det * ph0 * ph0 / float(G * G)
 
 
-def inverse(y, N, sigma=2.0, W=6, pix=None):
+def inverse(y, N, sigma=2.0, W=6, pix=None, brute=False):
     """Density-compensated inverse Radon transform ("inverse Radon", eq. :85 with
     the D of eq. :89): 1-D DFT of every projection, weights D, exact adjoint NDFT, real part."""
     y = _f64(y)
@@ -322,5 +327,5 @@ def inverse(y, N, sigma=2.0, W=6, pix=None):
     G = int(round(sigma * N))
     E = _centered_dft_matrix(n_det, -1)
     Yh = (y @ E.T) / n_det
-    D = density(n_angles, n_det, G, W, sigma)
+    D = density(n_angles, n_det, G, W, sigma, brute=brute)
     return np.real(ndft1(Yh * D, N, pix=pix)) * inverse_scale(n_det, G, W, sigma)

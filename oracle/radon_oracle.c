@@ -415,8 +415,13 @@ static void polar_kappa(int a, int k, int n_angles, int n_det, int G, double *kx
 {
     const double theta = M_PI * (double)a / (double)n_angles;
     const double rho = (double)G * (double)(k - n_det / 2) / (double)n_det;
-    *kx = rho * cos(theta);
-    *ky = rho * sin(theta);
+    /* theta = pi/2 (a = n_angles/2): the mathematical values cos = 0, sin = 1.  libm's       */
+    /* cos(M_PI/2) = 6.1e-17 would push kappa_x off the exact tie of the tap rule S3           */
+    /* (x0 = ceil(kappa - W/2)) in a direction that depends on the sign of j.    */
+    const double c = (2 * a == n_angles) ? 0.0 : cos(theta);
+    const double s = (2 * a == n_angles) ? 1.0 : sin(theta);
+    *kx = rho * c;
+    *ky = rho * s;
 }
 
 static int imod(int a, int m)
@@ -486,9 +491,19 @@ void ogrid_grid(const double *pr, const double *pi, int G, int n_angles, int n_d
 /* the same separable Kaiser-Bessel kernel K(dx,dy) = phi(dx) phi(dy) on the   */
 /* oversampled grid's coordinates (kappa, polar_kappa above).  */
 /* is a garbled duplicate of the same formula (reading S11).                   */
-/* brute != 0: the double sum exactly as printed, O(M^2).  brute == 0: the    */
-/* same sum with the samples bucketed by integer cell so that only cells within*/
-/* the kernel's support are visited (identical terms, other order).            */
+/* brute != 0: the double sum exactly as printed, every one of the M^2 terms.  */
+/* brute == 0: the same sum without the terms that are exactly zero: K vanishes */
+/* outside |dy| < W/2, so the samples are sorted by their y coordinate and, for */
+/* sample i, only the contiguous run of the sorted list with |ky_i - ky_j| <   */
+/* W/2 is visited (found by bisection; a 1-D sort-and-scan, no cell buckets).   */
+/* No wrap mod G: eq. :89 as printed has none.                                  */
+static const double *g_sort_key;
+static int cmp_by_key(const void *a, const void *b)
+{
+    const double x = g_sort_key[*(const long long *)a], y = g_sort_key[*(const long long *)b];
+    return (x > y) - (x < y);
+}
+
 void odensity(int n_angles, int n_det, int G, int W, double beta, int brute, double *D)
 {
     const long long M = (long long)n_angles * n_det;
@@ -504,37 +519,32 @@ void odensity(int n_angles, int n_det, int G, int W, double beta, int brute, dou
             D[i] = 1.0 / s;
         }
     } else {
-        /* buckets: cell (cx,cy) = floor(kappa) + G/2 + 1 in a (G+3)^2 array (kappa in [-G/2, G/2]) */
-        const int B = G + 3, R = W / 2 + 1;
-        long long *start = (long long *)calloc((size_t)B * B + 1, sizeof(long long));
-        long long *order = (long long *)malloc(sizeof(long long) * (size_t)M);
-        int *cell = (int *)malloc(sizeof(int) * (size_t)M);
-        for (long long m = 0; m < M; ++m) {
-            const int cx = (int)floor(kx[m]) + G / 2 + 1, cy = (int)floor(ky[m]) + G / 2 + 1;
-            cell[m] = cy * B + cx;
-            ++start[cell[m] + 1];
-        }
-        for (size_t c = 0; c < (size_t)B * B; ++c) start[c + 1] += start[c];
-        long long *fill = (long long *)malloc(sizeof(long long) * (size_t)B * B);
-        memcpy(fill, start, sizeof(long long) * (size_t)B * B);
-        for (long long m = 0; m < M; ++m) order[fill[cell[m]]++] = m;
+        long long *by_y = (long long *)malloc(sizeof(long long) * (size_t)M);
+        double *ys = (double *)malloc(sizeof(double) * (size_t)M);
+        for (long long m = 0; m < M; ++m) by_y[m] = m;
+        g_sort_key = ky;
+        qsort(by_y, (size_t)M, sizeof(long long), cmp_by_key);
+        for (long long m = 0; m < M; ++m) ys[m] = ky[by_y[m]];
+        const double hw = 0.5 * (double)W;
 #pragma omp parallel for schedule(dynamic, 64)
         for (long long i = 0; i < M; ++i) {
-            const int cx = cell[i] % B, cy = cell[i] / B;
+            /* first sorted position with ys >= ky_i - W/2 */
+            long long lo = 0, hi = M;
+            const double ymin = ky[i] - hw - 1e-9;   /* slack: okb_phi itself decides the support */
+            while (lo < hi) {
+                const long long mid = (lo + hi) / 2;
+                if (ys[mid] < ymin) lo = mid + 1; else hi = mid;
+            }
             double s = 0.0;
-            for (int y = cy - R; y <= cy + R; ++y) {
-                if (y < 0 || y >= B) continue;
-                for (int x = cx - R; x <= cx + R; ++x) {
-                    if (x < 0 || x >= B) continue;
-                    for (long long q = start[y * B + x]; q < start[y * B + x + 1]; ++q) {
-                        const long long j = order[q];
-                        s += okb_phi(kx[i] - kx[j], W, beta) * okb_phi(ky[i] - ky[j], W, beta);
-                    }
-                }
+            for (long long q = lo; q < M && ys[q] <= ky[i] + hw + 1e-9; ++q) {
+                const long long j = by_y[q];
+                const double dx = kx[i] - kx[j];
+                if (fabs(dx) > hw + 1e-9) continue;    /* phi(dx) == 0 there */
+                s += okb_phi(dx, W, beta) * okb_phi(ky[i] - ky[j], W, beta);
             }
             D[i] = 1.0 / s;
         }
-        free(start); free(order); free(cell); free(fill);
+        free(by_y); free(ys);
     }
     free(kx); free(ky);
 }
