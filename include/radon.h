@@ -99,9 +99,13 @@ int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batc
 int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batch, void *stream);
 
 /* Same operators on HOST buffers (pinned or pageable): slices are copied to the
- * device, transformed and copied back on two internal streams so that the copies
- * of neighbouring slices overlap the kernels; returns after the last copy has
- * landed (synchronous).  h_x: batch*N*N fp32, h_sino: batch*n_angles*n_det fp32. */
+ * device, transformed and copied back on four internal streams (one workspace each) so
+ * that the copies of neighbouring slices overlap the kernels.  Synchronous on both
+ * sides: the call first waits for everything queued on the device (cudaDeviceSynchronize:
+ * device-pointer calls of this plan still in flight on a caller stream share its workspace)
+ * and returns after the last copy has landed.  While stage timing is enabled the slices
+ * run one by one on a single internal stream.
+ * h_x: batch*N*N fp32, h_sino: batch*n_angles*n_det fp32. */
 int radon_forward_host(radon_plan *p, const float *h_x, float *h_sino, int batch);
 int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x, int batch);
 
@@ -128,7 +132,8 @@ int radon_proj_fft(radon_plan *p, const float *d_sino, float *d_polar, void *str
 
 /* Stage timing (measurement only).  While enabled, radon_forward / radon_adjoint (and the
  * batch, host and nufft entry points) record one CUDA event on their stream at every stage
- * boundary (pool of 8192 events; recording stops silently when it is full).
+ * boundary (the event pool grows on demand; if an event cannot be created the sample is
+ * truncated and radon_plan_stage_times reports RADON_ENOMEM once).
  * radon_plan_stage_times waits for the last recorded event, adds the elapsed device time of
  * every recorded stage to total_ms[stage] and its count to launches[stage], then clears the
  * pool.  Stages: 0 de-apodise+pad+column FFT, 1 row FFT, 2 inverse gridding (gather),

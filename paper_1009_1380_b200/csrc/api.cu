@@ -40,6 +40,7 @@ struct StageTimer {
     std::vector<cudaEvent_t> ev;      // pool, created on first enable
     std::vector<int> stage;           // stage id that STARTS at ev[i]; -1 = end of a sequence
     size_t used = 0;
+    bool overflow = false;            // an event could not be created: the sample is truncated
     double acc_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
@@ -57,7 +58,8 @@ struct radon_plan {
     cudaStream_t hstream[NWS] = {};
     cudaEvent_t hevent[NWS] = {};
     cudaEvent_t fork_event = nullptr;
-    float *dev_density = nullptr;   // D of PAPER.md:89 times the quadrature scale (built on first radon_inverse)
+    float *dev_density = nullptr;   // D of PAPER.md:89 times the quadrature scale, pair-symmetrised (density_setup)
+    std::vector<float> host_density;   // the same table exactly as eq. :89 gives it (radon_plan_density)
     double density_scale = 0.0;
 };
 
@@ -247,7 +249,15 @@ static int check_launch()
 static inline void mark(radon_plan *p, cudaStream_t st, int stage)
 {
     StageTimer &t = p->timer;
-    if (!t.enabled || t.used >= t.ev.size()) return;
+    if (!t.enabled) return;
+    if (t.used >= t.ev.size()) {                 // pool full: grow it (measurement mode only)
+        const size_t n = t.ev.size() + STAGE_EVENT_POOL;
+        t.ev.resize(n, nullptr);
+        t.stage.resize(n, -1);
+        for (size_t i = t.used; i < n; ++i)
+            if (cudaEventCreate(&t.ev[i]) != cudaSuccess) { t.ev.resize(i); t.stage.resize(i); break; }
+        if (t.used >= t.ev.size()) { t.overflow = true; return; }
+    }
     cudaEventRecord(t.ev[t.used], st);
     t.stage[t.used++] = stage;
 }
@@ -333,7 +343,9 @@ extern "C" int radon_plan_stage_times(radon_plan *p, double total_ms[8], long lo
         if (launches) launches[s] = t.cnt[s];
         t.acc_ms[s] = 0; t.cnt[s] = 0;
     }
-    return RADON_OK;
+    const bool truncated = t.overflow;
+    t.overflow = false;
+    return truncated ? RADON_ENOMEM : RADON_OK;
 }
 
 extern "C" int radon_forward(radon_plan *p, const float *d_x, float *d_sino, void *stream)
@@ -354,10 +366,25 @@ static int density_setup(radon_plan *p)
     if (p->dev_density) return RADON_OK;
     std::vector<float> D;
     try {
-        build_density(p->geo, D, &p->density_scale);
+        build_density(p->geo, p->host_density, &p->density_scale);
+        D = p->host_density;
     } catch (const std::bad_alloc &) {
         return RADON_ENOMEM;
     }
+    // radon_inverse runs the Hermitian-half scatter, which grids the pair (j, -j) as ONE complex
+    // value and its conjugate: that is Re{D_j Yh_j e + D_-j conj(Yh_j) conj(e)} only if both
+    // carry the same weight.  For odd n_det the sample set is point symmetric and D_j == D_-j;
+    // for even n_det j = -n/2 has no partner and D_j != D_-j near the band edge.  The real part
+    // only ever sees the pair sum (D_j + D_-j) Re{Yh_j e}, so giving both the mean is exact.
+    const int n = p->dev.n_det;
+    if ((n & 1) == 0)
+        for (int a = 0; a < p->dev.n_angles; ++a) {
+            float *row = D.data() + (size_t)a * n;
+            for (int k = 1; k < n / 2; ++k) {
+                const float m = 0.5f * (row[k] + row[n - k]);
+                row[k] = m; row[n - k] = m;
+            }
+        }
     return dev_upload(p, &p->dev_density, D);
 }
 
@@ -375,8 +402,7 @@ extern "C" int radon_plan_density(radon_plan *p, float *h_density, double *scale
     int rc = density_setup(p);
     if (rc) return rc;
     if (scale) *scale = p->density_scale;
-    if (h_density)
-        CUDA_TRY(cudaMemcpy(h_density, p->dev_density, (size_t)p->M * sizeof(float), cudaMemcpyDeviceToHost));
+    if (h_density) std::memcpy(h_density, p->host_density.data(), (size_t)p->M * sizeof(float));
     return RADON_OK;
 }
 
@@ -431,17 +457,22 @@ static int batch_run(radon_plan *p, bool fwd, const float *d_in, float *d_out, i
     if (!p->fork_event) CUDA_TRY(cudaEventCreateWithFlags(&p->fork_event, cudaEventDisableTiming));
     CUDA_TRY(cudaEventRecord(p->fork_event, user));
     for (int l = 0; l < lanes; ++l) CUDA_TRY(cudaStreamWaitEvent(p->hstream[l], p->fork_event, 0));
-    for (int b = 0; b < batch; ++b) {
+    for (int b = 0; b < batch && rc == RADON_OK; ++b) {
         const int l = b % lanes;
         rc = fwd ? forward_ws(p, p->ws[l], d_in + b * n_in, d_out + b * n_out, p->hstream[l])
                  : adjoint_ws(p, p->ws[l], d_in + b * n_in, d_out + b * n_out, p->hstream[l]);
-        if (rc) return rc;
     }
+    // join the lanes back into the caller's stream, also after a failure in the middle of the
+    // fork (whatever was queued on the lanes stays ordered before the caller's next work)
     for (int l = 0; l < lanes; ++l) {
-        CUDA_TRY(cudaEventRecord(p->hevent[l], p->hstream[l]));
-        CUDA_TRY(cudaStreamWaitEvent(user, p->hevent[l], 0));
+        cudaError_t e = cudaEventRecord(p->hevent[l], p->hstream[l]);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(user, p->hevent[l], 0);
+        if (e != cudaSuccess && rc == RADON_OK) {
+            g_last_cuda_error = std::string("batch join: ") + cudaGetErrorString(e);
+            rc = RADON_ECUDA;
+        }
     }
-    return RADON_OK;
+    return rc;
 }
 
 extern "C" int radon_forward_batch(radon_plan *p, const float *d_x, float *d_sino, int batch, void *stream)
@@ -454,7 +485,7 @@ extern "C" int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_
     return batch_run(p, false, d_sino, d_x, batch, (cudaStream_t)stream);
 }
 
-// ---- host-buffer entry points: two streams, copies of slice b+1 overlap kernels of slice b
+// ---- host-buffer entry points: NWS internal streams, copies of slice b+1 overlap kernels of slice b
 static int host_setup(radon_plan *p)
 {
     const int G = p->dev.G, N = p->dev.N;
@@ -479,10 +510,15 @@ static int host_run(radon_plan *p, bool fwd, const float *h_in, float *h_out, in
     if (!p || !h_in || !h_out || batch < 0) return RADON_EINVAL;
     int rc = host_setup(p);
     if (rc) return rc;
+    // The internal streams share ws[0..] with device-pointer calls the caller may still have in
+    // flight on a stream this call cannot see: order after everything queued on the device.
+    // (The host entry points are synchronous anyway: they return after the last copy landed.)
+    CUDA_TRY(cudaDeviceSynchronize());
     const size_t nx = (size_t)p->dev.N * p->dev.N, ns = (size_t)p->M;
     const size_t n_in = fwd ? nx : ns, n_out = fwd ? ns : nx;
+    const int lanes = p->timer.enabled ? 1 : NWS;   // stage events mean something on one stream only
     for (int b = 0; b < batch; ++b) {
-        const int i = b % NWS;
+        const int i = b % lanes;
         cudaStream_t st = p->hstream[i];
         Workspace &w = p->ws[i];
         float *d_in = fwd ? w.img : w.sino, *d_out = fwd ? w.sino : w.img;

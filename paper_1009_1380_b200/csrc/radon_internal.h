@@ -66,12 +66,12 @@ constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, 
 #endif
 constexpr int GT_X = RADON_GT_X, GT_Y = RADON_GT_Y;
 constexpr int GT_PITCH = GT_X + KH + 1;   // complex per smem row: 16-byte multiple for the bulk copies
-constexpr int GT_ROWS = GT_Y + KH;    // 69
+constexpr int GT_ROWS = GT_Y + KH;    // 21 rows staged per tile
 #ifndef RADON_GWARPS
 #define RADON_GWARPS 24
 #endif
 constexpr int GATHER_WARPS = RADON_GWARPS;      // consumer warps of the persistent gather CTA (+1 producer warp)
-constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : RADON_GSTAGES;   // tiles in flight per CTA (74 KB each)
+constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : RADON_GSTAGES;   // tiles in flight per CTA (GT_ROWS x GT_PITCH x 8 B = 65.5 KB each)
 #ifndef RADON_GCOST
 #define RADON_GCOST 16
 #endif
