@@ -25,9 +25,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-        ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
-    subprocess.run(cmd, check=True)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    flags = [f for f in NVCC_FLAGS if f not in ("-shared", "-lpthread")] + (["-Xptxas", "-v"] if verbose else [])
+    # one nvcc per translation unit, side by side (the FFT templates dominate the build time)
+    procs, objs = [], []
+    for f in SOURCES:
+        obj = os.path.join(objdir, os.path.splitext(f)[0] + ".o")
+        objs.append(obj)
+        procs.append(subprocess.Popen([nvcc] + flags + ["-c", os.path.join(CSRC, f), "-o", obj]))
+    failed = [f for f, pr in zip(SOURCES, procs) if pr.wait() != 0]
+    if failed:
+        raise subprocess.CalledProcessError(1, "nvcc -c " + " ".join(failed))
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs + ["-lpthread"], check=True)
     return LIB
 
 

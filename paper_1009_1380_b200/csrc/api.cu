@@ -29,6 +29,7 @@ struct Workspace {
     float2 *dcbuf = nullptr;   // (W+1)^2 values: the summed j = 0 samples on the centre window
     float2 *scratch = nullptr; // partial rectangles of the scatter's split tiles (per workspace:
                                // two slices may be gridded at the same time on different streams)
+    int *tickets = nullptr;    // counters of the merge jobs (zero between launches)
     float *img = nullptr;      // N x N   (host-buffer entry points only)
     float *sino = nullptr;     // M       (host-buffer entry points only)
 };
@@ -53,6 +54,7 @@ struct radon_plan {
     Workspace ws[NWS];
     long long M = 0;
     int n_partial = 0;         // scratch slots a workspace needs (max over the two schedule sets)
+    int n_jobs = 0;            // ticket counters a workspace needs (likewise)
     size_t device_bytes = 0;
     long long gather_slots[2] = {0, 0}, gather_filled[2] = {0, 0}, scatter_slots[2] = {0, 0}, scatter_filled[2] = {0, 0};
     cudaStream_t hstream[NWS] = {};
@@ -117,7 +119,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
         cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
         cudaFree(q.merge_jobs);
     }
-    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.dcbuf); cudaFree(w.img); cudaFree(w.sino); }
+    for (auto &w : p->ws) { cudaFree(w.T); cudaFree(w.grid); cudaFree(w.polar); cudaFree(w.scratch); cudaFree(w.tickets); cudaFree(w.dcbuf); cudaFree(w.img); cudaFree(w.sino); }
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     if (p->fork_event) cudaEventDestroy(p->fork_event);
     cudaFree(p->dev_density);
@@ -126,6 +128,23 @@ extern "C" int radon_plan_destroy(radon_plan *p)
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
     }
     delete p;
+    return RADON_OK;
+}
+
+static int workspace_alloc(radon_plan *p, Workspace &w)
+{
+    const int G = p->dev.G, N = p->dev.N;
+    int rc;
+    if (!w.T && (rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
+    if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
+    if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
+    if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
+    if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
+    if (!w.tickets) {
+        const size_t n = (size_t)std::max(p->n_jobs, 1) * MERGE_COUNTERS_PER_JOB;
+        if ((rc = dev_alloc(p, &w.tickets, n))) return rc;
+        CUDA_TRY(cudaMemset(w.tickets, 0, n * sizeof(int)));
+    }
     return RADON_OK;
 }
 
@@ -177,18 +196,9 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         q.n_gather_ctas = (int)sch.gather_ctas.size();
         q.n_scatter_ctas = (int)sch.scatter_ctas.size();
         q.n_merge_jobs = (int)sch.merge_jobs.size();
-        {   // is every cell of the centre window (rows ky >= 0 only on the half grid) inside a split rectangle?
-            bool all = !sch.merge_jobs.empty();
-            for (int uy = (h == 1 ? 0 : -KW / 2); uy <= KW / 2 && all; ++uy)
-                for (int ux = -KW / 2; ux <= KW / 2 && all; ++ux) {
-                    const int cx = G / 2 + ux, cy = G / 2 + uy;
-                    bool in = false;
-                    for (const MergeJob &mj : sch.merge_jobs)
-                        in = in || (cx >= mj.rx0 && cx < mj.rx0 + mj.rw && cy >= mj.ry0 && cy < mj.ry0 + mj.rh);
-                    all = in;
-                }
-            q.dc_fused = all;
-        }
+        q.n_dc_jobs = (int)sch.dc_jobs.size();
+        if (q.n_dc_jobs > MAX_DC_JOBS) return RADON_EINVAL;
+        for (int i = 0; i < q.n_dc_jobs; ++i) q.dc_jobs[i] = sch.dc_jobs[i];
         if ((rc = dev_upload(p, &q.gather_ctas, sch.gather_ctas))) return rc;
         q.n_gather_workers = (int)sch.gather_worker_begin.size() - 1;
         if ((rc = dev_upload(p, &q.gather_worker_begin, sch.gather_worker_begin))) return rc;
@@ -197,18 +207,12 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;
         if ((rc = dev_upload(p, &q.merge_jobs, sch.merge_jobs))) return rc;
         n_partial = std::max(n_partial, sch.n_partial_slots);
+        p->n_jobs = std::max(p->n_jobs, (int)sch.merge_jobs.size());
     }
     // workspaces: the first serves the device-pointer calls, all of them the host-buffer entry
     // points (copies and kernels of NWS slices overlap); allocated on first use beyond the first
-    for (int i = 0; i < 1; ++i) {
-        Workspace &w = p->ws[i];
-        if ((rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
-        if ((rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
-        if ((rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
-        if ((rc = dev_alloc(p, &w.scratch, (size_t)std::max(n_partial, 1) * SR_X * SR_Y))) return rc;
-        if ((rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
-    }
     p->n_partial = n_partial;
+    return workspace_alloc(p, p->ws[0]);
     return RADON_OK;
 }
 
@@ -279,7 +283,7 @@ static int nufft2_ws(radon_plan *p, Workspace &w, bool half, const float *d_x, f
 static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st)
 {
     mark(p, st, 5);
-    if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, w.dcbuf, st)) return RADON_ECUDA;             // A2
+    if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, w.dcbuf, w.tickets, st)) return RADON_ECUDA;             // A2
     mark(p, st, 6);
     if (launch_fft2d_pass(2, p->dev, w.grid, w.T, half ? 0 : 1, st)) return RADON_ECUDA;   // A3 (rows)
     mark(p, st, 7);
@@ -488,17 +492,11 @@ extern "C" int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_
 // ---- host-buffer entry points: NWS internal streams, copies of slice b+1 overlap kernels of slice b
 static int host_setup(radon_plan *p)
 {
-    const int G = p->dev.G, N = p->dev.N;
     for (int i = 0; i < NWS; ++i) {
         if (!p->hstream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
         if (!p->hevent[i]) CUDA_TRY(cudaEventCreateWithFlags(&p->hevent[i], cudaEventDisableTiming));
         int rc;
-        Workspace &w = p->ws[i];
-        if (!w.T && (rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
-        if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
-        if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
-        if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
-        if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
+        if ((rc = workspace_alloc(p, p->ws[i]))) return rc;
         if (!p->ws[i].img && (rc = dev_alloc(p, &p->ws[i].img, (size_t)p->dev.N * p->dev.N))) return rc;
         if (!p->ws[i].sino && (rc = dev_alloc(p, &p->ws[i].sino, (size_t)p->M))) return rc;
     }
@@ -568,7 +566,7 @@ extern "C" int radon_interp_only(radon_plan *p, const float *d_grid, float *d_po
 extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
-    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, p->ws[0].dcbuf, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, p->ws[0].dcbuf, p->ws[0].tickets, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 

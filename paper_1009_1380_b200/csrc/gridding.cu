@@ -2,8 +2,9 @@
 //
 //   gather_kernel    F3  inverse gridding, PAPER.md:87 (regular grid -> polar samples)
 //   scatter_kernel   A2  gridding, PAPER.md:85 with D == 1 (polar samples -> regular grid)
-//   merge_kernel         fixed-order sum of the partial rectangles of split tiles
-//   dc_kernel            the j = 0 samples of all angles, summed and gridded once (DESIGN.md R-tie)
+//                        (+ inside the same launch: the j = 0 samples of all angles summed and
+//                        gridded once, DESIGN.md R-tie, and the fixed-order sum of the partial
+//                        rectangles of split tiles by the last CTA of a tile to finish)
 // (the FFT passes live in fft2d.cu, the projection DFTs in proj.cu)
 #include "kernels.h"
 #include "async_copy.cuh"
@@ -415,44 +416,152 @@ __device__ __forceinline__ bool dc_compute(const float2 *__restrict__ polar, con
     return !(a2 == 0.f && (b2 == 0.f || !half));
 }
 
-// Stand-alone form (plans whose centre rectangles are not split: nobody else could add the
-// window after the scatter): one thread per cell adds its value to the grid, no atomics.
-constexpr int DC_THREADS = 256;
-__global__ void __launch_bounds__(DC_THREADS)
-dc_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, const float *__restrict__ g_lut,
-          const KbPoly kp, int G, int n_det, int n_angles, int half)
+// Fixed-order sum of the partial rectangles of a merge job (split rectangle and / or centre
+// window), rows [y_begin, y_end) of the rectangle: NT threads, two cells (16 bytes) per access,
+// four pairs times four slots in flight per thread.  The order of the additions is the slot
+// order, whoever runs this: bitwise reproducible.  dcbuf: the summed j = 0 samples on the
+// (W+1)^2 centre window (DESIGN.md R-tie).
+template <int NT>
+__device__ __forceinline__ void merge_rows(const MergeJob &j, int y_begin, int y_end, const float2 *__restrict__ scratch,
+                                           float2 *__restrict__ grid, int G, const float2 *__restrict__ dcbuf)
 {
-    __shared__ float2 part[DC_THREADS];
-    float2 add;
-    int ux, uy;
-    if (!dc_compute<DC_THREADS>(polar, g_lut, kp, n_det, n_angles, half, part, add, ux, uy)) return;
-    float2 *cell = grid + (size_t)((G / 2 + uy) & (G - 1)) * G + ((G / 2 + ux) & (G - 1));
-    const float2 c = *cell;
-    *cell = make_float2(c.x + add.x, c.y + add.y);
+    const int ppr = j.rw >> 1, p_begin = ppr * y_begin, p_end = ppr * y_end;        // rw is even (check_schedules)
+    const float4 *src = reinterpret_cast<const float4 *>(scratch + (size_t)j.first_slot * (SR_X * SR_Y));
+    constexpr int SLOT4 = SR_X * SR_Y / 2, ROW4 = SR_X / 2;
+    const bool has_dc = j.expected > j.n_slots;
+    for (int i0 = p_begin + threadIdx.x; i0 < p_end; i0 += 4 * NT) {
+        float4 sum[4];
+        int off[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i = min(i0 + q * NT, p_end - 1), y = i / ppr, x = i - y * ppr;
+            off[q] = y * ROW4 + x;
+            sum[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        for (int s0 = 0; s0 < j.n_slots; s0 += 4) {
+            float4 v[4][4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t)
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    v[t][q] = (s0 + t < j.n_slots) ? __ldcg(&src[(size_t)(s0 + t) * SLOT4 + off[q]])
+                                                   : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int t = 0; t < 4; ++t)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    sum[q].x += v[t][q].x; sum[q].y += v[t][q].y; sum[q].z += v[t][q].z; sum[q].w += v[t][q].w;
+                }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i = i0 + q * NT;
+            if (i >= p_end) continue;
+            const int y = i / ppr, x = 2 * (i - y * ppr);
+            if (has_dc) {
+                const int uy = j.ry0 + y - G / 2, ux = j.rx0 + x - G / 2;
+                if (uy >= -KW / 2 && uy <= KW / 2) {
+                    if (ux >= -KW / 2 && ux <= KW / 2) {
+                        const float2 d = __ldcg(&dcbuf[(uy + KW / 2) * (KW + 1) + ux + KW / 2]);
+                        sum[q].x += d.x; sum[q].y += d.y;
+                    }
+                    if (ux + 1 >= -KW / 2 && ux + 1 <= KW / 2) {
+                        const float2 d = __ldcg(&dcbuf[(uy + KW / 2) * (KW + 1) + ux + 1 + KW / 2]);
+                        sum[q].z += d.x; sum[q].w += d.y;
+                    }
+                }
+            }
+            *reinterpret_cast<float4 *>(grid + (size_t)(j.ry0 + y) * G + j.rx0 + x) = sum[q];
+        }
+    }
 }
+
+// A CTA's part in merge job `job` (all NT threads call it, after this CTA's contribution to the
+// job is complete and fenced).  Three counters per job: arrivals, row chunks claimed, departures.
+// The job is READY once all `expected` contributions have arrived; from then on any of its CTAs
+// claims row chunks and merges them.  The CTA that makes the job ready always drains the chunk
+// counter, so the merge completes whoever helps; the others (the CTAs of a split rectangle get
+// the same number of rounds and finish together) wait a BOUNDED time for the job to become
+// ready, so that the rows are merged side by side instead of by the last CTA alone, and leave
+// without helping when the bound expires.  The last CTA to depart re-arms the counters for the
+// next launch (also under graph replay: no host-side epoch).
+constexpr int MERGE_COUNTERS = MERGE_COUNTERS_PER_JOB;   // ints per job: arrivals, chunks, departures, pad
+#ifndef RADON_MERGE_WAIT_NS
+#define RADON_MERGE_WAIT_NS 20000
+#endif
+template <int NT>
+__device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *__restrict__ jobs, int *__restrict__ tickets,
+                                           const float2 *__restrict__ scratch, float2 *__restrict__ grid, int G,
+                                           const float2 *__restrict__ dcbuf, int *s_flag)
+{
+    int *cnt = tickets + job * MERGE_COUNTERS;
+    const MergeJob j = jobs[job];
+    __syncthreads();                              // every thread's writes are fenced
+    if (threadIdx.x == 0) {
+        bool ready = atomicAdd(&cnt[0], 1) == j.expected - 1;
+        if (!ready && wait) {
+            unsigned long long t0, t1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+            do {
+                __nanosleep(256);
+                int a;
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(a) : "l"(&cnt[0]) : "memory");
+                ready = a >= j.expected;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+            } while (!ready && t1 - t0 < (unsigned long long)RADON_MERGE_WAIT_NS);
+        }
+        *s_flag = ready ? 1 : 0;
+    }
+    __syncthreads();
+    if (*s_flag) {
+        __threadfence();                          // the other CTAs' slots, fenced before their arrivals
+        // chunks of rows: about two per contributing CTA, an even number of rows each
+        int rows = max(2, (j.rh / (2 * j.n_slots)) & ~1);
+        const int n_chunks = (j.rh + rows - 1) / rows;
+        for (;;) {
+            __syncthreads();
+            if (threadIdx.x == 0) *s_flag = atomicAdd(&cnt[1], 1);
+            __syncthreads();
+            const int c = *s_flag;
+            if (c >= n_chunks) break;
+            merge_rows<NT>(j, c * rows, min(j.rh, (c + 1) * rows), scratch, grid, G, dcbuf);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&cnt[2], 1) == j.expected - 1) {
+        cnt[0] = 0; cnt[1] = 0; cnt[2] = 0;       // everybody has left: nobody reads the counters any more
+    }
+}
+
+struct DcJobs { int n; int job[MAX_DC_JOBS]; };
 
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
                const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
-               int G, int n_det, int nyq_split, float2 *__restrict__ dcbuf, int n_angles, int half)
+               int G, int n_det, int nyq_split, float2 *__restrict__ dcbuf, int n_angles, int half,
+               const MergeJob *__restrict__ jobs, int *__restrict__ tickets, const DcJobs dcj)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *acc = reinterpret_cast<float2 *>(smem_raw);
-    if (dcbuf != nullptr && blockIdx.x == gridDim.x - 1) {
-        // one extra CTA: the j = 0 samples, summed while the others grid; merge_kernel adds
-        // dcbuf to the centre window when it writes those cells (DESIGN.md R-tie)
+    __shared__ int s_flag;
+    if (blockIdx.x == 0) {
+        // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
+        // footprint of the sum is added by the merge of the centre rectangles (DESIGN.md R-tie)
         float2 add;
         int ux, uy;
         dc_compute<SCATTER_THREADS>(polar, g_lut, kp, n_det, n_angles, half, acc, add, ux, uy);
         if (threadIdx.x < DC_CELLS) dcbuf[threadIdx.x] = add;
+        __threadfence();
+        for (int q = 0; q < dcj.n; ++q)
+            join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
         return;
     }
     float *s_lut = reinterpret_cast<float *>(smem_raw + SCATTER_ACC_BYTES);
     __shared__ ScatterCta cta;
 
     if (threadIdx.x < sizeof(ScatterCta) / 4)
-        reinterpret_cast<int *>(&cta)[threadIdx.x] = reinterpret_cast<const int *>(&ctas[blockIdx.x])[threadIdx.x];
+        reinterpret_cast<int *>(&cta)[threadIdx.x] = reinterpret_cast<const int *>(&ctas[blockIdx.x - 1])[threadIdx.x];
     load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
 
@@ -538,42 +647,20 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     if (threadIdx.x < cta.rh)
         bulk_s2g(dst + (size_t)threadIdx.x * dpitch, acc + threadIdx.x * ACC_PITCH, (uint32_t)(cta.rw * sizeof(float2)));
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the reads
-}
-
-// Fixed-order sum of the partial rectangles of a split (heavy) rectangle: one thread per cell.
-constexpr int MERGE_THREADS = 256;
-constexpr int MERGE_CHUNKS = (SR_X * SR_Y + MERGE_THREADS - 1) / MERGE_THREADS;
-__global__ void __launch_bounds__(MERGE_THREADS)
-merge_kernel(const float2 *__restrict__ scratch, float2 *__restrict__ grid,
-             const MergeJob *__restrict__ jobs, int G, const float2 *__restrict__ dcbuf)
-{
-    const MergeJob j = jobs[blockIdx.x / MERGE_CHUNKS];
-    const int i = (blockIdx.x % MERGE_CHUNKS) * MERGE_THREADS + threadIdx.x;
-    if (i >= j.rw * j.rh) return;
-    const int y = i / j.rw, x = i - y * j.rw;
-    const float2 *src = scratch + (size_t)j.first_slot * (SR_X * SR_Y) + y * SR_X + x;
-    float sr = 0.f, si = 0.f;
-#pragma unroll 4
-    for (int s = 0; s < j.n_slots; ++s) {
-        const float2 c = __ldg(&src[(size_t)s * (SR_X * SR_Y)]);
-        sr += c.x;
-        si += c.y;
+    if (cta.job < 0) {
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the reads
+        return;
     }
-    if (dcbuf != nullptr) {            // centre window: the summed j = 0 samples (dc_compute)
-        const int ux = j.rx0 + x - G / 2, uy = j.ry0 + y - G / 2;
-        if (ux >= -KW / 2 && ux <= KW / 2 && uy >= -KW / 2 && uy <= KW / 2) {
-            const float2 d = dcbuf[(uy + KW / 2) * (KW + 1) + ux + KW / 2];
-            sr += d.x;
-            si += d.y;
-        }
-    }
-    grid[(size_t)(j.ry0 + y) * G + j.rx0 + x] = make_float2(sr, si);
+    // partial rectangle: its writes must have landed, and be visible device-wide, before the ticket
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    asm volatile("fence.proxy.async;" ::: "memory");
+    __threadfence();
+    join_merge<SCATTER_THREADS>(cta.job, true, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
 }
 
 // The j = 0 samples (k = n/2) of all angles sit at kappa = (0,0) and share one footprint, so
-// they are left out of the scatter schedules: their values are summed here (fixed order) and
-// the footprint is added once, after scatter + merge, one thread per cell (no atomics).
+// they are left out of the scatter schedules: CTA 0 sums their values (fixed order) and the
+// footprint of the sum is added once, by the merge of the centre rectangles (no atomics).
 // Full grid: V * wA(kx) wA(ky), wA = the rule-A taps [-W/2, W/2) of an exact tie (delta = 0).
 // Hermitian half (rows ky >= 0 only; the rows below are implied by symmetry): the Hermitian
 // part of that footprint, (V wA(kx) wA(ky) + conj(V) wB(kx) wB(ky)) / 2, wB(u) = wA(-u) the
@@ -590,25 +677,18 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
 }
 
 int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch,
-                   float2 *dcbuf, cudaStream_t st)
+                   float2 *dcbuf, int *tickets, cudaStream_t st)
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     const int nyq = (half && (p.n_det & 1) == 0) ? 1 : 0;
-    // dc_fused: every cell of the centre window lies in a split rectangle, so merge_kernel can
-    // add the summed j = 0 samples; they are summed by one extra CTA of the scatter launch
-    float2 *dcb = q.dc_fused ? dcbuf : nullptr;
-    scatter_kernel<<<q.n_scatter_ctas + (dcb ? 1 : 0), SCATTER_THREADS, SCATTER_SMEM, st>>>(
+    DcJobs dcj;
+    dcj.n = q.n_dc_jobs;
+    for (int i = 0; i < MAX_DC_JOBS; ++i) dcj.job[i] = q.dc_jobs[i];
+    // CTA 0 sums the j = 0 samples; CTA b > 0 grids scatter_ctas[b - 1] (heaviest first)
+    scatter_kernel<<<q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st>>>(
         polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, nyq,
-        dcb, p.n_angles, half ? 1 : 0);
+        dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);
     count_launch();
-    if (q.n_merge_jobs > 0) {
-        merge_kernel<<<q.n_merge_jobs * MERGE_CHUNKS, MERGE_THREADS, 0, st>>>(scratch, grid, q.merge_jobs, p.G, dcb);
-        count_launch();
-    }
-    if (!dcb) {
-        dc_kernel<<<1, DC_THREADS, 0, st>>>(polar, grid, p.lut, p.kb, p.G, p.n_det, p.n_angles, half ? 1 : 0);
-        count_launch();
-    }
     return 0;
 }
 

@@ -29,7 +29,7 @@ struct DevicePlan {
         ScatterCta *scatter_ctas = nullptr; int n_scatter_ctas = 0;
         Slot *scatter_slots = nullptr;
         MergeJob *merge_jobs = nullptr;     int n_merge_jobs = 0;
-        bool dc_fused = false;              // the centre window lies in split rectangles: merge adds the j = 0 sum
+        int dc_jobs[MAX_DC_JOBS] = {0, 0, 0, 0}; int n_dc_jobs = 0;    // merge jobs that add the j = 0 sum
     } sched[2];
 };
 
@@ -80,8 +80,10 @@ static inline int set_smem(F kernel, size_t bytes)
 int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *polar, cudaStream_t st);
 // scratch: room for the partial rectangles of the schedule's split tiles (one set per stream in flight)
 // dcbuf: (W+1)^2 float2 per stream in flight (the summed j = 0 samples on the centre window)
+// tickets: MERGE_COUNTERS zero-initialised ints per merge job per stream in flight (re-armed by the kernel)
+constexpr int MERGE_COUNTERS_PER_JOB = 4;
 int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *grid, float2 *scratch,
-                   float2 *dcbuf, cudaStream_t st);
+                   float2 *dcbuf, int *tickets, cudaStream_t st);
 // which: 0 colpass_fwd (x -> T), 1 rowpass_fwd (T -> grid; flag 1: also write every mirrored row,
 // flag 2: only the mirrored rows the half gather reads, |ky| <= W/2 and |ky - G/2| <= W/2),
 // 2 rowpass_inv (grid -> T; flag: fold the mirrored rows in), 3 colpass_inv (T -> x).

@@ -18,11 +18,13 @@
 //         fixed -> bitwise reproducible;
 //   * tiles whose sample count (polar sampling is ~1/r dense: PAPER.md:57's imbalance) would
 //     make one block run long are split over several warps / blocks by dealing their samples
-//     round-robin; partial rectangles are summed in a fixed order by a merge kernel.
+//     round-robin; partial rectangles are summed in slot order by the last CTA of the tile
+//     to finish (ticket), inside the scatter launch.
 #include "radon_internal.h"
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <thread>
@@ -515,7 +517,8 @@ static void build_scatter(const Geometry &g, Schedules &out)
     const bool half = out.half;
     const int k_end = scatter_k_end(g, half);
     // measured at config 4: 48 is best for the half schedule (66 vs 79 us), 96 for the full one (108 vs 118 us)
-    const int round_max = half ? SCATTER_ROUND_MAX / 2 : SCATTER_ROUND_MAX;
+    int round_max = half ? SCATTER_ROUND_MAX / 2 : SCATTER_ROUND_MAX;
+    if (const char *e = std::getenv(half ? "RADON_TUNE_RMAX_HALF" : "RADON_TUNE_RMAX_FULL")) round_max = std::atoi(e);
     const int nrx = (G + SR_X - 1) / SR_X;
     std::vector<RowSeg> segs;
     std::vector<RectGeom> rects;
@@ -641,18 +644,30 @@ static void build_scatter(const Geometry &g, Schedules &out)
         const int base = (int)(out.scatter_slots.size() / 32);
         out.scatter_slots.insert(out.scatter_slots.end(), tmp_slots.begin(), tmp_slots.end());
         out.scatter_filled += f;
-        int first_slot = -1;
-        if (K > 1) {
+        // cells of the centre window (the footprint of the summed j = 0 samples, DESIGN.md R-tie;
+        // rows ky >= 0 only on the half grid) in this rectangle: then it is a merge job even when
+        // one CTA grids it, because the merge is where that sum is added
+        bool has_dc = false;
+        for (int uy = (half ? 0 : -KW / 2); uy <= KW / 2; ++uy)
+            for (int ux = -KW / 2; ux <= KW / 2; ++ux) {
+                const int cx = G / 2 + ux, cy = G / 2 + uy;
+                has_dc = has_dc || (cx >= rx0 && cx < rx0 + rw && cy >= ry0 && cy < ry0 + rh);
+            }
+        int first_slot = -1, job = -1;
+        if (K > 1 || has_dc) {
             first_slot = out.n_partial_slots;
             out.n_partial_slots += K;
-            MergeJob mj{rx0, ry0, rw, rh, first_slot, K};
+            job = (int)out.merge_jobs.size();
+            MergeJob mj{rx0, ry0, rw, rh, first_slot, K, K + (has_dc ? 1 : 0), 0};
             out.merge_jobs.push_back(mj);
+            if (has_dc) out.dc_jobs.push_back(job);
         }
         for (int kk = 0; kk < K; ++kk) {
             Pending p;
             std::memset(&p.cta, 0, sizeof(p.cta));
             p.cta.rx0 = rx0; p.cta.ry0 = ry0; p.cta.rw = rw; p.cta.rh = rh;
-            p.cta.partial_slot = (K > 1) ? first_slot + kk : -1;
+            p.cta.partial_slot = (job >= 0) ? first_slot + kk : -1;
+            p.cta.job = job;
             p.work = 0;
             for (int it = 0; it < SCATTER_ITEMS; ++it) {
                 p.cta.items[it] = geom[it];
@@ -811,6 +826,32 @@ long long check_schedules(const Geometry &g, const Schedules &s)
                         }
                 }
             }
+        }
+    }
+    {   // every cell of the centre window lies in exactly one dc job; tickets are consistent
+        if ((int)s.dc_jobs.size() > MAX_DC_JOBS) ++bad;
+        std::vector<int> is_dc(s.merge_jobs.size(), 0);
+        for (int j : s.dc_jobs) { if (j < 0 || j >= (int)s.merge_jobs.size()) { ++bad; continue; } ++is_dc[j]; }
+        for (size_t j = 0; j < s.merge_jobs.size(); ++j)
+            if (is_dc[j] > 1 || s.merge_jobs[j].expected != s.merge_jobs[j].n_slots + is_dc[j]) ++bad;
+        for (int uy = (half ? 0 : -KW / 2); uy <= KW / 2; ++uy)
+            for (int ux = -KW / 2; ux <= KW / 2; ++ux) {
+                const int cx = G / 2 + ux, cy = G / 2 + uy;
+                int n = 0;
+                for (int j : s.dc_jobs) {
+                    if (j < 0 || j >= (int)s.merge_jobs.size()) continue;
+                    const MergeJob &mj = s.merge_jobs[j];
+                    n += (cx >= mj.rx0 && cx < mj.rx0 + mj.rw && cy >= mj.ry0 && cy < mj.ry0 + mj.rh) ? 1 : 0;
+                }
+                if (n != 1) ++bad;
+            }
+        for (const ScatterCta &c : s.scatter_ctas) {
+            if ((c.partial_slot >= 0) != (c.job >= 0)) { ++bad; continue; }
+            if (c.job < 0) continue;
+            if (c.job >= (int)s.merge_jobs.size()) { ++bad; continue; }
+            const MergeJob &mj = s.merge_jobs[c.job];
+            if (c.partial_slot < mj.first_slot || c.partial_slot >= mj.first_slot + mj.n_slots ||
+                c.rx0 != mj.rx0 || c.ry0 != mj.ry0 || c.rw != mj.rw || c.rh != mj.rh) ++bad;
         }
     }
     for (const MergeJob &mj : s.merge_jobs) {

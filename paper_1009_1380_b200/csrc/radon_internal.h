@@ -133,14 +133,22 @@ struct ScatterItem {            // one warp: quadrant (relative to the rectangle
 struct ScatterCta {
     int rx0, ry0, rw, rh;       // output rectangle (cells this CTA, alone, writes)
     int partial_slot;           // -1: write the grid; >= 0: write this scratch slot
-    int pad0, pad1, pad2;
+    int job;                    // merge job the partial rectangle belongs to (-1: none)
+    int pad1, pad2;
     ScatterItem items[SCATTER_ITEMS];
 };
 
-struct MergeJob {               // sum n_slots partial rectangles, in order, into the grid
+// A rectangle whose samples are split over several CTAs (polar sampling is ~1/r dense), or
+// that holds cells of the centre window the summed j = 0 samples are added to: every CTA of
+// the job writes its partial rectangle to a scratch slot and takes a ticket; whoever draws the
+// last ticket sums the slots IN SLOT ORDER (bitwise reproducible whatever the arrival order).
+struct MergeJob {
     int rx0, ry0, rw, rh;
     int first_slot, n_slots;
+    int expected;               // tickets: n_slots, + 1 when the j = 0 sum (dc) takes part
+    int pad;
 };
+constexpr int MAX_DC_JOBS = 4;  // the (W+1)^2 centre window touches at most 2 x 2 rectangles
 
 // ---- host-side geometry + schedules ----------------------------------------------
 struct Geometry {
@@ -161,6 +169,7 @@ struct Schedules {
     std::vector<Slot> scatter_slots;
     std::vector<ScatterCta> scatter_ctas;
     std::vector<MergeJob> merge_jobs;
+    std::vector<int> dc_jobs;               // merge jobs whose rectangle holds cells of the centre window
     int n_partial_slots = 0;
     bool half = false;
     long long gather_filled = 0, scatter_filled = 0;
