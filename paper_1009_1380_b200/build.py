@@ -28,6 +28,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     flags = [f for f in NVCC_FLAGS if f not in ("-shared", "-lpthread")] + (["-Xptxas", "-v"] if verbose else [])
+    flags += os.environ.get("RADON_NVCC_DEFS", "").split()      # tuning builds: -DRADON_...=...
     # one nvcc per translation unit, side by side (the FFT templates dominate the build time)
     procs, objs = [], []
     for f in SOURCES:

@@ -330,9 +330,25 @@ __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float 
     RADON_ROW_LD(O0, c) RADON_ROW_LD(O1, d) RADON_ROW_LD(O2, e) RADON_ROW_FMA(V0, c) RADON_ROW_FMA(V1, d) \
     RADON_ROW_FMA(V2, e) RADON_ROW_ST(O0, c) RADON_ROW_ST(O1, d) RADON_ROW_ST(O2, e) RADON_WARP_BAR
 
+// byte offsets of footprint rows 1..5 as literals (they become immediate offsets of the PTX block)
+#if RADON_ST_X * RADON_SQ_X == 128
+#define RADON_RO1 1040
+#define RADON_RO2 2080
+#define RADON_RO3 3120
+#define RADON_RO4 4160
+#define RADON_RO5 5200
+#elif RADON_ST_X * RADON_SQ_X == 64
+#define RADON_RO1 528
+#define RADON_RO2 1056
+#define RADON_RO3 1584
+#define RADON_RO4 2112
+#define RADON_RO5 2640
+#else
+#error "add the row offsets of this accumulator pitch"
+#endif
 __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, float vr, float vi, const Taps &tp)
 {
-    static_assert(KW == 6 && ACC_PITCH * sizeof(float2) == 1040, "row offsets below are written for W = 6, pitch 130");
+    static_assert(KW == 6 && ACC_PITCH * sizeof(float2) == RADON_RO1, "row offsets are written for W = 6 and this pitch");
     uint64_t v[KW], w[KW];
 #pragma unroll
     for (int l = 0; l < KW; ++l) {
@@ -348,27 +364,26 @@ __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, f
         "mov.b64 d0, 0;\n mov.b64 d1, 0;\n mov.b64 d2, 0;\n mov.b64 d3, 0;\n mov.b64 d4, 0;\n mov.b64 d5, 0;\n"
         "mov.b64 e0, 0;\n mov.b64 e1, 0;\n mov.b64 e2, 0;\n mov.b64 e3, 0;\n mov.b64 e4, 0;\n mov.b64 e5, 0;\n"
 #if RADON_SC_STEP_ROWS == 1
-        RADON_STEP1(0, "%2") RADON_STEP1(1040, "%3") RADON_STEP1(2080, "%4")
-        RADON_STEP1(3120, "%5") RADON_STEP1(4160, "%6") RADON_STEP1(5200, "%7")
+        RADON_STEP1(0, "%2") RADON_STEP1(RADON_RO1, "%3") RADON_STEP1(RADON_RO2, "%4")
+        RADON_STEP1(RADON_RO3, "%5") RADON_STEP1(RADON_RO4, "%6") RADON_STEP1(RADON_RO5, "%7")
 #elif RADON_SC_STEP_ROWS == 2
-        RADON_STEP2(0, "%2", 1040, "%3") RADON_STEP2(2080, "%4", 3120, "%5") RADON_STEP2(4160, "%6", 5200, "%7")
+        RADON_STEP2(0, "%2", RADON_RO1, "%3") RADON_STEP2(RADON_RO2, "%4", RADON_RO3, "%5") RADON_STEP2(RADON_RO4, "%6", RADON_RO5, "%7")
 #else
-        RADON_STEP3(0, "%2", 1040, "%3", 2080, "%4") RADON_STEP3(3120, "%5", 4160, "%6", 5200, "%7")
+        RADON_STEP3(0, "%2", RADON_RO1, "%3", RADON_RO2, "%4") RADON_STEP3(RADON_RO3, "%5", RADON_RO4, "%6", RADON_RO5, "%7")
 #endif
         "}\n" ::"r"(addr), "r"(act), "l"(v[0]), "l"(v[1]), "l"(v[2]), "l"(v[3]), "l"(v[4]), "l"(v[5]),
         "l"(w[0]), "l"(w[1]), "l"(w[2]), "l"(w[3]), "l"(w[4]), "l"(w[5]) : "memory");
 }
 
 constexpr int DC_CELLS = (KW + 1) * (KW + 1);
-// NT threads of one CTA: sum the j = 0 samples (fixed order), then thread t < DC_CELLS holds the
-// value to add to window cell t (offset ux = t % (W+1) - W/2, uy = t / (W+1) - W/2 from DC);
-// returns false where nothing is to be added.  part: NT float2 of shared memory.
+// NT threads of one CTA: sum the j = 0 samples of all angles (fixed order) and write the value
+// to add to each cell of the (W+1)^2 centre window to dcbuf (cell c: offset ux = c % (W+1) - W/2,
+// uy = c / (W+1) - W/2 from DC; zero where nothing is to be added).  part: NT float2 of shared memory.
 template <int NT>
-__device__ __forceinline__ bool dc_compute(const float2 *__restrict__ polar, const float *__restrict__ g_lut,
+__device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, const float *__restrict__ g_lut,
                                            const KbPoly &kp, int n_det, int n_angles, int half,
-                                           float2 *part, float2 &add, int &ux, int &uy)
+                                           float2 *part, float2 *__restrict__ dcbuf)
 {
-    static_assert(DC_CELLS <= NT, "one thread per cell of the (W+1)^2 window");
     const int t = threadIdx.x, cd = n_det / 2;
     float sr = 0.f, si = 0.f;
     for (int a0 = 0; a0 < n_angles; a0 += 8 * NT) {              // 8 independent loads in flight
@@ -396,24 +411,24 @@ __device__ __forceinline__ bool dc_compute(const float2 *__restrict__ polar, con
     kb_poly_weights(kp, 0.f, wa);
     kb_poly_weights(kp, 1.f, wb);
 #endif
-    add = make_float2(0.f, 0.f);
-    ux = t % (KW + 1) - KW / 2; uy = t / (KW + 1) - KW / 2;     // cell offset from DC: -W/2 .. W/2
-    if (t >= DC_CELLS) return false;
     auto tap = [](const float (&w)[KW], int l) {
         float r = 0.f;
 #pragma unroll
         for (int q = 0; q < KW; ++q) r = (q == l) ? w[q] : r;
         return r;
     };
-    const float a2 = tap(wa, ux + KW / 2) * tap(wa, uy + KW / 2);           // taps -W/2 .. W/2-1
-    const float b2 = tap(wb, ux + KW / 2 - 1) * tap(wb, uy + KW / 2 - 1);   // taps -W/2+1 .. W/2
-    if (half) {
-        if (uy < 0) return false;
-        add = make_float2(0.5f * V.x * (a2 + b2), 0.5f * V.y * (a2 - b2));
-    } else {
-        add = make_float2(V.x * a2, V.y * a2);
+    for (int c = t; c < DC_CELLS; c += NT) {
+        const int ux = c % (KW + 1) - KW / 2, uy = c / (KW + 1) - KW / 2;     // cell offset from DC: -W/2 .. W/2
+        const float a2 = tap(wa, ux + KW / 2) * tap(wa, uy + KW / 2);           // taps -W/2 .. W/2-1
+        const float b2 = tap(wb, ux + KW / 2 - 1) * tap(wb, uy + KW / 2 - 1);   // taps -W/2+1 .. W/2
+        float2 add = make_float2(0.f, 0.f);
+        if (half) {
+            if (uy >= 0) add = make_float2(0.5f * V.x * (a2 + b2), 0.5f * V.y * (a2 - b2));
+        } else {
+            add = make_float2(V.x * a2, V.y * a2);
+        }
+        dcbuf[c] = add;
     }
-    return !(a2 == 0.f && (b2 == 0.f || !half));
 }
 
 // Fixed-order sum of the partial rectangles of a merge job (split rectangle and / or centre
@@ -548,10 +563,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     if (blockIdx.x == 0) {
         // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
         // footprint of the sum is added by the merge of the centre rectangles (DESIGN.md R-tie)
-        float2 add;
-        int ux, uy;
-        dc_compute<SCATTER_THREADS>(polar, g_lut, kp, n_det, n_angles, half, acc, add, ux, uy);
-        if (threadIdx.x < DC_CELLS) dcbuf[threadIdx.x] = add;
+        dc_compute<SCATTER_THREADS>(polar, g_lut, kp, n_det, n_angles, half, acc, dcbuf);
         __threadfence();
         for (int q = 0; q < dcj.n; ++q)
             join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
