@@ -28,6 +28,13 @@ Functions (each cites the passage it follows; details in radon_oracle.c):
    and the density-compensated inverse Radon transform (PAPER.md:51,
   :85): weights times the exact adjoint NDFT.
 
+* ``polyfilter``  O-filter: the sinogram filter of the paper's objective
+  ("3rd order polynomial fit", PAPER.md:27; filter(Radon{x} - data), :31, :47):
+  least-squares polynomial fit along one axis of the sinogram, subtracted.
+* ``ista_step``   O-solver: one iteration x <- S_tau(x - alpha A^T F (A x - b)) of the
+  iterative soft-thresholding stand-in for the solver loop,
+  on any (forward, adjoint) pair of this module.
+
 All pinned in tests/test_oracle_pins.py; nothing here is
 "parity unpinned".
 """
@@ -329,3 +336,37 @@ def inverse(y, N, sigma=2.0, W=6, pix=None, brute=False):
     Yh = (y @ E.T) / n_det
     D = density(n_angles, n_det, G, W, sigma, brute=brute)
     return np.real(ndft1(Yh * D, N, pix=pix)) * inverse_scale(n_det, G, W, sigma)
+
+
+# ---- O-filter / O-solver ----------------
+
+def polyfilter(sino, order=3, axis=1):
+    """filter(.) of PAPER.md:31/:47 under reading R-filter: along `axis` of
+    the sinogram (1: the detector coordinate of every projection, the default; 0: the angle
+    coordinate of every detector bin) fit a polynomial of degree `order` by least squares
+    ("3rd order polynomial fit") and subtract it ("polynomial subtraction", :41).
+    Plain normal equations on the Vandermonde matrix of t in [-1, 1], fp64."""
+    z = np.moveaxis(_f64(sino), axis, -1)
+    n = z.shape[-1]
+    t = np.linspace(-1.0, 1.0, n) if n > 1 else np.zeros(1)
+    V = np.vander(t, order + 1, increasing=True)            # n x (order + 1)
+    coef = np.linalg.solve(V.T @ V, V.T @ z[..., None])     # normal equations, one right-hand side per line
+    out = z - (V @ coef)[..., 0]
+    return np.moveaxis(out, -1, axis)
+
+
+def soft_threshold(v, tau):
+    """S_tau(v) = sign(v) max(|v| - tau, 0): the proximal map of tau ||.||_1."""
+    v = _f64(v)
+    return np.sign(v) * np.maximum(np.abs(v) - tau, 0.0)
+
+
+def ista_step(x, b, alpha, tau, fwd, adj, order=None):
+    """One iteration of x <- S_tau(x - alpha A^T F (A x - b)), F = polyfilter(order) or the
+    identity (order None): the gradient step on (1/2)||F(Ax - b)||^2 (F is an orthogonal
+    projector: F^T F = F) followed by the l1 shrinkage, the building block a basis-pursuit
+    solver repeats around y = Radon{x}.  fwd(x) / adj(y): the operator pair."""
+    r = fwd(x) - _f64(b)
+    if order is not None:
+        r = polyfilter(r, order)
+    return soft_threshold(_f64(x) - alpha * adj(r), tau)

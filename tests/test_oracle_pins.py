@@ -395,3 +395,85 @@ def test_inverse_recovers_a_gaussian_blob():
     # a pixel subset is exact (independent sums)
     pix = np.array([5, 77, N * N - 1, (N // 2 - 7) * N + N // 2 + 5])
     assert np.allclose(oracle.inverse(oracle.forward(x, na, nd), N, pix=pix), xr.ravel()[pix], rtol=1e-12, atol=1e-14)
+
+
+# ---------------------------------------------------------------- O-filter / O-solver ----
+@pytest.mark.parametrize("axis", [0, 1])
+def test_filter_annihilates_polynomials_and_is_an_orthogonal_projector(axis):
+    """PAPER.md:27 "3rd order polynomial fit ... polynomial subtraction" (:41): whatever the
+    basis used, fit-and-subtract of degree p is I - P with P the orthogonal projector onto the
+    polynomials of degree <= p sampled on the line: it maps every such polynomial to zero, is
+    idempotent and symmetric.  None of this uses the oracle's own Vandermonde matrix."""
+    shape = (37, 53)
+    n = shape[axis]
+    s = np.arange(n, dtype=np.float64)
+    for order in (0, 1, 3, 5):
+        poly = sum(RNG.standard_normal() * (s / n - 0.3) ** d for d in range(order + 1))
+        z = np.moveaxis(np.broadcast_to(poly, (shape[1 - axis], n)).copy() * RNG.standard_normal((shape[1 - axis], 1)), -1, axis)
+        assert np.abs(oracle.polyfilter(z, order, axis)).max() < 1e-9 * np.abs(z).max()
+        y, w = RNG.standard_normal(shape), RNG.standard_normal(shape)
+        Fy = oracle.polyfilter(y, order, axis)
+        assert np.abs(oracle.polyfilter(Fy, order, axis) - Fy).max() < 1e-11              # F F = F
+        assert abs(np.vdot(Fy, w) - np.vdot(y, oracle.polyfilter(w, order, axis))) < 1e-10  # F^T = F
+        # a polynomial of degree order + 1 is NOT annihilated (the degree is what it says)
+        assert np.abs(oracle.polyfilter(np.moveaxis(np.broadcast_to(s ** (order + 1), (shape[1 - axis], n)), -1, axis),
+                                        order, axis)).max() > 1e-3
+
+
+def test_filter_closed_forms_and_library_fit():
+    """order 0 = subtract the mean; order 1 = subtract the regression line with slope
+    cov(s,z)/var(s) (textbook closed forms); any order = the residual of numpy's own
+    polynomial least-squares routine (a different algorithm: QR/SVD on a scaled basis)."""
+    y = RNG.standard_normal((9, 41))
+    assert np.abs(oracle.polyfilter(y, 0) - (y - y.mean(axis=1, keepdims=True))).max() < 1e-12
+    s = np.arange(41.0)
+    sc = s - s.mean()
+    slope = (y * sc).sum(axis=1, keepdims=True) / (sc * sc).sum()
+    assert np.abs(oracle.polyfilter(y, 1) - (y - y.mean(axis=1, keepdims=True) - slope * sc)).max() < 1e-12
+    for order in (2, 3, 4):
+        c = np.polynomial.polynomial.polyfit(s, y.T, order)             # (order+1, 9)
+        fit = np.polynomial.polynomial.polyval(s, c)                     # (9, 41)
+        assert np.abs(oracle.polyfilter(y, order) - (y - fit)).max() < 1e-10
+        assert np.abs(oracle.polyfilter(y.T, order, axis=0) - (y - fit).T).max() < 1e-10
+
+
+def test_filter_leaves_fast_oscillations_alone():
+    """The filter removes slowly varying background only: the alternating sequence (-1)^s has
+    inner product at most ~sqrt((2d+1)/n) with the unit-norm degree-d polynomial (it only
+    sees the polynomial's variation over one sample), so ||z - F z|| <= (p+1) ||z|| / sqrt(n)."""
+    for n in (91, 725, 2048):
+        z = ((-1.0) ** np.arange(n))[None, :]
+        d = oracle.polyfilter(z, 3) - z
+        assert np.linalg.norm(d) / np.linalg.norm(z) < 4.0 / np.sqrt(n)
+
+
+def test_soft_threshold_and_ista_step_follow_their_definitions():
+    """S_tau is the proximal map of tau |.|: it minimises (1/2)(u - v)^2 + tau |u| (checked by
+    brute force on a fine grid); one ISTA step on the dense matrix of config-0-sized operator equals
+    the same formula written with explicit matrices (A from the closed form D_n, pin C7)."""
+    v = np.array([-2.0, -0.3, 0.0, 0.2, 1.7]); tau = 0.5
+    u = np.linspace(-3, 3, 60001)
+    brute = np.array([u[np.argmin(0.5 * (u - vi) ** 2 + tau * np.abs(u))] for vi in v])
+    assert np.abs(oracle.soft_threshold(v, tau) - brute).max() < 2e-4
+    N, n_angles, n_det = 8, 5, 9
+    th = np.pi * np.arange(n_angles) / n_angles
+    X = (np.arange(N) - N // 2)[None, :].repeat(N, 0).ravel(); Y = (np.arange(N) - N // 2)[:, None].repeat(N, 1).ravel()
+    t = np.arange(n_det) - n_det // 2
+    A = np.stack([dirichlet_np(t[k % n_det] - (X * np.cos(th[k // n_det]) + Y * np.sin(th[k // n_det])), n_det)
+                  for k in range(n_angles * n_det)])
+    x = RNG.standard_normal((N, N)); b = RNG.standard_normal((n_angles, n_det)); alpha, tau = 0.01, 0.05
+    fwd = lambda u: oracle.forward(u, n_angles, n_det)
+    adj = lambda y: oracle.adjoint(y, N)
+    got = oracle.ista_step(x, b, alpha, tau, fwd, adj)
+    g = A.T @ (A @ x.ravel() - b.ravel())
+    w = x.ravel() - alpha * g
+    ref = np.sign(w) * np.maximum(np.abs(w) - tau, 0)
+    assert np.abs(got.ravel() - ref).max() < 1e-12
+    # with the filter: gradient of (1/2)||F(Ax - b)||^2 by central differences
+    got_f = oracle.ista_step(x, b, alpha, 0.0, fwd, adj, order=3)
+    f = lambda u: 0.5 * np.sum(oracle.polyfilter((A @ u).reshape(n_angles, n_det) - b, 3) ** 2)
+    e = np.zeros(N * N); grad = np.zeros(N * N)
+    for i in range(N * N):
+        e[:] = 0; e[i] = 1e-5
+        grad[i] = (f(x.ravel() + e) - f(x.ravel() - e)) / 2e-5
+    assert np.abs(got_f.ravel() - (x.ravel() - alpha * grad)).max() < 1e-8
