@@ -53,8 +53,11 @@ def stage_bytes(N, G, M, n_angles, W=6):
     }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 4, from the ncu --set full
-# captures summarised in profiles/r01d_end_of_round1_kernels.md (A2 = scatter + merge + dc).
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 4: NOT measured by this run
+# (ncu cannot run inside it) but copied from the ncu --set full capture named below, one slice at a
+# time.  Values below the algorithmic bytes mean that part of a stage's output was still in the
+# 126 MB L2 when the kernel ended (one-slice capture: the grid written by A2 is read by A3 from L2).
+NCU_TRAFFIC_SOURCE = "profiles/r02_kernels.md (ncu --set full, one slice at a time; copied, not measured by this run)"
 NCU_DRAM_BYTES = {
     "F1_colfft": 16.99e6, "F2_rowfft": 45.03e6, "F3_gather": 69.34e6, "F4_proj_ifft": 8.59e6,
     "A1_proj_fft": 8.46e6, "A2_scatter": 47.15e6, "A3_rowifft": 71.55e6, "A4_colifft": 33.73e6,
@@ -168,13 +171,26 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value * args.slices,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "slices_per_step": args.slices, "kind": "cpu oracle, extrapolated"},
+        "config": {"workload": WORKLOAD, "slices_per_step_per_gpu": args.slices, "kind": "cpu oracle, extrapolated"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gpu_launches": 0,
+        "gpu_launches": 0, "gpus_used": 0,
     }
     print(json.dumps(line))
     return 0
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start N ranks on this node (the
+    driver's own launch line) and hand over to them."""
+    import socket
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -193,6 +209,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
 
     import numpy as np
     import torch
@@ -209,7 +227,10 @@ def main():
     dev = torch.device("cuda", local_rank)
     cfg = workloads.get_config(4)
     B = args.slices
+    t_plan = time.perf_counter()
     plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    torch.cuda.synchronize()
+    plan_create_ms = (time.perf_counter() - t_plan) * 1e3
 
     # synthetic slices (configs[4] recipe), distinct per rank; resident in HBM before timing
     n_unique = min(B, 8)
@@ -307,7 +328,8 @@ def main():
     if dom:
         ach = per_stage[dom]["GBps"]
         roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                    "frac": round(ach / peak, 4), "traffic": traffic, "peak_source": peak_src,
+                    "frac": round(ach / peak, 4), "traffic": traffic, "traffic_source": NCU_TRAFFIC_SOURCE,
+                    "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": sbytes[dom],
                     "us_per_launch": per_stage[dom]["us_per_launch"]}
 
@@ -382,9 +404,10 @@ def main():
     next_rows = {"radon_inverse_us_per_call": round(e0.elapsed_time(e1) / 20 * 1e3, 1),
                  "note": "A1 with density weights (PAPER.md:89) + A2-A4; one slice at a time"}
 
-    # ---- SURVEY 8(f) item 3 / BASELINE.json configs[2]: the operator pair inside a solver loop
-    #      (iterative soft-thresholding: x <- S_tau(x - alpha A^T (A x - b)));
-    #      the vector updates are torch elementwise ops, the two operator calls are this library ----
+    # ---- SURVEY 8(f) items 3-4 / BASELINE.json configs[2]: the solver iteration
+    #      x <- S_tau(x - alpha A^T F (A x - b)) inside the library:
+    #      radon_solver_run = one iteration (8 kernels, residual / filter / update fused into the
+    #      epilogues) captured as a CUDA graph and launched n times; F = the polynomial sinogram filter ----
     c3 = workloads.get_config(3)
     p3 = rb.RadonPlan(c3.N, c3.n_angles, c3.n_det)
     xt3 = torch.from_numpy(workloads.make_image(3)).float().to(dev)
@@ -395,27 +418,42 @@ def main():
         lam = float(w3.norm() / v3.norm())
         v3 = w3 / w3.norm()
     alpha, tau = 1.0 / lam, 1e-4
-    x3 = torch.zeros_like(xt3); r3 = torch.empty_like(b3); g3 = torch.empty_like(xt3)
-
-    def ista(n_it):
-        nonlocal x3
-        for _ in range(n_it):
-            p3.radon_forward(x3, r3)
-            r3.sub_(b3)
-            p3.radon_adjoint(r3, g3)
-            x3 = torch.nn.functional.softshrink(x3 - alpha * g3, tau)
-
-    ista(10)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    ista(100)                                              # 200 alternating operator calls
-    e1.record(stream)
-    torch.cuda.synchronize()
-    res = float((p3.radon_forward(x3) - b3).norm() / b3.norm())
-    next_rows["solver_loop_config3"] = {"iterations_per_s": round(100 / (e0.elapsed_time(e1) * 1e-3), 1),
-                                        "operator_calls": 200, "relative_residual_after_110": round(res, 4),
-                                        "note": "ISTA on configs[2] (1024^2, 64 x 1449); latency bound at this size"}
+    solver = {}
+    for label, filtered in (("plain", False), ("filtered_order3", True)):
+        x3 = torch.zeros_like(xt3)
+        p3.radon_solver_run(x3, b3, alpha, tau, 10, filtered)
+        n0 = rb.kernel_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        p3.radon_solver_run(x3, b3, alpha, tau, 100, filtered)     # 200 alternating operator calls
+        e1.record(stream)
+        torch.cuda.synchronize()
+        r = p3.radon_forward(x3) - b3
+        solver[label] = {"iterations_per_s": round(100 / (e0.elapsed_time(e1) * 1e-3), 1),
+                         "us_per_iteration": round(e0.elapsed_time(e1) * 10, 1),
+                         "library_kernels_in_loop": int(rb.kernel_launch_count() - n0),
+                         "relative_residual_after_110": round(float(r.norm() / b3.norm()), 4)}
+    next_rows["solver_loop_config3"] = {**solver["plain"], "operator_calls": 200, "filtered": solver["filtered_order3"],
+                                        "note": "radon_solver_run on configs[2] (1024^2, 64 x 1449): graph-captured "
+                                                "iteration, no kernel outside the library; latency bound at this size"}
     del p3
+    # filter(Radon{x}) against Radon{x} at config 4 (the filter runs in the epilogue of the F4 kernel)
+    xf, sf = x[0], sino[0]
+    ft = {}
+    for label, fn in (("radon_forward", lambda: plan.radon_forward(xf, sf)),
+                      ("radon_forward_filtered", lambda: plan.radon_forward_filtered(xf, sf)),
+                      ("radon_filter_axis0", lambda: plan.radon_filter(sf, out=sino[1], axis=0)),
+                      ("radon_filter_axis1", lambda: plan.radon_filter(sf, out=sino[1], axis=1))):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(20):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ft[label] = round(e0.elapsed_time(e1) / 20 * 1e3, 1)
+    next_rows["sinogram_filter_us_per_call_config4"] = ft
 
     if rank != 0:
         return 0
@@ -434,6 +472,10 @@ def main():
                    "l2": f"inputs {B * cfg.N * cfg.N * 4 / 1e6:.0f} MB/step cycle through HBM (> 126 MB L2); per-slice grid 134 MB > L2"},
         "samples_per_s": 2.0 * cfg.M * value, "us_per_pair": t_pair_us,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "plan": {"plan_create_ms": round(plan_create_ms, 1), "plan_device_bytes": int(plan.workspace_bytes),
+                 "plan_device_bytes_after_run": int(plan.device_bytes()),
+                 "note": "radon_plan_create: tables + host-built schedules + first workspace; the batched calls "
+                         "add three more workspaces on first use"},
         "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "paper_shape": paper_shape, "next_rows": next_rows,
         "cpu_baseline": cpu_baseline,
     }

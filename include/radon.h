@@ -166,6 +166,44 @@ int radon_plan_density(radon_plan *p, float *h_density, double *scale);
 /* The same table without a plan or a GPU (host only; used by the CPU tests). */
 int radon_density_host(int N, int n_angles, int n_det, float sigma, int W, float *h_density, double *scale);
 
+/* ---- the sinogram filter of the paper's objective and the solver iteration -------------------
+ * "we employed a 3rd order polynomial fit to smooth the sinogram and reduce the ringing
+ * artifacts"; the reconstruction solves min ||x||_1 subject to
+ * ||filter(Radon{x} - data)||_2 < eps, "filter is a polynomial interpolation operator"
+ * (PAPER.md:31, :47), applied as "polynomial subtraction".  Reading R-filter
+ * (DESIGN.md section 4): along one axis of the sinogram the least-squares polynomial of degree
+ * `order` is subtracted; the operator is an orthogonal projector (symmetric, idempotent).
+ *
+ * radon_plan_set_filter: order 0..7 (default 3, used when a filtered call comes first); builds the
+ * orthonormal discrete polynomial bases (fp64 on the host) and uploads them; synchronises the
+ * device.  EINVAL: order outside [0, 7]. */
+int radon_plan_set_filter(radon_plan *p, int order);
+/* d_out = filter(d_in), both n_angles*n_det fp32 (device; d_out may equal d_in).
+ * axis 0: along the detector coordinate of every projection (the exposure-to-exposure
+ * fluctuation of the illuminating beam); axis 1: along the angle coordinate of every
+ * detector bin.  Asynchronous on `stream`.  EINVAL: null pointer, axis not 0 or 1. */
+int radon_filter(radon_plan *p, const float *d_in, float *d_out, int axis, void *stream);
+/* filter(Radon{x}) and Radon^T{filter(y)}, filter along the projections (axis 0): for orders up to
+ * 3 the filter runs inside the projection DFT kernels (no extra pass over the sinogram). */
+int radon_forward_filtered(radon_plan *p, const float *d_x, float *d_sino, void *stream);
+int radon_adjoint_filtered(radon_plan *p, const float *d_sino, float *d_x, void *stream);
+/* Host only, no GPU: the basis the kernels use, h_q[s*(order+1) + d] = q_d(s), s < n. */
+int radon_filter_basis_host(int n, int order, float *h_q);
+
+/* One iteration of iterative soft-thresholding on the paper's objective (the
+ * solver "requires us to provide a function to perform y = Radon{x}" every iteration):
+ *   x <- S_tau( x - alpha * Radon^T{ F( Radon{x} - b ) } ),  S_tau(v) = sign(v) max(|v| - tau, 0),
+ * F = the sinogram filter along the projections (filtered != 0) or the identity.  d_x: N*N fp32,
+ * read and overwritten in place; d_b: the data, n_angles*n_det fp32.  Eight kernel launches: the
+ * residual and the filter run in the epilogue of the projection inverse DFT, the update and the
+ * shrinkage in the epilogue of the last inverse FFT pass.  EINVAL: null pointer, tau < 0. */
+int radon_solver_step(radon_plan *p, float *d_x, const float *d_b, float alpha, float tau, int filtered,
+                      void *stream);
+/* n_iter such iterations; one iteration is captured into a CUDA graph inside the library (again
+ * whenever an argument changes) and launched n_iter times on `stream`. */
+int radon_solver_run(radon_plan *p, float *d_x, const float *d_b, float alpha, float tau, int filtered,
+                     int n_iter, void *stream);
+
 /* A plan holds two schedule sets.  half = 0: every polar sample and the whole grid (arbitrary
  * complex data: radon_nufft2/1, radon_interp_only, radon_grid_only).  half = 1: the Hermitian
  * half used by radon_forward / radon_adjoint, whose image and sinogram are real: the polar

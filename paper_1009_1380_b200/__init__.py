@@ -15,8 +15,10 @@ from .binding import (
     schedule_host_stats,
     kb_weights_host,
     density_host,
+    filter_basis_host,
     EXPORTED_SYMBOLS,
 )
 
 __all__ = ["RadonError", "RadonPlan", "lib", "lib_path", "kernel_launch_count",
-           "schedule_selfcheck", "schedule_host_stats", "kb_weights_host", "density_host", "EXPORTED_SYMBOLS"]
+           "schedule_selfcheck", "schedule_host_stats", "kb_weights_host", "density_host", "filter_basis_host",
+           "EXPORTED_SYMBOLS"]

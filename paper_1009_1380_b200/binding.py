@@ -36,6 +36,13 @@ _SIGNATURES = {
     "radon_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_plan_density": (c_int, [c_void_p, c_void_p, P(ctypes.c_double)]),
     "radon_density_host": (c_int, [c_int, c_int, c_int, c_float, c_int, c_void_p, P(ctypes.c_double)]),
+    "radon_plan_set_filter": (c_int, [c_void_p, c_int]),
+    "radon_filter": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "radon_forward_filtered": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_adjoint_filtered": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_filter_basis_host": (c_int, [c_int, c_int, c_void_p]),
+    "radon_solver_step": (c_int, [c_void_p, c_void_p, c_void_p, c_float, c_float, c_int, c_void_p]),
+    "radon_solver_run": (c_int, [c_void_p, c_void_p, c_void_p, c_float, c_float, c_int, c_int, c_void_p]),
     "radon_kernel_launch_count": (c_ll, []),
     "radon_strerror": (ctypes.c_char_p, [c_int]),
     "radon_last_cuda_error": (ctypes.c_char_p, []),
@@ -87,6 +94,15 @@ def density_host(N, n_angles, n_det, sigma=2.0, W=6):
     _check(lib().radon_density_host(N, n_angles, n_det, sigma, W, out.ctypes.data_as(c_void_p), ctypes.byref(sc)),
            "radon_density_host")
     return out, float(sc.value)
+
+
+def filter_basis_host(n, order):
+    """Host-only: the orthonormal discrete polynomial basis of the sinogram filter, (n, order+1) float32."""
+    import numpy as np
+
+    q = np.empty((n, order + 1), dtype=np.float32)
+    _check(lib().radon_filter_basis_host(n, order, q.ctypes.data_as(c_void_p)), "radon_filter_basis_host")
+    return q
 
 
 def kernel_launch_count() -> int:
@@ -166,6 +182,12 @@ class RadonPlan:
 
         return torch.empty(shape, dtype=dtype, device="cuda")
 
+    def device_bytes(self) -> int:
+        """Device bytes the plan owns now (workspaces of the batched / host calls are allocated on first use)."""
+        wb = c_size_t()
+        _check(lib().radon_plan_info(self._h, None, None, None, None, None, wb), "radon_plan_info")
+        return int(wb.value)
+
     def schedule_stats(self, half=False):
         v = [c_ll(), c_ll(), c_int(), c_ll(), c_ll(), c_int()]
         _check(lib().radon_plan_schedule_stats(self._h, int(half), *v), "radon_plan_schedule_stats")
@@ -210,6 +232,55 @@ class RadonPlan:
         x = self._new((self.N, self.N), torch.float32) if x is None else x
         self._chk(x, torch.float32, self.N * self.N, "x")
         _check(lib().radon_inverse(self._h, _ptr(sino), _ptr(x), self._stream()), "radon_inverse")
+        return x
+
+    def set_filter(self, order: int):
+        _check(lib().radon_plan_set_filter(self._h, int(order)), "radon_plan_set_filter")
+
+    def radon_filter(self, sino, out=None, axis=0):
+        import torch
+
+        self._chk(sino, torch.float32, self.M, "sino")
+        out = self._new((self.n_angles, self.n_det), torch.float32) if out is None else out
+        self._chk(out, torch.float32, self.M, "out")
+        _check(lib().radon_filter(self._h, _ptr(sino), _ptr(out), int(axis), self._stream()), "radon_filter")
+        return out
+
+    def radon_forward_filtered(self, x, sino=None):
+        import torch
+
+        self._chk(x, torch.float32, self.N * self.N, "x")
+        sino = self._new((self.n_angles, self.n_det), torch.float32) if sino is None else sino
+        self._chk(sino, torch.float32, self.M, "sino")
+        _check(lib().radon_forward_filtered(self._h, _ptr(x), _ptr(sino), self._stream()), "radon_forward_filtered")
+        return sino
+
+    def radon_adjoint_filtered(self, sino, x=None):
+        import torch
+
+        self._chk(sino, torch.float32, self.M, "sino")
+        x = self._new((self.N, self.N), torch.float32) if x is None else x
+        self._chk(x, torch.float32, self.N * self.N, "x")
+        _check(lib().radon_adjoint_filtered(self._h, _ptr(sino), _ptr(x), self._stream()), "radon_adjoint_filtered")
+        return x
+
+    def radon_solver_step(self, x, b, alpha, tau, filtered=False):
+        """x <- S_tau(x - alpha A^T F (A x - b)) in place."""
+        import torch
+
+        self._chk(x, torch.float32, self.N * self.N, "x")
+        self._chk(b, torch.float32, self.M, "b")
+        _check(lib().radon_solver_step(self._h, _ptr(x), _ptr(b), float(alpha), float(tau), int(filtered), self._stream()),
+               "radon_solver_step")
+        return x
+
+    def radon_solver_run(self, x, b, alpha, tau, n_iter, filtered=False):
+        import torch
+
+        self._chk(x, torch.float32, self.N * self.N, "x")
+        self._chk(b, torch.float32, self.M, "b")
+        _check(lib().radon_solver_run(self._h, _ptr(x), _ptr(b), float(alpha), float(tau), int(filtered), int(n_iter),
+                                      self._stream()), "radon_solver_run")
         return x
 
     def density(self):

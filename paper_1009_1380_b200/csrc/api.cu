@@ -63,6 +63,20 @@ struct radon_plan {
     float *dev_density = nullptr;   // D of PAPER.md:89 times the quadrature scale, pair-symmetrised (density_setup)
     std::vector<float> host_density;   // the same table exactly as eq. :89 gives it (radon_plan_density)
     double density_scale = 0.0;
+    // polynomial sinogram filter: orthonormal bases along the detector (n_det)
+    // and along the angles (n_angles), built on first use or by radon_plan_set_filter
+    int filter_order = -1;
+    float *filter_q[2] = {nullptr, nullptr};
+    // solver iteration: residual sinogram, and the iteration captured as a CUDA graph
+    float *resid = nullptr;
+    struct SolverGraph {
+        cudaGraphExec_t exec = nullptr;
+        const float *x = nullptr, *b = nullptr;
+        float alpha = 0.f, tau = 0.f;
+        int filtered = 0;
+        long long kernels = 0;            // kernel nodes of one iteration
+    } sgraph;
+    cudaStream_t capture_stream = nullptr;
 };
 
 template <typename T>
@@ -123,6 +137,9 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     for (cudaEvent_t e : p->timer.ev) cudaEventDestroy(e);
     if (p->fork_event) cudaEventDestroy(p->fork_event);
     cudaFree(p->dev_density);
+    cudaFree(p->filter_q[0]); cudaFree(p->filter_q[1]); cudaFree(p->resid);
+    if (p->sgraph.exec) cudaGraphExecDestroy(p->sgraph.exec);
+    if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     for (int i = 0; i < NWS; ++i) {
         if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
         if (p->hevent[i]) cudaEventDestroy(p->hevent[i]);
@@ -280,23 +297,26 @@ static int nufft2_ws(radon_plan *p, Workspace &w, bool half, const float *d_x, f
 
 // half: d_polar is Hermitian along every row (the DFT of a real sinogram); only the grid rows
 // ky = 0 .. G/2 are gridded and the row pass reads them without folding.
-static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st)
+static int nufft1_ws(radon_plan *p, Workspace &w, bool half, const float2 *d_polar, float *d_x, cudaStream_t st,
+                     const IstaUpdate *upd = nullptr)
 {
     mark(p, st, 5);
     if (launch_scatter(p->dev, half, d_polar, w.grid, w.scratch, w.dcbuf, w.tickets, st)) return RADON_ECUDA;             // A2
     mark(p, st, 6);
     if (launch_fft2d_pass(2, p->dev, w.grid, w.T, half ? 0 : 1, st)) return RADON_ECUDA;   // A3 (rows)
     mark(p, st, 7);
-    if (launch_fft2d_pass(3, p->dev, w.T, d_x, 0, st)) return RADON_ECUDA;        // A3 (columns) + A4
+    if (launch_fft2d_pass(3, p->dev, w.T, d_x, 0, st, upd)) return RADON_ECUDA;   // A3 (columns) + A4 (+ solver update)
     return check_launch();
 }
 
-static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_sino, cudaStream_t st)
+// ex.sub: the data, subtracted from the sinogram (residual); ex.q: filter basis (filter along the projections)
+static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_sino, cudaStream_t st,
+                      const ProjExtra &ex = ProjExtra())
 {
     int rc = nufft2_ws(p, w, true, d_x, w.polar, st);
     if (rc) return rc;
     mark(p, st, 3);
-    if (launch_proj(true, true, p->dev, (const float *)w.polar, d_sino, nullptr, st)) return RADON_ECUDA;   // F4
+    if (launch_proj(true, true, p->dev, (const float *)w.polar, d_sino, nullptr, st, ex)) return RADON_ECUDA;   // F4
     mark(p, st, -1);
     return check_launch();
 }
@@ -304,13 +324,15 @@ static int forward_ws(radon_plan *p, Workspace &w, const float *d_x, float *d_si
 // dens == nullptr: the exact transpose of forward_ws (D == 1, reading S11); else the inverse
 // Radon transform of PAPER.md:51 / :85 with the density compensation D of :89
 static int adjoint_ws(radon_plan *p, Workspace &w, const float *d_sino, float *d_x, cudaStream_t st,
-                      const float *dens = nullptr)
+                      const float *dens = nullptr, const float *filter_q = nullptr, const IstaUpdate *upd = nullptr)
 {
     mark(p, st, 4);
-    if (launch_proj(false, false, p->dev, d_sino, (float *)w.polar, dens, st)) return RADON_ECUDA;  // A1
+    ProjExtra ex;
+    ex.q = filter_q;
+    if (launch_proj(false, false, p->dev, d_sino, (float *)w.polar, dens, st, ex)) return RADON_ECUDA;  // A1
     int rc = check_launch();
     if (rc) return rc;
-    rc = nufft1_ws(p, w, true, w.polar, d_x, st);
+    rc = nufft1_ws(p, w, true, w.polar, d_x, st, upd);
     mark(p, st, -1);
     return rc;
 }
@@ -425,6 +447,165 @@ extern "C" int radon_density_host(int N, int n_angles, int n_det, float sigma, i
     } catch (...) {
         return RADON_ENOMEM;
     }
+    return RADON_OK;
+}
+
+// ---- polynomial sinogram filter and the solver iteration -------------
+static int filter_setup(radon_plan *p, int order)
+{
+    if (order < 0 || order >= FILTER_MAXQ) return RADON_EINVAL;
+    if (p->filter_order == order && p->filter_q[0] && p->filter_q[1]) return RADON_OK;
+    CUDA_TRY(cudaDeviceSynchronize());                    // kernels in flight may still read the old tables
+    cudaFree(p->filter_q[0]); cudaFree(p->filter_q[1]);
+    p->filter_q[0] = p->filter_q[1] = nullptr;
+    p->filter_order = -1;
+    if (p->sgraph.exec) { cudaGraphExecDestroy(p->sgraph.exec); p->sgraph.exec = nullptr; }
+    std::vector<float> q;
+    int rc;
+    try {
+        build_filter_basis(p->dev.n_det, order, q);
+        if ((rc = dev_upload(p, &p->filter_q[0], q))) return rc;
+        build_filter_basis(p->dev.n_angles, order, q);
+        if ((rc = dev_upload(p, &p->filter_q[1], q))) return rc;
+    } catch (const std::bad_alloc &) {
+        return RADON_ENOMEM;
+    }
+    p->filter_order = order;
+    return RADON_OK;
+}
+
+extern "C" int radon_plan_set_filter(radon_plan *p, int order)
+{
+    if (!p) return RADON_EINVAL;
+    return filter_setup(p, order);
+}
+
+extern "C" int radon_filter_basis_host(int n, int order, float *h_q)
+{
+    if (!h_q || n < 1 || order < 0 || order >= FILTER_MAXQ) return RADON_EINVAL;
+    try {
+        std::vector<float> q;
+        build_filter_basis(n, order, q);
+        for (int s = 0; s < n; ++s)
+            for (int d = 0; d <= order; ++d) h_q[(size_t)s * (order + 1) + d] = q[(size_t)s * FILTER_MAXQ + d];
+    } catch (...) {
+        return RADON_ENOMEM;
+    }
+    return RADON_OK;
+}
+
+static int filter_ready(radon_plan *p) { return p->filter_order >= 0 ? RADON_OK : filter_setup(p, 3); }
+
+extern "C" int radon_filter(radon_plan *p, const float *d_in, float *d_out, int axis, void *stream)
+{
+    if (!p || !d_in || !d_out || (axis != 0 && axis != 1)) return RADON_EINVAL;
+    int rc = filter_ready(p);
+    if (rc) return rc;
+    if (launch_filter(p->dev, axis, p->filter_q[axis], d_in, d_out, (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+// orders 0..3 run inside the projection DFT kernels; higher orders as a separate pass
+extern "C" int radon_forward_filtered(radon_plan *p, const float *d_x, float *d_sino, void *stream)
+{
+    if (!p || !d_x || !d_sino) return RADON_EINVAL;
+    int rc = filter_ready(p);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    ProjExtra ex;
+    if (p->filter_order < FILTER_FUSED_Q) ex.q = p->filter_q[0];
+    if ((rc = forward_ws(p, p->ws[0], d_x, d_sino, st, ex))) return rc;
+    if (!ex.q && launch_filter(p->dev, 0, p->filter_q[0], d_sino, d_sino, st)) return RADON_ECUDA;
+    return check_launch();
+}
+
+static int resid_ready(radon_plan *p)
+{
+    return p->resid ? RADON_OK : dev_alloc(p, &p->resid, (size_t)p->M);
+}
+
+extern "C" int radon_adjoint_filtered(radon_plan *p, const float *d_sino, float *d_x, void *stream)
+{
+    if (!p || !d_x || !d_sino) return RADON_EINVAL;
+    int rc = filter_ready(p);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->filter_order < FILTER_FUSED_Q) return adjoint_ws(p, p->ws[0], d_sino, d_x, st, nullptr, p->filter_q[0]);
+    if ((rc = resid_ready(p))) return rc;
+    if (launch_filter(p->dev, 0, p->filter_q[0], d_sino, p->resid, st)) return RADON_ECUDA;
+    return adjoint_ws(p, p->ws[0], p->resid, d_x, st);
+}
+
+// One iteration x <- S_tau(x - alpha Radon^T F (Radon x - b)), F the sinogram filter (filtered != 0)
+// or the identity: the residual and the filter run in the epilogue of F4, the update and the
+// shrinkage in the epilogue of A4; eight launches, no other kernels.
+static int solver_step_on(radon_plan *p, float *d_x, const float *d_b, float alpha, float tau, int filtered, cudaStream_t st)
+{
+    ProjExtra ex;
+    ex.sub = d_b;
+    const bool fused = filtered && p->filter_order < FILTER_FUSED_Q;
+    if (fused) ex.q = p->filter_q[0];
+    int rc = forward_ws(p, p->ws[0], d_x, p->resid, st, ex);
+    if (rc) return rc;
+    if (filtered && !fused && launch_filter(p->dev, 0, p->filter_q[0], p->resid, p->resid, st)) return RADON_ECUDA;
+    IstaUpdate upd;
+    upd.alpha = alpha; upd.tau = tau;
+    return adjoint_ws(p, p->ws[0], p->resid, d_x, st, nullptr, nullptr, &upd);
+}
+
+extern "C" int radon_solver_step(radon_plan *p, float *d_x, const float *d_b, float alpha, float tau, int filtered, void *stream)
+{
+    if (!p || !d_x || !d_b || !(tau >= 0.f)) return RADON_EINVAL;
+    int rc = resid_ready(p);
+    if (rc) return rc;
+    if (filtered && (rc = filter_ready(p))) return rc;
+    return solver_step_on(p, d_x, d_b, alpha, tau, filtered, (cudaStream_t)stream);
+}
+
+// n_iter iterations: one iteration is captured once into a CUDA graph (on an internal stream: the
+// caller's may be the legacy default stream, which cannot capture) and the graph is launched
+// n_iter times on the caller's stream; it is re-captured when x, b, alpha, tau or the filter change.
+extern "C" int radon_solver_run(radon_plan *p, float *d_x, const float *d_b, float alpha, float tau, int filtered,
+                                int n_iter, void *stream)
+{
+    if (!p || !d_x || !d_b || !(tau >= 0.f) || n_iter < 0) return RADON_EINVAL;
+    int rc = resid_ready(p);
+    if (rc) return rc;
+    if (filtered && (rc = filter_ready(p))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->timer.enabled) {                               // stage events are not captured: run the plain calls
+        for (int i = 0; i < n_iter && rc == RADON_OK; ++i) rc = solver_step_on(p, d_x, d_b, alpha, tau, filtered, st);
+        return rc;
+    }
+    radon_plan::SolverGraph &g = p->sgraph;
+    if (!g.exec || g.x != d_x || g.b != d_b || g.alpha != alpha || g.tau != tau || g.filtered != filtered) {
+        if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+        if (!p->capture_stream) CUDA_TRY(cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal));
+        const long long n0 = launch_count();
+        rc = solver_step_on(p, d_x, d_b, alpha, tau, filtered, p->capture_stream);
+        g.kernels = launch_count() - n0;
+        count_launch(-g.kernels);                       // captured, not launched
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamEndCapture(p->capture_stream, &graph);
+        if (rc == RADON_OK && e != cudaSuccess) {
+            g_last_cuda_error = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e);
+            rc = RADON_ECUDA;
+        }
+        if (rc == RADON_OK) {
+            e = cudaGraphInstantiate(&g.exec, graph, 0);
+            if (e != cudaSuccess) {
+                g_last_cuda_error = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e);
+                rc = RADON_ECUDA;
+                g.exec = nullptr;
+            }
+        }
+        if (graph) cudaGraphDestroy(graph);
+        if (rc) return rc;
+        g.x = d_x; g.b = d_b; g.alpha = alpha; g.tau = tau; g.filtered = filtered;
+    }
+    for (int i = 0; i < n_iter; ++i) CUDA_TRY(cudaGraphLaunch(g.exec, st));
+    count_launch(g.kernels * n_iter);
     return RADON_OK;
 }
 

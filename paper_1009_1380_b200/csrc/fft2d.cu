@@ -282,7 +282,7 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
 template <int L>
 __global__ void __launch_bounds__(ColCfg<L>::THREADS)
 colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapod,
-                   float *__restrict__ x, const float2 *__restrict__ tw, int N)
+                   float *x, const float2 *__restrict__ tw, int N, int update, float alpha, float tau)
 {
     extern __shared__ __align__(16) float2 s_fft[];
     using C = ColCfg<L>;
@@ -338,8 +338,19 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
             const float dy = __ldg(&deapod[iy]);
             const float2 z = sf[FFT_PAD((iy - c) & (L - 1))];
             float *row = x + (size_t)iy * N + ixc;
-            if (even) *reinterpret_cast<float2 *>(row) = make_float2(z.x * da * dy, z.y * db * dy);
-            else { row[0] = z.x * da * dy; if (has_b) row[1] = z.y * db * dy; }
+            float ga = z.x * da * dy, gb = z.y * db * dy;
+            if (update) {
+                // solver iteration: x <- S_tau(x - alpha g), g = Radon^T{residual}
+                // just computed; the thread that writes a pixel is the one that reads it
+                float xa, xb = 0.f;
+                if (even) { const float2 xo = *reinterpret_cast<const float2 *>(row); xa = xo.x; xb = xo.y; }
+                else { xa = row[0]; if (has_b) xb = row[1]; }
+                const float va = fmaf(-alpha, ga, xa), vb = fmaf(-alpha, gb, xb);
+                ga = copysignf(fmaxf(fabsf(va) - tau, 0.f), va);
+                gb = copysignf(fmaxf(fabsf(vb) - tau, 0.f), vb);
+            }
+            if (even) *reinterpret_cast<float2 *>(row) = make_float2(ga, gb);
+            else { row[0] = ga; if (has_b) row[1] = gb; }
         }
     }
 }
@@ -348,7 +359,8 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
 bool fft_length_supported(int L) { return L >= 16 && L <= 8192 && (L & (L - 1)) == 0; }
 
 template <int L>
-static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st)
+static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
+                        const IstaUpdate *upd)
 {
     using C = FftCfg<L>;
     using CC = ColCfg<L>;
@@ -378,7 +390,8 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
         break;
     case 3:
         if (set_smem(colpass_inv_kernel<L>, CC::SMEM)) return -1;
-        colpass_inv_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N);
+        colpass_inv_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
+                                                                           upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
         break;
     default:
         return -1;
@@ -387,9 +400,10 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
     return 0;
 }
 
-int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st)
+int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
+                      const IstaUpdate *upd)
 {
-    RADON_FOR_L(p.G, return fft2d_launch<LL>(which, p, in, out, flag, st);)
+    RADON_FOR_L(p.G, return fft2d_launch<LL>(which, p, in, out, flag, st, upd);)
     return -1;
 }
 

@@ -15,7 +15,7 @@ namespace radon {
 
 static std::atomic<long long> g_launches{0};
 long long launch_count() { return g_launches.load(); }
-void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+void count_launch(long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 // =====================================================================================
 // Sample coordinates and Kaiser-Bessel weights (shared by gather and scatter so that the

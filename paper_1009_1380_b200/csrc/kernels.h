@@ -33,10 +33,13 @@ struct DevicePlan {
     } sched[2];
 };
 
+// A4 epilogue of a solver iteration: x <- S_tau(x - alpha * g) in place, g the freshly computed adjoint
+struct IstaUpdate { float alpha = 0.f, tau = 0.f; };
+
 bool fft_length_supported(int L);
 int init_kernel_attributes();
 long long launch_count();
-void count_launch();
+void count_launch(long long n = 1);
 
 // Opt a kernel in to more than 48 KB of dynamic shared memory: once per (device, kernel); the
 // attribute call costs microseconds of host time, which a batch of back-to-back launches feels.
@@ -88,10 +91,19 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
 // flag 2: only the mirrored rows the half gather reads, |ky| <= W/2 and |ky - G/2| <= W/2),
 // 2 rowpass_inv (grid -> T; flag: fold the mirrored rows in), 3 colpass_inv (T -> x).
 // T holds the rows ky = 0..G/2 only (Hermitian half), N complex each.
-int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st);
+int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
+                      const IstaUpdate *upd = nullptr);
 // inv == false: sinogram -> polar (A1); inv == true: polar -> sinogram (F4).  half (F4 only):
 // the polar rows hold k >= n/2 (and k = 0 for even n); the rest is their conjugate mirror.
 // dens (A1 only, may be null): per-sample density weights multiplied into the output (radon_inverse).
-int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st);
+// sub (F4 only, may be null): a sinogram subtracted from the result (the residual Radon{x} - data);
+// q (may be null): basis of the polynomial sinogram filter (n_det x FILTER_MAXQ, orders <= 3), applied
+// along every projection to the output (F4, after `sub`) or to the input (A1): PAPER.md:27, :31.
+struct ProjExtra { const float *sub = nullptr; const float *q = nullptr; };
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st,
+                const ProjExtra &ex = ProjExtra());
+// axis 0: along the detector coordinate of every projection; 1: along the angles of every detector bin
+int launch_filter(const DevicePlan &p, int axis, const float *q, const float *in, float *out, cudaStream_t st);
+
 
 }  // namespace radon

@@ -228,6 +228,32 @@ void build_density(const Geometry &g, std::vector<float> &D, double *scale_out)
     for (auto &th : pool) th.join();
 }
 
+void build_filter_basis(int n, int order, std::vector<float> &q)
+{
+    const int nq = std::min(order, FILTER_MAXQ - 1) + 1;
+    std::vector<std::vector<double>> b(nq, std::vector<double>((size_t)n));
+    for (int d = 0; d < nq; ++d) {
+        for (int s = 0; s < n; ++s) {
+            const double t = n > 1 ? -1.0 + 2.0 * (double)s / (double)(n - 1) : 0.0;
+            b[d][s] = std::pow(t, d);
+        }
+        for (int pass = 0; pass < 2; ++pass)                     // modified Gram-Schmidt, twice
+            for (int e = 0; e < d; ++e) {
+                double dot = 0.0;
+                for (int s = 0; s < n; ++s) dot += b[e][s] * b[d][s];
+                for (int s = 0; s < n; ++s) b[d][s] -= dot * b[e][s];
+            }
+        double nrm = 0.0;
+        for (int s = 0; s < n; ++s) nrm += b[d][s] * b[d][s];
+        nrm = std::sqrt(nrm);
+        // more basis functions than points: the remaining ones vanish (the fit is exact already)
+        for (int s = 0; s < n; ++s) b[d][s] = (nrm > 1e-12 * std::sqrt((double)n)) ? b[d][s] / nrm : 0.0;
+    }
+    q.assign((size_t)n * FILTER_MAXQ, 0.f);
+    for (int d = 0; d < nq; ++d)
+        for (int s = 0; s < n; ++s) q[(size_t)s * FILTER_MAXQ + d] = (float)b[d][s];
+}
+
 void build_twiddles(int L, std::vector<float> &tw)
 {
     tw.resize(2 * (size_t)L);

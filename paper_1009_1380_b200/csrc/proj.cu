@@ -21,18 +21,89 @@ struct ProjCfg {
     static constexpr int THREADS = NF * TF;
     static constexpr int PADLEN = fft_padded_len(L);
     static constexpr size_t SMEM = (size_t)NF * PADLEN * sizeof(float2);
-    static constexpr int MIN_CTAS = 1024 / THREADS;      // <= 64 registers per thread
+    static constexpr int MIN_CTAS = (1024 / THREADS > 2) ? 1024 / THREADS - 1 : 1024 / THREADS;   // <= 72 registers per thread
 };
 
+// Sum NV values over the TF threads that share one FFT (thread t of FFT f in the CTA); every
+// thread of the group gets the sum.  TF < 32: butterflies inside the group's lanes; otherwise
+// butterflies inside each warp, then the group's warps through s_red in warp order (fixed
+// order: bitwise reproducible).  All threads of the CTA must call it.
+template <int TF, int NV>
+__device__ __forceinline__ void group_sum(float (&v)[NV], float *s_red, int f)
+{
+    constexpr int WIDTH = TF < 32 ? TF : 32;
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+#pragma unroll
+        for (int o = WIDTH / 2; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    if constexpr (TF > 32) {
+        constexpr int WG = TF / 32;                       // warps per group
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        __syncthreads();                                  // s_red free (a previous reduction was read)
+        if (lane == 0)
+#pragma unroll
+            for (int i = 0; i < NV; ++i) s_red[warp * NV + i] = v[i];
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            float a = 0.f;
+            for (int w = 0; w < WG; ++w) a += s_red[(f * WG + w) * NV + i];
+            v[i] = a;
+        }
+    }
+}
+
+// The polynomial sinogram filter along one projection held in registers (
+// filter.cu has the stand-alone kernels): z[i] is element idx(i) = t + i*TF of the row (only
+// elements < n count), q the orthonormal basis (n x FILTER_MAXQ floats, orders <= 3 in the first
+// four columns).  NR rows at once (the pair kernels hold two projections per thread).
+template <int TF, int NR>
+__device__ __forceinline__ void filter_rows_in_registers(float (&z)[NR][16], const float *__restrict__ q, int n,
+                                                         int t, int f, float *s_red)
+{
+    float c[NR * FILTER_FUSED_Q];
+#pragma unroll
+    for (int i = 0; i < NR * FILTER_FUSED_Q; ++i) c[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int k = t + i * TF;
+        if (k < n) {
+            const float4 b = __ldg(reinterpret_cast<const float4 *>(q + (size_t)k * FILTER_MAXQ));
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                c[r * 4 + 0] = fmaf(b.x, z[r][i], c[r * 4 + 0]); c[r * 4 + 1] = fmaf(b.y, z[r][i], c[r * 4 + 1]);
+                c[r * 4 + 2] = fmaf(b.z, z[r][i], c[r * 4 + 2]); c[r * 4 + 3] = fmaf(b.w, z[r][i], c[r * 4 + 3]);
+            }
+        }
+    }
+    group_sum<TF, NR * FILTER_FUSED_Q>(c, s_red, f);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const int k = t + i * TF;
+        if (k < n) {
+            const float4 b = __ldg(reinterpret_cast<const float4 *>(q + (size_t)k * FILTER_MAXQ));
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                float fit = b.x * c[r * 4 + 0];
+                fit = fmaf(b.y, c[r * 4 + 1], fit); fit = fmaf(b.z, c[r * 4 + 2], fit); fit = fmaf(b.w, c[r * 4 + 3], fit);
+                z[r][i] -= fit;
+            }
+        }
+    }
+}
+constexpr int PROJ_RED_FLOATS = 32 * 2 * FILTER_FUSED_Q;     // up to 32 warps x 8 values
+
 // BLUE: Bluestein form (two FFTs); false: n == L is a power of two, one FFT.
-template <int L, bool INV, bool BLUE>
-__global__ void __launch_bounds__(ProjCfg<L>::THREADS, BLUE ? 1 : ProjCfg<L>::MIN_CTAS)
+// FILT: the polynomial filter along the projection, on the output (INV, after `sub`) or the input.
+template <int L, bool INV, bool BLUE, bool FILT>
+__global__ void __launch_bounds__(ProjCfg<L>::THREADS, (BLUE || FILT) ? 1 : ProjCfg<L>::MIN_CTAS)
 proj_kernel(const float *__restrict__ in, float *__restrict__ out,
             const float2 *__restrict__ ta, const float2 *__restrict__ tb,
             const float2 *__restrict__ hf, const float2 *__restrict__ tw, int n, int n_rows, int half,
-            const float *__restrict__ dens)
+            const float *__restrict__ dens, const float *__restrict__ sub, const float *__restrict__ q)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    __shared__ float s_red[FILT ? PROJ_RED_FLOATS : 1];
     using C = ProjCfg<L>;
     constexpr int TF = C::TF;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -41,22 +112,38 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
     const bool live = row < n_rows;
 
     float2 v[16];
+    if constexpr (!INV && FILT) {
+        float z[1][16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int sidx = t + i * TF;
-        v[i] = make_float2(0.f, 0.f);
-        if (live && sidx < n) {
-            const float2 a = __ldg(&ta[sidx]);
-            if (INV) {
-                // half: the row holds k >= n/2 (and k = 0 for even n); P[c - j] = conj P[c + j]
-                const int c = n >> 1;
-                const bool mir = half && sidx < c && !(sidx == 0 && (n & 1) == 0);
-                float2 p = __ldg(&reinterpret_cast<const float2 *>(in)[(size_t)row * n + (mir ? 2 * c - sidx : sidx)]);
-                if (mir) p.y = -p.y;
-                v[i] = make_float2(p.x * a.x + p.y * a.y, p.x * a.y - p.y * a.x);   // conj(p) * a
-            } else {
-                const float y = __ldg(&in[(size_t)row * n + sidx]);
-                v[i] = make_float2(y * a.x, y * a.y);
+        for (int i = 0; i < 16; ++i) {
+            const int sidx = t + i * TF;
+            z[0][i] = (live && sidx < n) ? __ldg(&in[(size_t)row * n + sidx]) : 0.f;
+        }
+        filter_rows_in_registers<TF, 1>(z, q, n, t, f, s_red);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int sidx = t + i * TF;
+            v[i] = make_float2(0.f, 0.f);
+            if (live && sidx < n) { const float2 a = __ldg(&ta[sidx]); v[i] = make_float2(z[0][i] * a.x, z[0][i] * a.y); }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int sidx = t + i * TF;
+            v[i] = make_float2(0.f, 0.f);
+            if (live && sidx < n) {
+                const float2 a = __ldg(&ta[sidx]);
+                if (INV) {
+                    // half: the row holds k >= n/2 (and k = 0 for even n); P[c - j] = conj P[c + j]
+                    const int c = n >> 1;
+                    const bool mir = half && sidx < c && !(sidx == 0 && (n & 1) == 0);
+                    float2 p = __ldg(&reinterpret_cast<const float2 *>(in)[(size_t)row * n + (mir ? 2 * c - sidx : sidx)]);
+                    if (mir) p.y = -p.y;
+                    v[i] = make_float2(p.x * a.x + p.y * a.y, p.x * a.y - p.y * a.x);   // conj(p) * a
+                } else {
+                    const float y = __ldg(&in[(size_t)row * n + sidx]);
+                    v[i] = make_float2(y * a.x, y * a.y);
+                }
             }
         }
     }
@@ -67,14 +154,31 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
         __syncthreads();
         fft_reg<L, +1>(v, s, tw, t);
     }
-    if (!live) return;
+    if constexpr (INV) {
+        float z[1][16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int k = t + i * TF;
-        if (k < n) {
-            float2 r = cmul(v[i], __ldg(&tb[k]));
-            if (INV) out[(size_t)row * n + k] = r.x;
-            else {
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            z[0][i] = 0.f;
+            if (live && k < n) {
+                z[0][i] = cmul(v[i], __ldg(&tb[k])).x;
+                if (sub != nullptr) z[0][i] -= __ldg(&sub[(size_t)row * n + k]);     // residual Radon{x} - data
+            }
+        }
+        if constexpr (FILT) filter_rows_in_registers<TF, 1>(z, q, n, t, f, s_red);
+        if (!live) return;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            if (k < n) out[(size_t)row * n + k] = z[0][i];
+        }
+    } else {
+        if (!live) return;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            if (k < n) {
+                float2 r = cmul(v[i], __ldg(&tb[k]));
                 // radon_inverse: density compensation D applied to the sample
                 if (dens != nullptr) { const float w = __ldg(&dens[(size_t)row * n + k]); r.x *= w; r.y *= w; }
                 reinterpret_cast<float2 *>(out)[(size_t)row * n + k] = r;
@@ -93,13 +197,15 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
 //       half, mirrored and conjugated; the self-mirrored k = n/2 and the unpaired k = 0 keep
 //       their real part: that is what Re{.} of the single-row form leaves of them), one FFT of
 //       conj(P0 + i P1) .* a, r = b .* result; S0 = r.x, S1 = -r.y.
-template <int L, bool INV>
-__global__ void __launch_bounds__(ProjCfg<L>::THREADS, ProjCfg<L>::MIN_CTAS)
+template <int L, bool INV, bool FILT>
+__global__ void __launch_bounds__(ProjCfg<L>::THREADS, FILT ? (ProjCfg<L>::MIN_CTAS > 1 ? ProjCfg<L>::MIN_CTAS / 2 : 1) : ProjCfg<L>::MIN_CTAS)
 proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
                  const float2 *__restrict__ ta, const float2 *__restrict__ tb,
-                 const float2 *__restrict__ tw, int n_rows, const float *__restrict__ dens)
+                 const float2 *__restrict__ tw, int n_rows, const float *__restrict__ dens,
+                 const float *__restrict__ sub, const float *__restrict__ q)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    __shared__ float s_red[FILT ? PROJ_RED_FLOATS : 1];
     using C = ProjCfg<L>;
     constexpr int TF = C::TF, n = L, c = L / 2;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -108,35 +214,63 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
     const bool live0 = r0 < n_rows, live1 = r1 < n_rows;
 
     float2 v[16];
+    if constexpr (!INV && FILT) {
+        float z[2][16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int sidx = t + i * TF;
-        const float a = __ldg(&ta[sidx]).x;
-        if (INV) {
-            const bool self = sidx == 0 || sidx == c;            // keep the real part only
-            const bool mir = sidx < c && sidx != 0;
-            const int src = mir ? 2 * c - sidx : sidx;
-            const float2 *P = reinterpret_cast<const float2 *>(in);
-            float2 p0 = live0 ? __ldg(&P[(size_t)r0 * n + src]) : make_float2(0.f, 0.f);
-            float2 p1 = live1 ? __ldg(&P[(size_t)r1 * n + src]) : make_float2(0.f, 0.f);
-            if (mir) { p0.y = -p0.y; p1.y = -p1.y; }
-            if (self) { p0.y = 0.f; p1.y = 0.f; }
-            // z = p0 + i p1; v = conj(z) * a
-            v[i] = make_float2((p0.x - p1.y) * a, -(p0.y + p1.x) * a);
-        } else {
-            const float y0 = live0 ? __ldg(&in[(size_t)r0 * n + sidx]) : 0.f;
-            const float y1 = live1 ? __ldg(&in[(size_t)r1 * n + sidx]) : 0.f;
-            v[i] = make_float2(y0 * a, y1 * a);
+        for (int i = 0; i < 16; ++i) {
+            const int sidx = t + i * TF;
+            z[0][i] = live0 ? __ldg(&in[(size_t)r0 * n + sidx]) : 0.f;
+            z[1][i] = live1 ? __ldg(&in[(size_t)r1 * n + sidx]) : 0.f;
+        }
+        filter_rows_in_registers<TF, 2>(z, q, n, t, f, s_red);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const float a = __ldg(&ta[t + i * TF]).x;
+            v[i] = make_float2(z[0][i] * a, z[1][i] * a);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int sidx = t + i * TF;
+            const float a = __ldg(&ta[sidx]).x;
+            if (INV) {
+                const bool self = sidx == 0 || sidx == c;            // keep the real part only
+                const bool mir = sidx < c && sidx != 0;
+                const int src = mir ? 2 * c - sidx : sidx;
+                const float2 *P = reinterpret_cast<const float2 *>(in);
+                float2 p0 = live0 ? __ldg(&P[(size_t)r0 * n + src]) : make_float2(0.f, 0.f);
+                float2 p1 = live1 ? __ldg(&P[(size_t)r1 * n + src]) : make_float2(0.f, 0.f);
+                if (mir) { p0.y = -p0.y; p1.y = -p1.y; }
+                if (self) { p0.y = 0.f; p1.y = 0.f; }
+                // z = p0 + i p1; v = conj(z) * a
+                v[i] = make_float2((p0.x - p1.y) * a, -(p0.y + p1.x) * a);
+            } else {
+                const float y0 = live0 ? __ldg(&in[(size_t)r0 * n + sidx]) : 0.f;
+                const float y1 = live1 ? __ldg(&in[(size_t)r1 * n + sidx]) : 0.f;
+                v[i] = make_float2(y0 * a, y1 * a);
+            }
         }
     }
     fft_reg<L, -1>(v, s, tw, t);
     if (INV) {
+        float z[2][16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
             const int k = t + i * TF;
             const float b = __ldg(&tb[k]).x;
-            if (live0) out[(size_t)r0 * n + k] = v[i].x * b;
-            if (live1) out[(size_t)r1 * n + k] = -v[i].y * b;
+            z[0][i] = v[i].x * b;
+            z[1][i] = -v[i].y * b;
+            if (sub != nullptr) {                                  // residual Radon{x} - data
+                if (live0) z[0][i] -= __ldg(&sub[(size_t)r0 * n + k]);
+                if (live1) z[1][i] -= __ldg(&sub[(size_t)r1 * n + k]);
+            }
+        }
+        if constexpr (FILT) filter_rows_in_registers<TF, 2>(z, q, n, t, f, s_red);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int k = t + i * TF;
+            if (live0) out[(size_t)r0 * n + k] = z[0][i];
+            if (live1) out[(size_t)r1 * n + k] = z[1][i];
         }
     } else {
         __syncthreads();
@@ -162,41 +296,53 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
 }
 
 template <int L>
-static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st)
+static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens,
+                       cudaStream_t st, const ProjExtra &ex)
 {
     using C = ProjCfg<L>;
     const int blocks = (p.n_angles + C::NF - 1) / C::NF;
-#define RADON_PROJ(INV_, BLUE_)                                                                          \
+    const bool filt = ex.q != nullptr;
+#define RADON_PROJ(INV_, BLUE_, FILT_)                                                                   \
     {                                                                                                    \
-        if (set_smem(proj_kernel<L, INV_, BLUE_>, C::SMEM)) return -1;                                   \
-        proj_kernel<L, INV_, BLUE_><<<blocks, C::THREADS, C::SMEM, st>>>(                                \
-            in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0, dens); \
+        if (set_smem(proj_kernel<L, INV_, BLUE_, FILT_>, C::SMEM)) return -1;                            \
+        proj_kernel<L, INV_, BLUE_, FILT_><<<blocks, C::THREADS, C::SMEM, st>>>(                         \
+            in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0, dens,  \
+            ex.sub, ex.q);                                                                               \
+    }
+#define RADON_PROJ_PAIR(INV_, FILT_)                                                                     \
+    {                                                                                                    \
+        if (set_smem(proj_pair_kernel<L, INV_, FILT_>, C::SMEM)) return -1;                              \
+        proj_pair_kernel<L, INV_, FILT_><<<pair_blocks, C::THREADS, C::SMEM, st>>>(                      \
+            in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens, ex.sub, ex.q);                      \
     }
     const bool blue = p.chirp_hf != nullptr;
     if (!blue && (!inv || half)) {        // n_det a power of two: two projections per FFT
         const int pair_blocks = ((p.n_angles + 1) / 2 + C::NF - 1) / C::NF;
-        if (inv) {
-            if (set_smem(proj_pair_kernel<L, true>, C::SMEM)) return -1;
-            proj_pair_kernel<L, true><<<pair_blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens);
-        } else {
-            if (set_smem(proj_pair_kernel<L, false>, C::SMEM)) return -1;
-            proj_pair_kernel<L, false><<<pair_blocks, C::THREADS, C::SMEM, st>>>(in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens);
-        }
+        if (inv && filt) RADON_PROJ_PAIR(true, true)
+        else if (inv) RADON_PROJ_PAIR(true, false)
+        else if (filt) RADON_PROJ_PAIR(false, true)
+        else RADON_PROJ_PAIR(false, false)
         count_launch();
         return 0;
     }
-    if (inv && blue) RADON_PROJ(true, true)
-    else if (inv) RADON_PROJ(true, false)
-    else if (blue) RADON_PROJ(false, true)
-    else RADON_PROJ(false, false)
+    if (inv && blue && filt) RADON_PROJ(true, true, true)
+    else if (inv && blue) RADON_PROJ(true, true, false)
+    else if (inv && filt) RADON_PROJ(true, false, true)
+    else if (inv) RADON_PROJ(true, false, false)
+    else if (blue && filt) RADON_PROJ(false, true, true)
+    else if (blue) RADON_PROJ(false, true, false)
+    else if (filt) RADON_PROJ(false, false, true)
+    else RADON_PROJ(false, false, false)
 #undef RADON_PROJ
+#undef RADON_PROJ_PAIR
     count_launch();
     return 0;
 }
 
-int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st)
+int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st,
+                const ProjExtra &ex)
 {
-    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, half, p, in, out, dens, st);)
+    RADON_FOR_L(p.LP, return proj_launch<LL>(inv, half, p, in, out, dens, st, ex);)
     return -1;
 }
 

@@ -198,6 +198,12 @@ void build_twiddles(int L, std::vector<float> &tw);                            /
 // L == n when n is a power of two: then hf is empty and a/b are the centring phases).
 void build_chirp(int n, int L, std::vector<float> &a, std::vector<float> &b, std::vector<float> &hf);
 int next_pow2(int v);
+// Sinogram filter: orthonormal discrete polynomials q_0 .. q_order on n
+// equispaced points, fp64 Gram-Schmidt (twice) on the monomials of t in [-1, 1], stored fp32 as
+// q[s * FILTER_MAXQ + d] (rows beyond the order are zero).
+constexpr int FILTER_MAXQ = 8;              // orders 0 .. 7
+constexpr int FILTER_FUSED_Q = 4;           // the fused kernels (proj.cu) carry orders 0 .. 3
+void build_filter_basis(int n, int order, std::vector<float> &q);
 // Density compensation of the inverse Radon transform: D_i = 1 / sum_j K(x_i - x_j, y_i - y_j)
 // over all polar samples, times the quadrature scale n phihat(0)^2 / G^2; fp64, stored fp32.
 void build_density(const Geometry &g, std::vector<float> &D, double *scale_out);

@@ -137,3 +137,16 @@ def test_bench_reference_arm_prints_the_contract_line():
         assert key in line, key
     assert line["impl"] == "reference" and line["unit"] == "pairs/s" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["cpu_baseline"]["kind"] == "oracle"
+
+
+@pytest.mark.parametrize("n,order", [(91, 3), (2048, 3), (725, 0), (64, 5), (3, 3)])
+def test_filter_basis_of_the_library_spans_the_oracle_projector(n, order):
+    """The plan-time basis of the sinogram filter (fp64 Gram-Schmidt -> fp32) against
+    O-filter: z - Q Q^T z must be the oracle's fit-and-subtract on random lines."""
+    import oracle
+
+    q = rb.filter_basis_host(n, order).astype(np.float64)
+    z = np.random.default_rng(5).standard_normal((7, n)) + np.linspace(-2, 3, n)[None, :] ** 3
+    got = z - (z @ q) @ q.T
+    ref = oracle.polyfilter(z, min(order, n - 1))
+    assert np.linalg.norm(got - ref) / np.linalg.norm(z) < 5e-7
