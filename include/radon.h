@@ -73,7 +73,7 @@ typedef struct radon_plan radon_plan;   /* opaque, owned by the library */
  * oversampling sigma (G = sigma*N must be an even integer; this build needs a
  * power of two, 16 <= G <= 8192) and Kaiser-Bessel width W (this build: 6).
  * Builds, for the current CUDA device: per-angle fp64 direction table (Fourier
- * slice geometry), Kaiser-Bessel LUT and de-apodisation vectors,
+ * slice geometry), Kaiser-Bessel weight table (polynomial pieces) and de-apodisation vectors,
  * the conflict-free gather/scatter schedules (the plan-time binning that takes
  * the place of the paper's load-balanced bins), FFT twiddles and
  * chirp tables, and the workspace.  EINVAL: N < 8, n_angles < 1, n_det < 2,

@@ -127,7 +127,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     if (!p) return RADON_OK;
     cudaDeviceSynchronize();
     DevicePlan &d = p->dev;
-    cudaFree(d.cs); cudaFree(d.lut); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
+    cudaFree(d.cs); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
     cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
     for (auto &q : d.sched) {
         cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
@@ -185,14 +185,10 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     int rc;
     // P1: Fourier-slice directions, fp64
     if ((rc = dev_upload(p, &d.cs, p->geo.cs))) return rc;
-    // P2: Kaiser-Bessel LUT, de-apodisation
-    std::vector<float> lut, deapod, tw, ca, cb, hf;
+    // P2: Kaiser-Bessel polynomial pieces, de-apodisation
+    std::vector<float> deapod, tw, ca, cb, hf;
     build_kb_poly(W, sigma, d.kb);
     build_deapod(N, G, W, sigma, deapod);
-#if RADON_KB_LUT
-    build_kb_lut(W, sigma, lut);
-    if ((rc = dev_upload(p, &d.lut, lut))) return rc;
-#endif
     if ((rc = dev_upload(p, &d.deapod, deapod))) return rc;
     build_twiddles(G, tw);
     if ((rc = dev_upload(p, &d.tw_G, tw))) return rc;
@@ -501,7 +497,7 @@ extern "C" int radon_filter(radon_plan *p, const float *d_in, float *d_out, int 
     if (!p || !d_in || !d_out || (axis != 0 && axis != 1)) return RADON_EINVAL;
     int rc = filter_ready(p);
     if (rc) return rc;
-    if (launch_filter(p->dev, axis, p->filter_q[axis], d_in, d_out, (cudaStream_t)stream)) return RADON_ECUDA;
+    if (launch_filter(p->dev, axis, p->filter_q[axis], p->filter_order, d_in, d_out, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
 }
 
@@ -515,7 +511,7 @@ extern "C" int radon_forward_filtered(radon_plan *p, const float *d_x, float *d_
     ProjExtra ex;
     if (p->filter_order < FILTER_FUSED_Q) ex.q = p->filter_q[0];
     if ((rc = forward_ws(p, p->ws[0], d_x, d_sino, st, ex))) return rc;
-    if (!ex.q && launch_filter(p->dev, 0, p->filter_q[0], d_sino, d_sino, st)) return RADON_ECUDA;
+    if (!ex.q && launch_filter(p->dev, 0, p->filter_q[0], p->filter_order, d_sino, d_sino, st)) return RADON_ECUDA;
     return check_launch();
 }
 
@@ -532,7 +528,7 @@ extern "C" int radon_adjoint_filtered(radon_plan *p, const float *d_sino, float 
     cudaStream_t st = (cudaStream_t)stream;
     if (p->filter_order < FILTER_FUSED_Q) return adjoint_ws(p, p->ws[0], d_sino, d_x, st, nullptr, p->filter_q[0]);
     if ((rc = resid_ready(p))) return rc;
-    if (launch_filter(p->dev, 0, p->filter_q[0], d_sino, p->resid, st)) return RADON_ECUDA;
+    if (launch_filter(p->dev, 0, p->filter_q[0], p->filter_order, d_sino, p->resid, st)) return RADON_ECUDA;
     return adjoint_ws(p, p->ws[0], p->resid, d_x, st);
 }
 
@@ -547,7 +543,7 @@ static int solver_step_on(radon_plan *p, float *d_x, const float *d_b, float alp
     if (fused) ex.q = p->filter_q[0];
     int rc = forward_ws(p, p->ws[0], d_x, p->resid, st, ex);
     if (rc) return rc;
-    if (filtered && !fused && launch_filter(p->dev, 0, p->filter_q[0], p->resid, p->resid, st)) return RADON_ECUDA;
+    if (filtered && !fused && launch_filter(p->dev, 0, p->filter_q[0], p->filter_order, p->resid, p->resid, st)) return RADON_ECUDA;
     IstaUpdate upd;
     upd.alpha = alpha; upd.tau = tau;
     return adjoint_ws(p, p->ws[0], p->resid, d_x, st, nullptr, nullptr, &upd);

@@ -25,26 +25,10 @@ struct Taps {
     float wx[KW], wy[KW];
 };
 
-// LUT row `it` holds, for tap l = 0..KW-1, (phi(it/S - W/2 + l), slope to the next row).
-__device__ __forceinline__ void lut_weights(const float *lut, float delta, float (&w)[KW])
-{
-    const float t = delta * (float)LUT_S;
-    int it = (int)t;
-    it = min(it, LUT_S - 1);
-    const float e = t - (float)it;
-    const float4 *row = reinterpret_cast<const float4 *>(lut + it * LUT_ROW);
-#pragma unroll
-    for (int q = 0; q < KW / 2; ++q) {
-        const float4 r = row[q];
-        w[2 * q] = fmaf(e, r.y, r.x);
-        w[2 * q + 1] = fmaf(e, r.w, r.z);
-    }
-}
-
 // Polar sample (a,k) -> fractional offsets of its first tap: delta = x0 - (gx - W/2) in [0,1).
 // fp64 on purpose (an fp32 product G*j/n*cos loses 2.6e-5 at G = 4096).
 // d = cs[a] = (G/n)(cos theta_a, sin theta_a).
-__device__ __forceinline__ void sample_taps_dir(const double2 d, const float *lut, const KbPoly &kp,
+__device__ __forceinline__ void sample_taps_dir(const double2 d, const KbPoly &kp,
                                                 int k, int cd, double halfG, Taps &tp)
 {
     const double jj = (double)(k - cd);
@@ -52,30 +36,9 @@ __device__ __forceinline__ void sample_taps_dir(const double2 d, const float *lu
     const double gy = fma(jj, d.y, halfG) - 0.5 * KW;
     const float dx = (float)(ceil(gx) - gx);
     const float dy = (float)(ceil(gy) - gy);
-#if RADON_KB_LUT
-    lut_weights(lut, dx, tp.wx);
-    lut_weights(lut, dy, tp.wy);
-#else
     kb_poly_weights(kp, dx, tp.wx);
     kb_poly_weights(kp, dy, tp.wy);
-#endif
 }
-__device__ __forceinline__ void sample_taps(const double2 *__restrict__ cs, const float *lut, const KbPoly &kp,
-                                            int a, int k, int cd, double halfG, Taps &tp)
-{
-    sample_taps_dir(__ldg(&cs[a]), lut, kp, k, cd, halfG, tp);
-}
-
-__device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__restrict__ g_lut)
-{
-#if !RADON_KB_LUT
-    return;
-#endif
-    const float4 *src = reinterpret_cast<const float4 *>(g_lut);
-    float4 *dst = reinterpret_cast<float4 *>(s_lut);
-    for (int i = threadIdx.x; i < LUT_S * LUT_ROW / 4; i += blockDim.x) dst[i] = __ldg(&src[i]);
-}
-
 // =====================================================================================
 // F3: inverse gridding (gather)
 // =====================================================================================
@@ -89,9 +52,8 @@ __device__ __forceinline__ void load_lut_to_smem(float *s_lut, const float *__re
 // "empty" mbarrier.  The 36 taps of a sample are 64-bit shared-memory loads that the
 // plan-time schedule made conflict free; slots are fetched two rounds ahead, ray directions one.
 constexpr int GATHER_THREADS = (GATHER_WARPS + 1) * 32;
-constexpr size_t LUT_SMEM = RADON_KB_LUT ? (size_t)LUT_S * LUT_ROW * sizeof(float) : 0;
 constexpr size_t GATHER_TILE_BYTES = (size_t)GT_ROWS * GT_PITCH * sizeof(float2);
-constexpr size_t GATHER_SMEM = GATHER_STAGES * GATHER_TILE_BYTES + LUT_SMEM;
+constexpr size_t GATHER_SMEM = GATHER_STAGES * GATHER_TILE_BYTES;
 static_assert((GT_PITCH * sizeof(float2)) % 16 == 0 && GT_X % 2 == 0, "bulk copies need 16-byte rows");
 static_assert(GATHER_TILE_BYTES % 16 == 0, "stage buffers stay 16-byte aligned");
 
@@ -114,11 +76,10 @@ __global__ void __launch_bounds__(GATHER_THREADS, 1)
 gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
               const GatherCta *__restrict__ items, const int *__restrict__ worker_begin,
               const Slot *__restrict__ slots,
-              const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
+              const double2 *__restrict__ cs, const KbPoly kp,
               int G, int n_det)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float *s_lut = reinterpret_cast<float *>(smem_raw + GATHER_STAGES * GATHER_TILE_BYTES);
     __shared__ __align__(8) uint64_t full[GATHER_STAGES], empty[GATHER_STAGES];
 
     const int it_begin = worker_begin[blockIdx.x], it_end = worker_begin[blockIdx.x + 1];
@@ -126,7 +87,6 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     if (threadIdx.x == 0) {
         for (int s = 0; s < GATHER_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], GATHER_WARPS); }
     }
-    load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
 
     if (warp == GATHER_WARPS) {
@@ -193,7 +153,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             const bool act = sl.ak != SLOT_EMPTY;
             const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
             Taps tp;
-            sample_taps_dir(d, s_lut, kp, k, cd, halfG, tp);
+            sample_taps_dir(d, kp, k, cd, halfG, tp);
             if (act) {
                 const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
 #if RADON_GATHER_PACKED
@@ -259,7 +219,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
 // rectangle leaves through the copy engine (bulk shared -> global stores, one per row).
 constexpr int SCATTER_THREADS = SCATTER_ITEMS * 32;
 constexpr size_t SCATTER_ACC_BYTES = (size_t)SR_Y * ACC_PITCH * sizeof(float2);
-constexpr size_t SCATTER_SMEM = SCATTER_ACC_BYTES + LUT_SMEM;
+constexpr size_t SCATTER_SMEM = SCATTER_ACC_BYTES;
 static_assert((ACC_PITCH * sizeof(float2)) % 16 == 0, "bulk stores need 16-byte rows");
 
 __device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes)
@@ -380,8 +340,7 @@ constexpr int DC_CELLS = (KW + 1) * (KW + 1);
 // to add to each cell of the (W+1)^2 centre window to dcbuf (cell c: offset ux = c % (W+1) - W/2,
 // uy = c / (W+1) - W/2 from DC; zero where nothing is to be added).  part: NT float2 of shared memory.
 template <int NT>
-__device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, const float *__restrict__ g_lut,
-                                           const KbPoly &kp, int n_det, int n_angles, int half,
+__device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, const KbPoly &kp, int n_det, int n_angles, int half,
                                            float2 *part, float2 *__restrict__ dcbuf)
 {
     const int t = threadIdx.x, cd = n_det / 2;
@@ -404,13 +363,8 @@ __device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, con
     }
     const float2 V = part[0];
     float wa[KW], wb[KW];
-#if RADON_KB_LUT
-    lut_weights(g_lut, 0.f, wa);
-    lut_weights(g_lut, 1.f, wb);
-#else
     kb_poly_weights(kp, 0.f, wa);
     kb_poly_weights(kp, 1.f, wb);
-#endif
     auto tap = [](const float (&w)[KW], int l) {
         float r = 0.f;
 #pragma unroll
@@ -553,7 +507,7 @@ struct DcJobs { int n; int job[MAX_DC_JOBS]; };
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
-               const double2 *__restrict__ cs, const float *__restrict__ g_lut, const KbPoly kp,
+               const double2 *__restrict__ cs, const KbPoly kp,
                int G, int n_det, int nyq_split, float2 *__restrict__ dcbuf, int n_angles, int half,
                const MergeJob *__restrict__ jobs, int *__restrict__ tickets, const DcJobs dcj)
 {
@@ -563,18 +517,16 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     if (blockIdx.x == 0) {
         // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
         // footprint of the sum is added by the merge of the centre rectangles (DESIGN.md R-tie)
-        dc_compute<SCATTER_THREADS>(polar, g_lut, kp, n_det, n_angles, half, acc, dcbuf);
+        dc_compute<SCATTER_THREADS>(polar, kp, n_det, n_angles, half, acc, dcbuf);
         __threadfence();
         for (int q = 0; q < dcj.n; ++q)
             join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
         return;
     }
-    float *s_lut = reinterpret_cast<float *>(smem_raw + SCATTER_ACC_BYTES);
     __shared__ ScatterCta cta;
 
     if (threadIdx.x < sizeof(ScatterCta) / 4)
         reinterpret_cast<int *>(&cta)[threadIdx.x] = reinterpret_cast<const int *>(&ctas[blockIdx.x - 1])[threadIdx.x];
-    load_lut_to_smem(s_lut, g_lut);
     __syncthreads();
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -626,7 +578,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         // at the point of use, so that the prefetched load stays off the critical path.
         if (nyq_split && (k0 == 0 || k0 == n_det)) v0 = make_float2(0.5f * v0.x, k0 == 0 ? 0.5f * v0.y : -0.5f * v0.y);
         Taps tp;
-        sample_taps_dir(d0, s_lut, kp, k0, cd, halfG, tp);
+        sample_taps_dir(d0, kp, k0, cd, halfG, tp);
         const int bx = (int)(s0.lxy & 0xffff), by = (int)(s0.lxy >> 16);   // biased by KH
         const uint32_t base = origin + (uint32_t)((by * ACC_PITCH + bx) * (int)sizeof(float2));
         if (RADON_SC_FAST && r < item.fast_count) {   // warp-uniform: footprints wholly inside the quadrant
@@ -683,7 +635,7 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     if (q.n_gather_ctas == 0) return 0;
     gather_kernel<<<q.n_gather_workers, GATHER_THREADS, GATHER_SMEM, st>>>(
-        grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.lut, p.kb, p.G, p.n_det);
+        grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.kb, p.G, p.n_det);
     count_launch();
     return 0;
 }
@@ -698,7 +650,7 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
     for (int i = 0; i < MAX_DC_JOBS; ++i) dcj.job[i] = q.dc_jobs[i];
     // CTA 0 sums the j = 0 samples; CTA b > 0 grids scatter_ctas[b - 1] (heaviest first)
     scatter_kernel<<<q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st>>>(
-        polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.lut, p.kb, p.G, p.n_det, nyq,
+        polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.kb, p.G, p.n_det, nyq,
         dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);
     count_launch();
     return 0;

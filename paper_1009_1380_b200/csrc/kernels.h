@@ -14,7 +14,6 @@ struct DevicePlan {
     int n_sm = 148;               // multiprocessors of the device (persistent grids)
     // tables
     double2 *cs = nullptr;        // per angle (G/n)(cos, sin), fp64
-    float *lut = nullptr;         // LUT_S x LUT_ROW (only with RADON_KB_LUT)
     KbPoly kb;                    // polynomial pieces of the Kaiser-Bessel kernel
     float *deapod = nullptr;      // N
     float2 *tw_G = nullptr;       // twiddles for length G
@@ -103,7 +102,8 @@ struct ProjExtra { const float *sub = nullptr; const float *q = nullptr; };
 int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float *out, const float *dens, cudaStream_t st,
                 const ProjExtra &ex = ProjExtra());
 // axis 0: along the detector coordinate of every projection; 1: along the angles of every detector bin
-int launch_filter(const DevicePlan &p, int axis, const float *q, const float *in, float *out, cudaStream_t st);
+// order > 3: the basis has more than four columns
+int launch_filter(const DevicePlan &p, int axis, const float *q, int order, const float *in, float *out, cudaStream_t st);
 
 
 }  // namespace radon

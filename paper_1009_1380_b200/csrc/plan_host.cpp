@@ -24,7 +24,6 @@
 
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <thread>
@@ -94,20 +93,6 @@ static double kb_phi(double u, int W, double beta, double inv_i0b)
     const double arg = 1.0 - t * t;
     if (arg < 0.0) return (arg > -1e-12) ? inv_i0b : 0.0;   // |u| == W/2 up to rounding
     return kb_i0(beta * std::sqrt(arg)) * inv_i0b;
-}
-
-void build_kb_lut(int W, double sigma, std::vector<float> &lut)
-{
-    const double beta = kb_beta(W, sigma), inv = 1.0 / kb_i0(beta);
-    lut.assign((size_t)LUT_S * 2 * W, 0.f);
-    for (int r = 0; r < LUT_S; ++r)
-        for (int l = 0; l < W; ++l) {
-            const double u0 = (double)r / LUT_S - 0.5 * W + l;
-            const double u1 = (double)(r + 1) / LUT_S - 0.5 * W + l;
-            const double v0 = kb_phi(u0, W, beta, inv), v1 = kb_phi(u1, W, beta, inv);
-            lut[((size_t)r * W + l) * 2 + 0] = (float)v0;
-            lut[((size_t)r * W + l) * 2 + 1] = (float)(v1 - v0);
-        }
 }
 
 // Polynomial pieces of the kernel: for tap l (l < W/2) and delta in [0,1), z = 2 delta - 1,
@@ -537,14 +522,12 @@ static void scatter_rects(const Geometry &g, bool half, std::vector<RowSeg> &seg
     }
 }
 
-static void build_scatter(const Geometry &g, Schedules &out)
+static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
 {
     const int G = g.G;
     const bool half = out.half;
     const int k_end = scatter_k_end(g, half);
-    // measured at config 4: 48 is best for the half schedule (66 vs 79 us), 96 for the full one (108 vs 118 us)
-    int round_max = half ? SCATTER_ROUND_MAX / 2 : SCATTER_ROUND_MAX;
-    if (const char *e = std::getenv(half ? "RADON_TUNE_RMAX_HALF" : "RADON_TUNE_RMAX_FULL")) round_max = std::atoi(e);
+    int round_max = SCATTER_ROUND_MAX;       // set below, once the incidences are counted
     const int nrx = (G + SR_X - 1) / SR_X;
     std::vector<RowSeg> segs;
     std::vector<RectGeom> rects;
@@ -589,6 +572,19 @@ static void build_scatter(const Geometry &g, Schedules &out)
             }
     }
 
+    // Rounds a warp runs before a tile's samples are split over several CTAs.  A tile that runs
+    // alone takes ~0.4 us per round whatever the rest of the device does, so the limit follows the
+    // load: about 1.8 x the mean number of rounds per resident warp (measured at config 4: 48 rounds
+    // is best for the Hermitian-half schedule, mean 26.5, and 96 for the full one, mean 53; at the
+    // small configs, where a handful of centre tiles hold most samples, the lower limit:
+    // bare gridding at config 1 39 -> 15 us, config 3 51 -> 20 us).
+    {
+        long long est_rounds = 0;
+        for (int r = 0; r < nrect; ++r) est_rounds += (count[r + 1] - count[r] + 27) / 28;
+        const double slots = (double)std::max(1, n_workers) * SCATTER_CTAS_PER_SM * SCATTER_ITEMS;
+        round_max = (int)std::lround(1.8 * (double)est_rounds / slots);
+        round_max = std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, round_max));
+    }
     struct Pending { ScatterCta cta; long long work; };
     std::vector<Pending> ctas;
     std::vector<Cand> quad[SCATTER_ITEMS];
@@ -716,7 +712,7 @@ void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers
     out = Schedules();
     out.half = half;
     build_gather(g, out, n_workers);
-    build_scatter(g, out);
+    build_scatter(g, out, n_workers);
 }
 
 // ---------------------------------------------------------------- self check -----

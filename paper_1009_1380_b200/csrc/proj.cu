@@ -21,7 +21,7 @@ struct ProjCfg {
     static constexpr int THREADS = NF * TF;
     static constexpr int PADLEN = fft_padded_len(L);
     static constexpr size_t SMEM = (size_t)NF * PADLEN * sizeof(float2);
-    static constexpr int MIN_CTAS = (1024 / THREADS > 2) ? 1024 / THREADS - 1 : 1024 / THREADS;   // <= 72 registers per thread
+    static constexpr int MIN_CTAS = 1024 / THREADS;      // <= 64 registers per thread
 };
 
 // Sum NV values over the TF threads that share one FFT (thread t of FFT f in the CTA); every
@@ -159,10 +159,13 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
             const int k = t + i * TF;
-            z[0][i] = 0.f;
-            if (live && k < n) {
-                z[0][i] = cmul(v[i], __ldg(&tb[k])).x;
-                if (sub != nullptr) z[0][i] -= __ldg(&sub[(size_t)row * n + k]);     // residual Radon{x} - data
+            z[0][i] = (live && k < n) ? cmul(v[i], __ldg(&tb[k])).x : 0.f;
+        }
+        if (sub != nullptr) {                                      // residual Radon{x} - data (one branch: the loads stay batched)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const int k = t + i * TF;
+                z[0][i] -= (live && k < n) ? __ldg(&sub[(size_t)row * n + k]) : 0.f;
             }
         }
         if constexpr (FILT) filter_rows_in_registers<TF, 1>(z, q, n, t, f, s_red);
@@ -256,13 +259,16 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
         float z[2][16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-            const int k = t + i * TF;
-            const float b = __ldg(&tb[k]).x;
+            const float b = __ldg(&tb[t + i * TF]).x;
             z[0][i] = v[i].x * b;
             z[1][i] = -v[i].y * b;
-            if (sub != nullptr) {                                  // residual Radon{x} - data
-                if (live0) z[0][i] -= __ldg(&sub[(size_t)r0 * n + k]);
-                if (live1) z[1][i] -= __ldg(&sub[(size_t)r1 * n + k]);
+        }
+        if (sub != nullptr) {                                      // residual Radon{x} - data (one branch: the loads stay batched)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const int k = t + i * TF;
+                z[0][i] -= live0 ? __ldg(&sub[(size_t)r0 * n + k]) : 0.f;
+                z[1][i] -= live1 ? __ldg(&sub[(size_t)r1 * n + k]) : 0.f;
             }
         }
         if constexpr (FILT) filter_rows_in_registers<TF, 2>(z, q, n, t, f, s_red);

@@ -9,15 +9,13 @@ namespace radon {
 // ---- compile-time configuration -------------------------------------------------
 constexpr int KW = 6;                 // Kaiser-Bessel width this build is specialised for
 constexpr int KH = KW - 1;            // halo: a footprint reaches base .. base+KH
-// Kaiser-Bessel weight table.  Default: ONE polynomial piece per tap (degree KB_DEG in
-// z = 2*delta - 1, fitted in fp64 at plan time, max error ~7e-8), passed to the kernels in
-// the constant bank -- a lookup table whose rows are polynomial pieces, read as broadcast
-// operands, so it costs neither shared-memory bandwidth nor bank conflicts.
-// -DRADON_KB_LUT=1 builds the classic variant instead (LUT_S rows per grid unit in shared
-// memory, linear interpolation; ~3e-6 relative error at LUT_S = 256) for A/B measurements.
-#ifndef RADON_KB_LUT
-#define RADON_KB_LUT 0
-#endif
+// Kaiser-Bessel weights: ONE polynomial piece per tap (degree KB_DEG in z = 2*delta - 1, fitted
+// in fp64 at plan time, max error ~7e-8), passed to the kernels in the constant bank -- a lookup
+// table whose rows are polynomial pieces, read as broadcast operands, so it costs neither
+// shared-memory bandwidth nor bank conflicts.  north_star's shared-memory LUT with linear
+// interpolation was built and measured against it (profiles/r02_kb_lut_ab.md: 256 rows per grid
+// unit cost 3e-6 of the 1e-5 budget, 1024 rows 48 KB of shared memory per CTA, and either makes
+// the gather 56 % slower); the polynomial pieces are what the library ships.
 constexpr int KB_DEG = 7;
 constexpr int KB_HALF = (KB_DEG + 1) / 2;   // coefficients of the even / odd part
 struct KbPoly {                       // tap l: E_l(z^2) + z O_l(z^2); tap KW-1-l: E_l - z O_l
@@ -51,9 +49,6 @@ RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
         w[KW - 1 - l] = e - z * o;
     }
 }
-constexpr int LUT_S = 256;            // (RADON_KB_LUT) rows per grid unit, linear interpolation
-constexpr int LUT_ROW = 2 * KW;       // (RADON_KB_LUT) floats per row: (value, slope) per tap
-
 // Gather (inverse gridding): a work item is a GT_X x GT_Y tile of the grid (+halo), staged by
 // one bulk copy per tile row.  Wide, flat tiles: the copy engine spends ~65 cycles per copy
 // whatever its size (measured: 1 KB copies reach 4.5 TB/s over 148 SMs, >= 2 KB copies the HBM
@@ -71,7 +66,7 @@ constexpr int GT_ROWS = GT_Y + KH;    // 21 rows staged per tile
 #define RADON_GWARPS 24
 #endif
 constexpr int GATHER_WARPS = RADON_GWARPS;      // consumer warps of the persistent gather CTA (+1 producer warp)
-constexpr int GATHER_STAGES = RADON_KB_LUT ? 2 : RADON_GSTAGES;   // tiles in flight per CTA (GT_ROWS x GT_PITCH x 8 B = 65.5 KB each)
+constexpr int GATHER_STAGES = RADON_GSTAGES;   // tiles in flight per CTA (GT_ROWS x GT_PITCH x 8 B = 65.5 KB each)
 #ifndef RADON_GCOST
 #define RADON_GCOST 16
 #endif
@@ -111,8 +106,12 @@ constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
 constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
 constexpr int SB_W = ST_X + KH, SB_H = ST_Y + KH;   // range of biased base coordinates in a quadrant
-constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a rectangle's samples are split over CTAs
-                                      // (full schedule; the Hermitian-half one, with half the CTAs, splits at 48)
+constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples are split over CTAs: upper and
+#ifndef RADON_SC_RMIN
+#define RADON_SC_RMIN 12
+#endif
+constexpr int SCATTER_ROUND_MIN = RADON_SC_RMIN;  // lower limit (12: best over configs 1-3 and the paper's shape, 8..24 measured); the builder
+                                      // picks 1.8 x the mean rounds per resident warp
 constexpr int SCATTER_CTAS_PER_SM = RADON_SC_CTAS;
 
 // One lane's work in one round: which polar sample, and where its W x W footprint
@@ -190,7 +189,6 @@ long long check_schedules(const Geometry &g, const Schedules &s);
 // ---- host-side tables (all derived in fp64, stored fp32) -------------------------
 double kb_beta(int W, double sigma);
 double kb_i0(double z);
-void build_kb_lut(int W, double sigma, std::vector<float> &lut);              // LUT_S x LUT_ROW
 void build_kb_poly(int W, double sigma, KbPoly &kp);                            // Chebyshev fit, fp64
 void build_deapod(int N, int G, int W, double sigma, std::vector<float> &d);   // N floats
 void build_twiddles(int L, std::vector<float> &tw);                            // L x (cos, -sin)
