@@ -371,6 +371,7 @@ def main():
     #      pixels per angle", 3 ms FFTs + 6 ms gridding on a Tesla C1060): context, not the headline.
     #      Both readings of "1024x1024 grid": the oversampled grid, or the image. ------
     paper_shape = {}
+    gen_p = torch.Generator(device=dev); gen_p.manual_seed(99)
     for label, Np in (("grid_1024 (N=512, G=1024)", 512), ("image_1024 (N=1024, G=2048)", 1024)):
         pp = rb.RadonPlan(Np, 180, 1024)
         xp = torch.from_numpy(workloads.make_batch_slice(1, Np)).to(dev)
@@ -388,6 +389,23 @@ def main():
         paper_shape[label] = {"us_per_pair": round(us, 1), "pairs_per_s": round(1e6 / us, 1),
                               "paper_C1060_us_per_pair": 9000.0,
                               "note": "working set fits the 126 MB L2; 180 x 1024 samples, sigma=2, W=6"}
+        # the paper's own design for the gridding step (load-balanced quadtree bins, one
+        # thread block per bin, two per-bin strategies) against this library's, same sum, same data
+        cp = torch.view_as_complex(torch.randn((180, 1024, 2), device=dev, generator=gen_p))
+        cg = torch.empty((pp.G, pp.G), dtype=torch.complex64, device=dev)
+        cmpv = {}
+        for name, fn in (("radon_grid_only", lambda: pp.radon_grid_only(cp, cg)),
+                         ("radon_grid_only_paper_bins_4096", lambda: pp.radon_grid_only_paper_bins(cp, cg, n_bins=4096))):
+            for _ in range(3):
+                fn()
+            e0.record(stream)
+            for _ in range(10):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            cmpv[name + "_us"] = round(e0.elapsed_time(e1) / 10 * 1e3, 1)
+        cmpv["bins"] = pp.paper_bins_stats()
+        paper_shape[label]["gridding_design_comparison"] = cmpv
         del pp
 
     # ---- the density-compensated inverse Radon transform at this config ----

@@ -124,6 +124,18 @@ int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *
  * the result is bit-identical from run to run. */
 int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream);
 
+/* The paper's own GPU design for the same gridding sum, kept as a measured comparison (prior
+ * art, not the product path): load-balanced bins by recursive four-way splitting of the most
+ * expensive bin (cost = samples x grid points), one thread block per bin, one thread per grid
+ * point over the samples staged in shared memory when they fit (<= 1024), all threads per grid
+ * point otherwise.  n_bins: where the splitting stops; the bins are built on the
+ * host at the first call with a given n_bins (blocking).  Same arguments, tap rule and weights
+ * as radon_grid_only; the result differs by the order of the additions only. */
+int radon_grid_only_paper_bins(radon_plan *p, const float *d_polar, float *d_grid, int n_bins, void *stream);
+/* Bins of the last radon_grid_only_paper_bins call: count, sample incidences, samples of the
+ * largest bin, bins whose samples do not fit in shared memory.  EINVAL before the first call. */
+int radon_paper_bins_stats(const radon_plan *p, int *n_bins, long long *n_entries, int *max_samples, int *n_unstaged);
+
 /* 1-D transforms along the projections alone (last step):
  * radon_proj_ifft: polar 2*M floats -> sinogram, S = Re{(1/n) sum_k P exp(+i 2 pi j t/n)};
  * radon_proj_fft:  sinogram -> polar, its transpose Yh = (1/n) sum_s y exp(-i 2 pi j t/n). */

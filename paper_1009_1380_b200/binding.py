@@ -24,6 +24,8 @@ _SIGNATURES = {
     "radon_nufft1": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_interp_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_grid_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_grid_only_paper_bins": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "radon_paper_bins_stats": (c_int, [c_void_p, P(c_int), P(c_ll), P(c_int), P(c_int)]),
     "radon_proj_ifft": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_proj_fft": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_plan_stage_timing": (c_int, [c_void_p, c_int]),
@@ -362,6 +364,23 @@ class RadonPlan:
         self._chk(grid, torch.complex64, self.G * self.G, "grid")
         _check(lib().radon_grid_only(self._h, _ptr(polar), _ptr(grid), self._stream()), "radon_grid_only")
         return grid
+
+    def radon_grid_only_paper_bins(self, polar, grid=None, n_bins=4096):
+        """The paper's own bins / one-block-per-bin design: comparison only."""
+        import torch
+
+        self._chk(polar, torch.complex64, self.M, "polar")
+        grid = self._new((self.G, self.G), torch.complex64) if grid is None else grid
+        self._chk(grid, torch.complex64, self.G * self.G, "grid")
+        _check(lib().radon_grid_only_paper_bins(self._h, _ptr(polar), _ptr(grid), int(n_bins), self._stream()),
+               "radon_grid_only_paper_bins")
+        return grid
+
+    def paper_bins_stats(self):
+        nb, ne, mx, un = c_int(), c_ll(), c_int(), c_int()
+        _check(lib().radon_paper_bins_stats(self._h, nb, ne, mx, un), "radon_paper_bins_stats")
+        return {"bins": nb.value, "sample_incidences": ne.value, "max_samples_per_bin": mx.value,
+                "bins_not_fitting_shared_memory": un.value}
 
     def radon_proj_ifft(self, polar, sino=None):
         import torch

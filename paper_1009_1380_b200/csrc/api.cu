@@ -77,6 +77,11 @@ struct radon_plan {
         long long kernels = 0;            // kernel nodes of one iteration
     } sgraph;
     cudaStream_t capture_stream = nullptr;
+    // the paper's load-balanced bins (comparison variant, built on first use)
+    PaperBin *pb_bins = nullptr;
+    PaperBinEntry *pb_entries = nullptr;
+    int pb_n_bins = 0, pb_target = 0, pb_max_samples = 0, pb_unstaged = 0;
+    long long pb_n_entries = 0;
 };
 
 template <typename T>
@@ -138,6 +143,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     if (p->fork_event) cudaEventDestroy(p->fork_event);
     cudaFree(p->dev_density);
     cudaFree(p->filter_q[0]); cudaFree(p->filter_q[1]); cudaFree(p->resid);
+    cudaFree(p->pb_bins); cudaFree(p->pb_entries);
     if (p->sgraph.exec) cudaGraphExecDestroy(p->sgraph.exec);
     if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     for (int i = 0; i < NWS; ++i) {
@@ -745,6 +751,45 @@ extern "C" int radon_grid_only(radon_plan *p, const float *d_polar, float *d_gri
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
     if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, p->ws[0].scratch, p->ws[0].dcbuf, p->ws[0].tickets, (cudaStream_t)stream)) return RADON_ECUDA;
     return check_launch();
+}
+
+// ---- the paper's own gridding design, measured comparison ---------------------
+extern "C" int radon_grid_only_paper_bins(radon_plan *p, const float *d_polar, float *d_grid, int n_bins, void *stream)
+{
+    if (!p || !d_polar || !d_grid || n_bins < 1) return RADON_EINVAL;
+    if (!p->pb_bins || p->pb_target != n_bins) {
+        CUDA_TRY(cudaDeviceSynchronize());
+        cudaFree(p->pb_bins); cudaFree(p->pb_entries);
+        p->pb_bins = nullptr; p->pb_entries = nullptr;
+        PaperBins pb;
+        try {
+            build_paper_bins(p->geo, n_bins, pb);
+        } catch (const std::bad_alloc &) {
+            return RADON_ENOMEM;
+        }
+        int rc;
+        if ((rc = dev_upload(p, &p->pb_bins, pb.bins))) return rc;
+        if ((rc = dev_upload(p, &p->pb_entries, pb.entries))) return rc;
+        p->pb_n_bins = (int)pb.bins.size(); p->pb_target = n_bins; p->pb_n_entries = (long long)pb.entries.size();
+        p->pb_max_samples = 0; p->pb_unstaged = 0;
+        for (const PaperBin &b : pb.bins) {
+            p->pb_max_samples = std::max(p->pb_max_samples, b.count);
+            p->pb_unstaged += b.count > 1024 ? 1 : 0;
+        }
+    }
+    if (launch_paper_bins(p->dev, p->pb_bins, p->pb_n_bins, p->pb_entries, (const float2 *)d_polar, (float2 *)d_grid,
+                          (cudaStream_t)stream)) return RADON_ECUDA;
+    return check_launch();
+}
+
+extern "C" int radon_paper_bins_stats(const radon_plan *p, int *n_bins, long long *n_entries, int *max_samples, int *n_unstaged)
+{
+    if (!p || !p->pb_bins) return RADON_EINVAL;
+    if (n_bins) *n_bins = p->pb_n_bins;
+    if (n_entries) *n_entries = p->pb_n_entries;
+    if (max_samples) *max_samples = p->pb_max_samples;
+    if (n_unstaged) *n_unstaged = p->pb_unstaged;
+    return RADON_OK;
 }
 
 extern "C" int radon_proj_ifft(radon_plan *p, const float *d_polar, float *d_sino, void *stream)

@@ -8,6 +8,7 @@
 // (the FFT passes live in fft2d.cu, the projection DFTs in proj.cu)
 #include "kernels.h"
 #include "async_copy.cuh"
+#include "taps.cuh"
 
 #include <atomic>
 
@@ -17,28 +18,6 @@ static std::atomic<long long> g_launches{0};
 long long launch_count() { return g_launches.load(); }
 void count_launch(long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
-// =====================================================================================
-// Sample coordinates and Kaiser-Bessel weights (shared by gather and scatter so that the
-// two kernels use bit-identical tap positions and weights: exact transposes)
-// =====================================================================================
-struct Taps {
-    float wx[KW], wy[KW];
-};
-
-// Polar sample (a,k) -> fractional offsets of its first tap: delta = x0 - (gx - W/2) in [0,1).
-// fp64 on purpose (an fp32 product G*j/n*cos loses 2.6e-5 at G = 4096).
-// d = cs[a] = (G/n)(cos theta_a, sin theta_a).
-__device__ __forceinline__ void sample_taps_dir(const double2 d, const KbPoly &kp,
-                                                int k, int cd, double halfG, Taps &tp)
-{
-    const double jj = (double)(k - cd);
-    const double gx = fma(jj, d.x, halfG) - 0.5 * KW;
-    const double gy = fma(jj, d.y, halfG) - 0.5 * KW;
-    const float dx = (float)(ceil(gx) - gx);
-    const float dy = (float)(ceil(gy) - gy);
-    kb_poly_weights(kp, dx, tp.wx);
-    kb_poly_weights(kp, dy, tp.wy);
-}
 // =====================================================================================
 // F3: inverse gridding (gather)
 // =====================================================================================

@@ -106,4 +106,8 @@ int launch_proj(bool inv, bool half, const DevicePlan &p, const float *in, float
 int launch_filter(const DevicePlan &p, int axis, const float *q, int order, const float *in, float *out, cudaStream_t st);
 
 
+// The paper's own design, comparison only: one thread block per load-balanced bin
+int launch_paper_bins(const DevicePlan &p, const PaperBin *bins, int n_bins, const PaperBinEntry *entries,
+                      const float2 *polar, float2 *grid, cudaStream_t st);
+
 }  // namespace radon

@@ -707,6 +707,64 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
     for (auto &p : ctas) out.scatter_ctas.push_back(p.cta);
 }
 
+// ---------------------------------------------------------------- paper's bins ----
+void build_paper_bins(const Geometry &g, int n_bins_target, PaperBins &out)
+{
+    const int G = g.G;
+    struct Node { int x0, y0, w, h; std::vector<PaperBinEntry> e; };
+    auto cost = [](const Node &n) { return (long long)n.e.size() * n.w * n.h; };
+    auto base_of = [&](const PaperBinEntry &en, int &bx, int &by) {
+        int x0, y0;
+        g.base((int)(en.ak >> 16), (int)(en.ak & 0xffff), x0, y0);
+        bx = x0 + ((en.shift & 3) - 1) * G;
+        by = y0 + (((en.shift >> 2) & 3) - 1) * G;
+    };
+    std::vector<Node> nodes(1);
+    nodes[0] = Node{0, 0, G, G, {}};
+    for (int a = 0; a < g.n_angles; ++a)
+        for (int k = 0; k < g.n_det; ++k) {
+            int x0, y0;
+            g.base(a, k, x0, y0);
+            for (int sy = -1; sy <= 1; ++sy) {
+                const int by = y0 + sy * G;
+                if (by + KH < 0 || by > G - 1) continue;
+                for (int sx = -1; sx <= 1; ++sx) {
+                    const int bx = x0 + sx * G;
+                    if (bx + KH < 0 || bx > G - 1) continue;
+                    nodes[0].e.push_back(PaperBinEntry{((uint32_t)a << 16) | (uint32_t)k, (sx + 1) | ((sy + 1) << 2)});
+                }
+            }
+        }
+    // "recursively divides the most computationally intensive bin into four equally sized bins"
+    while ((int)nodes.size() < n_bins_target) {
+        int top = -1;
+        long long best = 0;
+        for (size_t i = 0; i < nodes.size(); ++i)
+            if (nodes[i].w >= 16 && nodes[i].h >= 16 && cost(nodes[i]) > best) { best = cost(nodes[i]); top = (int)i; }
+        if (top < 0) break;
+        Node parent = std::move(nodes[top]);
+        nodes[top] = std::move(nodes.back());
+        nodes.pop_back();
+        const int hw = parent.w / 2, hh = parent.h / 2;
+        for (int qy = 0; qy < 2; ++qy)
+            for (int qx = 0; qx < 2; ++qx) {
+                Node c{parent.x0 + qx * hw, parent.y0 + qy * hh, qx ? parent.w - hw : hw, qy ? parent.h - hh : hh, {}};
+                for (const PaperBinEntry &en : parent.e) {
+                    int bx, by;
+                    base_of(en, bx, by);
+                    if (bx + KH >= c.x0 && bx < c.x0 + c.w && by + KH >= c.y0 && by < c.y0 + c.h) c.e.push_back(en);
+                }
+                nodes.push_back(std::move(c));
+            }
+    }
+    std::stable_sort(nodes.begin(), nodes.end(), [&](const Node &a, const Node &b) { return cost(a) > cost(b); });
+    out.bins.clear(); out.entries.clear();
+    for (const Node &n : nodes) {
+        out.bins.push_back(PaperBin{n.x0, n.y0, n.w, n.h, (int)out.entries.size(), (int)n.e.size()});
+        out.entries.insert(out.entries.end(), n.e.begin(), n.e.end());
+    }
+}
+
 void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers)
 {
     out = Schedules();

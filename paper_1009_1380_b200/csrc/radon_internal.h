@@ -206,4 +206,25 @@ void build_filter_basis(int n, int order, std::vector<float> &q);
 // over all polar samples, times the quadrature scale n phihat(0)^2 / G^2; fp64, stored fp32.
 void build_density(const Geometry &g, std::vector<float> &D, double *scale_out);
 
+// ---- the paper's own gridding design, kept as a measured comparison ----------
+// "The load balancing algorithm starts by considering one bin containing all the points, and
+// recursively divides the most computationally intensive bin into four equally sized bins (the
+// computational cost is estimated as the number of samples times the number of grid points in
+// each bin) ... one thread block per bin."  A bin lists every sample image whose W x W footprint
+// touches it (a sample near a border is listed by both neighbours).
+struct PaperBin {
+    int x0, y0, w, h;           // cells [x0, x0 + w) x [y0, y0 + h) of the centred grid
+    int first, count;           // entries [first, first + count) of the sample list
+};
+struct PaperBinEntry {
+    uint32_t ak;                // (a << 16) | k
+    int32_t shift;              // wrap image: (sx + 1) | ((sy + 1) << 2), base cell = (x0 + sx G, y0 + sy G)
+};
+struct PaperBins {
+    std::vector<PaperBin> bins;             // heaviest first
+    std::vector<PaperBinEntry> entries;
+};
+// n_bins_target: stop splitting once there are this many bins (or no bin can be split: side 8)
+void build_paper_bins(const Geometry &g, int n_bins_target, PaperBins &out);
+
 }  // namespace radon
