@@ -490,9 +490,10 @@ def main():
                    "l2": f"inputs {B * cfg.N * cfg.N * 4 / 1e6:.0f} MB/step cycle through HBM (> 126 MB L2); per-slice grid 134 MB > L2"},
         "samples_per_s": 2.0 * cfg.M * value, "us_per_pair": t_pair_us,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "plan": {"plan_create_ms": round(plan_create_ms, 1), "plan_device_bytes": int(plan.workspace_bytes),
+        "plan": {"plan_create_ms": round(plan_create_ms, 1), "schedules_ms": round(plan.schedule_check(True, verify=False)[2], 1),
+                 "schedules_built_on_device": bool(plan.schedule_check(True, verify=False)[1]), "plan_device_bytes": int(plan.workspace_bytes),
                  "plan_device_bytes_after_run": int(plan.device_bytes()),
-                 "note": "radon_plan_create: tables + host-built schedules + first workspace; the batched calls "
+                 "note": "radon_plan_create: tables + schedules (CUDA kernels, plan_device.cu) + first workspace; the batched calls "
                          "add three more workspaces on first use"},
         "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "paper_shape": paper_shape, "next_rows": next_rows,
         "cpu_baseline": cpu_baseline,

@@ -230,6 +230,15 @@ int radon_plan_schedule_stats(const radon_plan *p, int half,
                               long long *gather_slots, long long *gather_filled, int *gather_ctas,
                               long long *scatter_slots, long long *scatter_filled, int *scatter_ctas);
 
+/* The schedules a plan uses are built by CUDA kernels (sample binning into tiles from the
+ * Fourier-slice geometry and first-fit packing into conflict-free rounds, one warp per tile share);
+ * the host builder below stays as the checker and as the fallback (a list that outgrows its
+ * scratch, or RADON_PLAN_BUILDER=host in the environment).  radon_plan_schedule_check downloads the
+ * plan's slot arrays and runs the same verification as radon_schedule_selfcheck on them.
+ * *n_violations (may be NULL: no check), *device_built (1 if kernels built this half's schedules),
+ * *build_ms (host wall time of both schedule sets inside radon_plan_create). */
+int radon_plan_schedule_check(radon_plan *p, int half, long long *n_violations, int *device_built, double *build_ms);
+
 /* Host-only self-check of the plan-time schedule builder; needs NO GPU.  Builds
  * the gather and scatter schedules for the geometry and verifies that every
  * sample is issued exactly once by the gather, that the scatter issues every

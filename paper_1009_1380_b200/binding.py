@@ -32,6 +32,7 @@ _SIGNATURES = {
     "radon_plan_stage_times": (c_int, [c_void_p, P(ctypes.c_double), P(c_ll)]),
     "radon_plan_info": (c_int, [c_void_p, P(c_int), P(c_int), P(c_int), P(c_int), P(c_ll), P(c_size_t)]),
     "radon_plan_schedule_stats": (c_int, [c_void_p, c_int, P(c_ll), P(c_ll), P(c_int), P(c_ll), P(c_ll), P(c_int)]),
+    "radon_plan_schedule_check": (c_int, [c_void_p, c_int, P(c_ll), P(c_int), P(ctypes.c_double)]),
     "radon_schedule_selfcheck": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_schedule_host_stats": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_kb_weights_host": (c_int, [c_int, c_float, c_float, P(c_float)]),
@@ -189,6 +190,15 @@ class RadonPlan:
         wb = c_size_t()
         _check(lib().radon_plan_info(self._h, None, None, None, None, None, wb), "radon_plan_info")
         return int(wb.value)
+
+    def schedule_check(self, half=False, verify=True):
+        """(violations or None, built_on_device, build_ms) of the schedules this plan uses."""
+        bad = c_ll(-1); dev = c_int(); ms = ctypes.c_double()
+        rc = lib().radon_plan_schedule_check(self._h, int(half), ctypes.byref(bad) if verify else None,
+                                             ctypes.byref(dev), ctypes.byref(ms))
+        if rc not in (0, -1):
+            _check(rc, "radon_plan_schedule_check")
+        return (int(bad.value) if verify else None), bool(dev.value), float(ms.value)
 
     def schedule_stats(self, half=False):
         v = [c_ll(), c_ll(), c_int(), c_ll(), c_ll(), c_int()]

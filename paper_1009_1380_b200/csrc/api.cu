@@ -2,12 +2,15 @@
 // sequences of radon_forward / radon_adjoint.  No torch types, no exceptions across the ABI.
 #include "../../include/radon.h"
 
+#include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
 
 #include "kernels.h"
+#include "plan_device.h"
 
 using namespace radon;
 
@@ -82,6 +85,11 @@ struct radon_plan {
     PaperBinEntry *pb_entries = nullptr;
     int pb_n_bins = 0, pb_target = 0, pb_max_samples = 0, pb_unstaged = 0;
     long long pb_n_entries = 0;
+    // P3: where the schedules were built (1: CUDA kernels of plan_device.cu, 0: host builder) and the
+    // host copy of everything but the slot arrays (radon_plan_schedule_check downloads those)
+    int device_built[2] = {0, 0};
+    Schedules meta[2];
+    double schedule_ms = 0.0;
 };
 
 template <typename T>
@@ -206,12 +214,42 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if (!hf.empty() && (rc = dev_upload(p, &d.chirp_hf, hf))) return rc;
     // P3: schedules
     int n_partial = 0;
+    const char *builder_env = std::getenv("RADON_PLAN_BUILDER");          // "host": force the host builder
+    const bool want_device = !(builder_env && std::strcmp(builder_env, "host") == 0);
+    const auto t_sched = std::chrono::steady_clock::now();
     for (int h = 0; h < 2; ++h) {
-        Schedules sch;
-        build_schedules(p->geo, sch, h == 1, d.n_sm);
+        Schedules &sch = p->meta[h];
         DevicePlan::Sched &q = d.sched[h];
-        p->gather_slots[h] = (long long)sch.gather_slots.size(); p->gather_filled[h] = sch.gather_filled;
-        p->scatter_slots[h] = (long long)sch.scatter_slots.size(); p->scatter_filled[h] = sch.scatter_filled;
+        Slot *dg = nullptr, *dsl = nullptr;
+        long long ng = 0, ns = 0;
+        int drc = want_device ? build_schedules_device(p->geo, d.cs, h == 1, d.n_sm, sch, &dg, &ng, &dsl, &ns) : -3;
+        if (drc == 0) {
+            p->device_built[h] = 1;
+            q.gather_slots = dg; q.scatter_slots = dsl;
+            p->device_bytes += (size_t)(ng + ns) * 32 * sizeof(Slot);
+            p->gather_slots[h] = ng * 32; p->scatter_slots[h] = ns * 32;
+        } else {
+            cudaGetLastError();                                          // a failed device build must not poison later calls
+            build_schedules(p->geo, sch, h == 1, d.n_sm);
+            p->gather_slots[h] = (long long)sch.gather_slots.size();
+            p->scatter_slots[h] = (long long)sch.scatter_slots.size();
+            if ((rc = dev_upload(p, &q.gather_slots, sch.gather_slots))) return rc;
+            if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;
+            sch.gather_slots.clear(); sch.gather_slots.shrink_to_fit();
+            sch.scatter_slots.clear(); sch.scatter_slots.shrink_to_fit();
+        }
+        p->gather_filled[h] = sch.gather_filled;
+        p->scatter_filled[h] = sch.scatter_filled;
+        if (std::getenv("RADON_PLAN_DEBUG")) {
+            long long rounds = 0, fast = 0, mx = 0, heavy = 0;
+            for (const ScatterCta &c : sch.scatter_ctas) {
+                rounds += c.items[0].round_count; fast += c.items[0].fast_count;
+                mx = std::max<long long>(mx, c.items[0].round_count);
+                heavy += c.partial_slot >= 0 ? 1 : 0;
+            }
+            fprintf(stderr, "schedule half=%d device=%d: scatter ctas %zu rounds %lld fast %lld max %lld partial ctas %lld jobs %zu\n",
+                    h, p->device_built[h], sch.scatter_ctas.size(), rounds, fast, mx, heavy, sch.merge_jobs.size());
+        }
         q.n_gather_ctas = (int)sch.gather_ctas.size();
         q.n_scatter_ctas = (int)sch.scatter_ctas.size();
         q.n_merge_jobs = (int)sch.merge_jobs.size();
@@ -221,13 +259,12 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         if ((rc = dev_upload(p, &q.gather_ctas, sch.gather_ctas))) return rc;
         q.n_gather_workers = (int)sch.gather_worker_begin.size() - 1;
         if ((rc = dev_upload(p, &q.gather_worker_begin, sch.gather_worker_begin))) return rc;
-        if ((rc = dev_upload(p, &q.gather_slots, sch.gather_slots))) return rc;
         if ((rc = dev_upload(p, &q.scatter_ctas, sch.scatter_ctas))) return rc;
-        if ((rc = dev_upload(p, &q.scatter_slots, sch.scatter_slots))) return rc;
         if ((rc = dev_upload(p, &q.merge_jobs, sch.merge_jobs))) return rc;
         n_partial = std::max(n_partial, sch.n_partial_slots);
         p->n_jobs = std::max(p->n_jobs, (int)sch.merge_jobs.size());
     }
+    p->schedule_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_sched).count();
     // workspaces: the first serves the device-pointer calls, all of them the host-buffer entry
     // points (copies and kernels of NWS slices overlap); allocated on first use beyond the first
     p->n_partial = n_partial;
@@ -832,6 +869,32 @@ extern "C" int radon_plan_schedule_stats(const radon_plan *p, int half,
     if (scatter_filled) *scatter_filled = p->scatter_filled[h];
     if (scatter_ctas) *scatter_ctas = p->dev.sched[h].n_scatter_ctas;
     return RADON_OK;
+}
+
+// Verifies the schedules the plan actually uses (device- or host-built): downloads the slot arrays
+// and runs the host checker on them.
+extern "C" int radon_plan_schedule_check(radon_plan *p, int half, long long *n_violations, int *device_built, double *build_ms)
+{
+    if (!p) return RADON_EINVAL;
+    const int h = half ? 1 : 0;
+    if (device_built) *device_built = p->device_built[h];
+    if (build_ms) *build_ms = p->schedule_ms;
+    if (!n_violations) return RADON_OK;
+    *n_violations = -1;
+    try {
+        Schedules sch = p->meta[h];
+        sch.gather_slots.resize((size_t)p->gather_slots[h]);
+        sch.scatter_slots.resize((size_t)p->scatter_slots[h]);
+        CUDA_TRY(cudaDeviceSynchronize());
+        if (!sch.gather_slots.empty())
+            CUDA_TRY(cudaMemcpy(sch.gather_slots.data(), p->dev.sched[h].gather_slots, sch.gather_slots.size() * sizeof(Slot), cudaMemcpyDeviceToHost));
+        if (!sch.scatter_slots.empty())
+            CUDA_TRY(cudaMemcpy(sch.scatter_slots.data(), p->dev.sched[h].scatter_slots, sch.scatter_slots.size() * sizeof(Slot), cudaMemcpyDeviceToHost));
+        *n_violations = check_schedules(p->geo, sch);
+        return *n_violations == 0 ? RADON_OK : RADON_EINVAL;
+    } catch (const std::bad_alloc &) {
+        return RADON_ENOMEM;
+    }
 }
 
 extern "C" int radon_schedule_selfcheck(int N, int n_angles, int n_det, float sigma, int W, int half,

@@ -422,6 +422,38 @@ static inline int half_k_end(const Geometry &g) { return g.n_det + ((g.n_det & 1
 static inline int scatter_k_end(const Geometry &g, bool half) { return half ? half_k_end(g) : g.n_det; }
 static inline bool scatter_k_valid(const Geometry &g, int k) { return k != g.n_det / 2; }
 
+// Items -> persistent CTAs of the gather (shared by the host and the device builder)
+void finish_gather(Schedules &out, int n_workers)
+{
+    std::stable_sort(out.gather_ctas.begin(), out.gather_ctas.end(),
+                     [](const GatherCta &x, const GatherCta &y) { return x.round_count > y.round_count; });
+    // Items -> persistent CTAs: longest processing time first onto the least loaded worker
+    // (deterministic: ties go to the lowest worker index), then grouped by worker.
+    const int P = std::max(1, n_workers);
+    std::vector<long long> load(P, 0);
+    std::vector<std::vector<GatherCta>> mine(P);
+    for (const GatherCta &c : out.gather_ctas) {
+        int w = 0;
+        for (int q = 1; q < P; ++q) if (load[q] < load[w]) w = q;
+        load[w] += c.round_count + GATHER_ITEM_COST;
+        mine[w].push_back(c);
+    }
+    out.gather_ctas.clear();
+    out.gather_worker_begin.assign(1, 0);
+    for (int w = 0; w < P; ++w) {
+        // a worker's items arrive heaviest first; interleave them heavy, light, heavy, ... so
+        // that the interpolation of a dense tile overlaps the staging of sparse ones (the
+        // copy engine runs GATHER_STAGES items ahead)
+        const std::vector<GatherCta> &m = mine[w];
+        for (size_t lo = 0, hi = m.size(); lo < hi;) {
+            out.gather_ctas.push_back(m[lo++]);
+            if (lo < hi) out.gather_ctas.push_back(m[--hi]);
+        }
+        out.gather_worker_begin.push_back((int)out.gather_ctas.size());
+    }
+}
+
+
 static void build_gather(const Geometry &g, Schedules &out, int n_workers)
 {
     const int G = g.G;
@@ -468,32 +500,7 @@ static void build_gather(const Geometry &g, Schedules &out, int n_workers)
             out.gather_ctas.push_back(c);
         }
     }
-    std::stable_sort(out.gather_ctas.begin(), out.gather_ctas.end(),
-                     [](const GatherCta &x, const GatherCta &y) { return x.round_count > y.round_count; });
-    // Items -> persistent CTAs: longest processing time first onto the least loaded worker
-    // (deterministic: ties go to the lowest worker index), then grouped by worker.
-    const int P = std::max(1, n_workers);
-    std::vector<long long> load(P, 0);
-    std::vector<std::vector<GatherCta>> mine(P);
-    for (const GatherCta &c : out.gather_ctas) {
-        int w = 0;
-        for (int q = 1; q < P; ++q) if (load[q] < load[w]) w = q;
-        load[w] += c.round_count + GATHER_ITEM_COST;
-        mine[w].push_back(c);
-    }
-    out.gather_ctas.clear();
-    out.gather_worker_begin.assign(1, 0);
-    for (int w = 0; w < P; ++w) {
-        // a worker's items arrive heaviest first; interleave them heavy, light, heavy, ... so
-        // that the interpolation of a dense tile overlaps the staging of sparse ones (the
-        // copy engine runs GATHER_STAGES items ahead)
-        const std::vector<GatherCta> &m = mine[w];
-        for (size_t lo = 0, hi = m.size(); lo < hi;) {
-            out.gather_ctas.push_back(m[lo++]);
-            if (lo < hi) out.gather_ctas.push_back(m[--hi]);
-        }
-        out.gather_worker_begin.push_back((int)out.gather_ctas.size());
-    }
+    finish_gather(out, n_workers);
 }
 
 // ---------------------------------------------------------------- scatter --------
@@ -581,9 +588,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
     {
         long long est_rounds = 0;
         for (int r = 0; r < nrect; ++r) est_rounds += (count[r + 1] - count[r] + 27) / 28;
-        const double slots = (double)std::max(1, n_workers) * SCATTER_CTAS_PER_SM * SCATTER_ITEMS;
-        round_max = (int)std::lround(1.8 * (double)est_rounds / slots);
-        round_max = std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, round_max));
+        round_max = scatter_round_limit(est_rounds, n_workers);
     }
     struct Pending { ScatterCta cta; long long work; };
     std::vector<Pending> ctas;
@@ -763,6 +768,31 @@ void build_paper_bins(const Geometry &g, int n_bins_target, PaperBins &out)
         out.bins.push_back(PaperBin{n.x0, n.y0, n.w, n.h, (int)out.entries.size(), (int)n.e.size()});
         out.entries.insert(out.entries.end(), n.e.begin(), n.e.end());
     }
+}
+
+// ---- helpers shared with the device builder (plan_device.cu) -------------------------------------
+void scatter_tile_rects(const Geometry &g, bool half, std::vector<TileRect> &tiles)
+{
+    std::vector<RowSeg> segs;
+    std::vector<RectGeom> rects;
+    std::vector<int> seg_first;
+    scatter_rects(g, half, segs, rects, seg_first);
+    tiles.clear();
+    for (const RectGeom &r : rects) tiles.push_back(TileRect{r.rx0, r.ry0, r.rw, r.rh});
+}
+
+void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1, int &scatter_k1)
+{
+    gather_k0 = half ? half_k_begin(g) : 0;
+    gather_k1 = half ? half_k_end(g) : g.n_det;
+    scatter_k1 = scatter_k_end(g, half);
+}
+
+int scatter_round_limit(long long est_rounds, int n_workers)
+{
+    const double slots = (double)std::max(1, n_workers) * SCATTER_CTAS_PER_SM * SCATTER_ITEMS;
+    const int r = (int)std::lround(1.8 * (double)est_rounds / slots);
+    return std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, r));
 }
 
 void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers)

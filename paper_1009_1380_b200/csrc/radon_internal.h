@@ -183,6 +183,12 @@ struct Schedules {
 // half == true:  Hermitian half for real images / sinograms (radon_forward, radon_adjoint).
 // n_workers: persistent CTAs of the gather (one per multiprocessor).
 void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers = 148);
+// pieces of the builder shared with the device-side builder (plan_device.cu)
+struct TileRect { int rx0, ry0, rw, rh; };
+void scatter_tile_rects(const Geometry &g, bool half, std::vector<TileRect> &tiles);   // tiles the scatter writes
+void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1, int &scatter_k1);
+int scatter_round_limit(long long est_rounds, int n_workers);    // rounds per warp before a tile is split
+void finish_gather(Schedules &out, int n_workers);               // gather items -> persistent CTAs
 // Returns the number of violated invariants (0 = schedules are valid).
 long long check_schedules(const Geometry &g, const Schedules &s);
 
