@@ -55,7 +55,11 @@ struct ColCfg {
 };
 
 // ---- F1 + first half of F2 ------------------------------------------------------------------
-template <int L>
+// S2: sigma = 2 exactly (L == 2 N, N even).  Then element t + i TF of a zero-padded line is inside
+// the image for i = 0..3 and 12..15 and exactly zero for i = 4..11, whatever t: the zero inputs of
+// the first radix-16 pass (forward) and the unused outputs of the last one (inverse) are known at
+// compile time and the butterflies that only move zeros / unused values are never generated.
+template <int L, bool S2>
 __global__ void __launch_bounds__(ColCfg<L>::THREADS)
 colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod,
                    float2 *__restrict__ T, const float2 *__restrict__ tw, int N)
@@ -104,7 +108,8 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const int iy = (t + i * TF + c) & (L - 1);         // zero padding pruned: rows >= N were never staged
-        v[i] = (live && iy < N) ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
+        if (S2) v[i] = (i < 4 || i >= 12) ? (live ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f)) : make_float2(0.f, 0.f);
+        else v[i] = (live && iy < N) ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
     }
     __syncthreads();
     fft_reg<L, -1>(v, s, tw, t);
@@ -131,7 +136,7 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
 }
 
 // ---- second half of F2: rows ky = 0..L/2 of T -> centred grid rows ky and -ky ----------------
-template <int L>
+template <int L, bool S2>
 __global__ void __launch_bounds__(FftCfg<L>::THREADS)
 rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
                    const float2 *__restrict__ tw, int N, int mirror)
@@ -149,7 +154,8 @@ rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const int ix = (t + i * TF + c) & (L - 1);
-        v[i] = (live && ix < N) ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f);
+        if (S2) v[i] = (i < 4 || i >= 12) ? (live ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f)) : make_float2(0.f, 0.f);
+        else v[i] = (live && ix < N) ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f);
     }
     fft_reg<L, -1>(v, s, tw, t);
     if (!live) return;
@@ -221,7 +227,7 @@ struct RowStageCfg {
     static constexpr size_t SMEM = C::SMEM + STAGE_BYTES;
 };
 
-template <int L>
+template <int L, bool S2>
 __global__ void __launch_bounds__(FftCfg<L>::THREADS, (FftCfg<L>::THREADS <= 256) ? 3 : 1)
 rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
                           const float2 *__restrict__ tw, int N, int n_groups)
@@ -272,14 +278,15 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
                 const int ix = (t + i * TF + c) & (L - 1);
-                if (ix < N) T[(size_t)ky * N + ix] = v[i];
+                if (S2) { if (i < 4 || i >= 12) T[(size_t)ky * N + ix] = v[i]; }
+                else if (ix < N) T[(size_t)ky * N + ix] = v[i];
             }
         }
     }
 }
 
 // ---- second half of A3 + A4: column pairs of T -> image ---------------------------------------
-template <int L>
+template <int L, bool S2>
 __global__ void __launch_bounds__(ColCfg<L>::THREADS)
 colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapod,
                    float *x, const float2 *__restrict__ tw, int N, int update, float alpha, float tau)
@@ -329,7 +336,8 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
     fft_reg<L, +1>(v, s, tw, t);
     __syncthreads();
 #pragma unroll
-    for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
+    for (int i = 0; i < 16; ++i)
+        if (!S2 || i < 4 || i >= 12) s[FFT_PAD(t + i * TF)] = v[i];       // S2: the other rows are cropped
     __syncthreads();
     if (ixc < N) {   // cooperative store: thread -> (row iy, pair fc); crop, de-apodise
         const bool has_b = ixc + 1 < N;
@@ -367,14 +375,25 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
     const int N = p.N;
     const int col_blocks = ((N + 1) / 2 + CC::NFC - 1) / CC::NFC, row_blocks = (L / 2 + 1 + C::NF - 1) / C::NF;
     const float2 *tw = p.tw_G;
+    const bool s2 = (L == 2 * N) && (N % 2 == 0) && L >= 64;      // sigma = 2: pruned first / last radix-16 pass
     switch (which) {
     case 0:
-        if (set_smem(colpass_fwd_kernel<L>, CC::SMEM)) return -1;
-        colpass_fwd_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+        if (s2) {
+            if (set_smem(colpass_fwd_kernel<L, true>, CC::SMEM)) return -1;
+            colpass_fwd_kernel<L, true><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+        } else {
+            if (set_smem(colpass_fwd_kernel<L, false>, CC::SMEM)) return -1;
+            colpass_fwd_kernel<L, false><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+        }
         break;
     case 1:
-        if (set_smem(rowpass_fwd_kernel<L>, C::SMEM)) return -1;
-        rowpass_fwd_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+        if (s2) {
+            if (set_smem(rowpass_fwd_kernel<L, true>, C::SMEM)) return -1;
+            rowpass_fwd_kernel<L, true><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+        } else {
+            if (set_smem(rowpass_fwd_kernel<L, false>, C::SMEM)) return -1;
+            rowpass_fwd_kernel<L, false><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+        }
         break;
     case 2:
         if (flag) {
@@ -382,16 +401,27 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
             rowpass_inv_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
         } else {
             using RS = RowStageCfg<L>;
-            if (set_smem(rowpass_inv_staged_kernel<L>, RS::SMEM)) return -1;
             const int per_sm = std::max(1, std::min(8, (int)((220u << 10) / (RS::SMEM + 1024))));
             const int ctas = std::min(row_blocks, p.n_sm * per_sm);
-            rowpass_inv_staged_kernel<L><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+            if (s2) {
+                if (set_smem(rowpass_inv_staged_kernel<L, true>, RS::SMEM)) return -1;
+                rowpass_inv_staged_kernel<L, true><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+            } else {
+                if (set_smem(rowpass_inv_staged_kernel<L, false>, RS::SMEM)) return -1;
+                rowpass_inv_staged_kernel<L, false><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+            }
         }
         break;
     case 3:
-        if (set_smem(colpass_inv_kernel<L>, CC::SMEM)) return -1;
-        colpass_inv_kernel<L><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
-                                                                           upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
+        if (s2) {
+            if (set_smem(colpass_inv_kernel<L, true>, CC::SMEM)) return -1;
+            colpass_inv_kernel<L, true><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
+                                                                                     upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
+        } else {
+            if (set_smem(colpass_inv_kernel<L, false>, CC::SMEM)) return -1;
+            colpass_inv_kernel<L, false><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
+                                                                                      upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
+        }
         break;
     default:
         return -1;
