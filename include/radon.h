@@ -109,6 +109,12 @@ int radon_adjoint_batch(radon_plan *p, const float *d_sino, float *d_x, int batc
 int radon_forward_host(radon_plan *p, const float *h_x, float *h_sino, int batch);
 int radon_adjoint_host(radon_plan *p, const float *h_sino, float *h_x, int batch);
 
+/* Both operators in one call, per slice: h_sino = Radon{h_x} and h_xt = Radon^T{h_sino} (the product
+ * a solver's gradient step needs).  The sinogram is not uploaded again, and because every slice has
+ * one upload and two downloads on its own lane, uploads and downloads of neighbouring slices use
+ * both PCIe directions at once.  Synchronous like the calls above.  h_xt: batch*N*N fp32. */
+int radon_forward_adjoint_host(radon_plan *p, const float *h_x, float *h_sino, float *h_xt, int batch);
+
 /* Bare NUFFT (type 2): image -> M = n_angles*n_det complex polar samples
  * F[a,k] (de-apodise + zero-pad, 2-D FFT, inverse gridding).  d_polar: 2*M floats. */
 int radon_nufft2(radon_plan *p, const float *d_x, float *d_polar, void *stream);

@@ -20,6 +20,7 @@ _SIGNATURES = {
     "radon_adjoint_batch": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "radon_forward_host": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "radon_adjoint_host": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
+    "radon_forward_adjoint_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_int]),
     "radon_nufft2": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_nufft1": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_interp_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -338,6 +339,16 @@ class RadonPlan:
         assert h_x.numel() == b * self.N * self.N and h_sino.numel() == b * self.M
         _check(lib().radon_adjoint_host(self._h, _ptr(h_sino), _ptr(h_x), b), "radon_adjoint_host")
         return h_x
+
+    def radon_forward_adjoint_host(self, h_x, h_sino, h_xt):
+        """h_sino = A h_x and h_xt = A^T h_sino per slice; CPU float32 tensors (pinned for overlap)."""
+        b = h_x.shape[0]
+        for t in (h_x, h_sino, h_xt):
+            assert (not t.is_cuda) and t.is_contiguous()
+        assert h_x.numel() == b * self.N * self.N == h_xt.numel() and h_sino.numel() == b * self.M
+        _check(lib().radon_forward_adjoint_host(self._h, _ptr(h_x), _ptr(h_sino), _ptr(h_xt), b),
+               "radon_forward_adjoint_host")
+        return h_sino, h_xt
 
     def radon_nufft2(self, x, polar=None):
         import torch

@@ -749,6 +749,31 @@ static int host_run(radon_plan *p, bool fwd, const float *h_in, float *h_out, in
     return RADON_OK;
 }
 
+// x -> (Radon{x}, Radon^T{Radon{x}}) per slice: what a solver's normal-equation / gradient step needs.
+// One upload (the image) and two downloads per slice, all on the slice's lane, so that the uploads
+// of later slices run against the downloads of earlier ones (both PCIe directions busy at once).
+extern "C" int radon_forward_adjoint_host(radon_plan *p, const float *h_x, float *h_sino, float *h_xt, int batch)
+{
+    if (!p || !h_x || !h_sino || !h_xt || batch < 0) return RADON_EINVAL;
+    int rc = host_setup(p);
+    if (rc) return rc;
+    CUDA_TRY(cudaDeviceSynchronize());              // see host_run
+    const size_t nx = (size_t)p->dev.N * p->dev.N, ns = (size_t)p->M;
+    const int lanes = p->timer.enabled ? 1 : NWS;
+    for (int b = 0; b < batch; ++b) {
+        const int i = b % lanes;
+        cudaStream_t st = p->hstream[i];
+        Workspace &w = p->ws[i];
+        CUDA_TRY(cudaMemcpyAsync(w.img, h_x + b * nx, nx * sizeof(float), cudaMemcpyHostToDevice, st));
+        if ((rc = forward_ws(p, w, w.img, w.sino, st))) return rc;
+        CUDA_TRY(cudaMemcpyAsync(h_sino + b * ns, w.sino, ns * sizeof(float), cudaMemcpyDeviceToHost, st));
+        if ((rc = adjoint_ws(p, w, w.sino, w.img, st))) return rc;
+        CUDA_TRY(cudaMemcpyAsync(h_xt + b * nx, w.img, nx * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
+    for (int i = 0; i < NWS; ++i) CUDA_TRY(cudaStreamSynchronize(p->hstream[i]));
+    return RADON_OK;
+}
+
 extern "C" int radon_forward_host(radon_plan *p, const float *h_x, float *h_sino, int batch)
 {
     return host_run(p, true, h_x, h_sino, batch);

@@ -379,3 +379,20 @@ def test_calls_can_be_captured_in_a_cuda_graph(rb):
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(s, ref_s) and torch.equal(xo, ref_x)
+
+
+def test_forward_adjoint_host_pair_call_equals_the_separate_host_calls(rb):
+    """radon_forward_adjoint_host (one upload, two downloads per slice, both PCIe directions in use)
+    returns exactly what radon_forward_host followed by radon_adjoint_host return."""
+    cfg = workloads.get_config(2)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    B = 6
+    hx = torch.from_numpy(np.stack([workloads.make_batch_slice(40 + i, cfg.N) for i in range(B)])).pin_memory()
+    hs = torch.empty((B, cfg.n_angles, cfg.n_det), dtype=torch.float32).pin_memory()
+    hxt = torch.empty((B, cfg.N, cfg.N), dtype=torch.float32).pin_memory()
+    plan.radon_forward_adjoint_host(hx, hs, hxt)
+    hs2 = torch.empty_like(hs); hxt2 = torch.empty_like(hxt)
+    plan.radon_forward_host(hx, hs2)
+    plan.radon_adjoint_host(hs2, hxt2)
+    assert torch.equal(hs, hs2) and torch.equal(hxt, hxt2)
+    plan.close()
