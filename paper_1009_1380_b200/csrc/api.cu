@@ -193,6 +193,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     DevicePlan &d = p->dev;
     d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det;
     d.n_sm = prop.multiProcessorCount;
+    d.pdl = G <= 2048;
     const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
     d.LP = pow2 ? n_det : std::max(16, next_pow2(2 * n_det - 1));
 
@@ -622,7 +623,9 @@ extern "C" int radon_solver_run(radon_plan *p, float *d_x, const float *d_b, flo
         if (!p->capture_stream) CUDA_TRY(cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking));
         CUDA_TRY(cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal));
         const long long n0 = launch_count();
+        pdl_suppress(true);
         rc = solver_step_on(p, d_x, d_b, alpha, tau, filtered, p->capture_stream);
+        pdl_suppress(false);
         g.kernels = launch_count() - n0;
         count_launch(-g.kernels);                       // captured, not launched
         cudaGraph_t graph = nullptr;

@@ -65,6 +65,7 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
                    float2 *__restrict__ T, const float2 *__restrict__ tw, int N)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    pdl_prologue();
     using C = ColCfg<L>;
     constexpr int TF = C::TF, NFC = C::NFC;
     const int c = N / 2;
@@ -116,6 +117,7 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
+    pdl_trigger();
     __syncthreads();
     {   // cooperative store: thread -> (ky, pair fc); untangle the packed pair:
         // A[k] = (Z[k] + conj Z[-k])/2, B[k] = (Z[k] - conj Z[-k])/(2i), k = 0..L/2
@@ -142,6 +144,7 @@ rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
                    const float2 *__restrict__ tw, int N, int mirror)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    pdl_prologue();
     using C = FftCfg<L>;
     constexpr int TF = C::TF;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -158,6 +161,7 @@ rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
         else v[i] = (live && ix < N) ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f);
     }
     fft_reg<L, -1>(v, s, tw, t);
+    pdl_trigger();
     if (!live) return;
     const int cy = (ky + L / 2) & (L - 1);
     float2 *row = grid + (size_t)cy * L;
@@ -183,6 +187,7 @@ rowpass_inv_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
                    const float2 *__restrict__ tw, int N, int fold)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    pdl_prologue();
     using C = FftCfg<L>;
     constexpr int TF = C::TF;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -207,6 +212,7 @@ rowpass_inv_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
         }
     }
     fft_reg<L, +1>(v, s, tw, t);
+    pdl_trigger();
     if (!live) return;
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
@@ -233,6 +239,7 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
                           const float2 *__restrict__ tw, int N, int n_groups)
 {
     extern __shared__ __align__(128) float2 s_rows[];   // FFT scratch, then the staged rows
+    pdl_prologue();
     using C = FftCfg<L>;
     constexpr int TF = C::TF, NF = C::NF;
     __shared__ __align__(8) uint64_t bar;
@@ -273,6 +280,7 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();                                    // stage is free; s is free (previous FFT done)
         if (threadIdx.x == 0 && g + (int)gridDim.x < n_groups) fetch(g + gridDim.x);
+        if (g + (int)gridDim.x >= n_groups) pdl_trigger();      // this CTA's last group
         fft_reg<L, +1>(v, s, tw, t);
         if (live) {
 #pragma unroll
@@ -292,6 +300,7 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
                    float *x, const float2 *__restrict__ tw, int N, int update, float alpha, float tau)
 {
     extern __shared__ __align__(16) float2 s_fft[];
+    pdl_prologue();
     using C = ColCfg<L>;
     constexpr int TF = C::TF, NFC = C::NFC;
     const int c = N / 2;
@@ -338,6 +347,7 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
 #pragma unroll
     for (int i = 0; i < 16; ++i)
         if (!S2 || i < 4 || i >= 12) s[FFT_PAD(t + i * TF)] = v[i];       // S2: the other rows are cropped
+    pdl_trigger();
     __syncthreads();
     if (ixc < N) {   // cooperative store: thread -> (row iy, pair fc); crop, de-apodise
         const bool has_b = ixc + 1 < N;
@@ -380,46 +390,46 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
     case 0:
         if (s2) {
             if (set_smem(colpass_fwd_kernel<L, true>, CC::SMEM)) return -1;
-            colpass_fwd_kernel<L, true><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+            launch_pdl(p.pdl, colpass_fwd_kernel<L, true>, col_blocks, CC::THREADS, CC::SMEM, st, (const float *)in, p.deapod, (float2 *)out, tw, N);
         } else {
             if (set_smem(colpass_fwd_kernel<L, false>, CC::SMEM)) return -1;
-            colpass_fwd_kernel<L, false><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float *)in, p.deapod, (float2 *)out, tw, N);
+            launch_pdl(p.pdl, colpass_fwd_kernel<L, false>, col_blocks, CC::THREADS, CC::SMEM, st, (const float *)in, p.deapod, (float2 *)out, tw, N);
         }
         break;
     case 1:
         if (s2) {
             if (set_smem(rowpass_fwd_kernel<L, true>, C::SMEM)) return -1;
-            rowpass_fwd_kernel<L, true><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+            launch_pdl(p.pdl, rowpass_fwd_kernel<L, true>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag);
         } else {
             if (set_smem(rowpass_fwd_kernel<L, false>, C::SMEM)) return -1;
-            rowpass_fwd_kernel<L, false><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+            launch_pdl(p.pdl, rowpass_fwd_kernel<L, false>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag);
         }
         break;
     case 2:
         if (flag) {
             if (set_smem(rowpass_inv_kernel<L>, C::SMEM)) return -1;
-            rowpass_inv_kernel<L><<<row_blocks, C::THREADS, C::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, flag);
+            launch_pdl(p.pdl, rowpass_inv_kernel<L>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag);
         } else {
             using RS = RowStageCfg<L>;
             const int per_sm = std::max(1, std::min(8, (int)((220u << 10) / (RS::SMEM + 1024))));
             const int ctas = std::min(row_blocks, p.n_sm * per_sm);
             if (s2) {
                 if (set_smem(rowpass_inv_staged_kernel<L, true>, RS::SMEM)) return -1;
-                rowpass_inv_staged_kernel<L, true><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+                launch_pdl(p.pdl, rowpass_inv_staged_kernel<L, true>, ctas, C::THREADS, RS::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, row_blocks);
             } else {
                 if (set_smem(rowpass_inv_staged_kernel<L, false>, RS::SMEM)) return -1;
-                rowpass_inv_staged_kernel<L, false><<<ctas, C::THREADS, RS::SMEM, st>>>((const float2 *)in, (float2 *)out, tw, N, row_blocks);
+                launch_pdl(p.pdl, rowpass_inv_staged_kernel<L, false>, ctas, C::THREADS, RS::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, row_blocks);
             }
         }
         break;
     case 3:
         if (s2) {
             if (set_smem(colpass_inv_kernel<L, true>, CC::SMEM)) return -1;
-            colpass_inv_kernel<L, true><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
+            launch_pdl(p.pdl, colpass_inv_kernel<L, true>, col_blocks, CC::THREADS, CC::SMEM, st, (const float2 *)in, p.deapod, (float *)out, tw, N,
                                                                                      upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
         } else {
             if (set_smem(colpass_inv_kernel<L, false>, CC::SMEM)) return -1;
-            colpass_inv_kernel<L, false><<<col_blocks, CC::THREADS, CC::SMEM, st>>>((const float2 *)in, p.deapod, (float *)out, tw, N,
+            launch_pdl(p.pdl, colpass_inv_kernel<L, false>, col_blocks, CC::THREADS, CC::SMEM, st, (const float2 *)in, p.deapod, (float *)out, tw, N,
                                                                                       upd ? 1 : 0, upd ? upd->alpha : 0.f, upd ? upd->tau : 0.f);
         }
         break;

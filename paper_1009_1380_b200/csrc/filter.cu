@@ -19,6 +19,7 @@ __global__ void __launch_bounds__(FROW_THREADS)
 filter_rows_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ q, int n, int hi)
 {
     __shared__ float part[FROW_THREADS / 32][FILTER_MAXQ];
+    pdl_prologue();
     const float *z = in + (size_t)blockIdx.x * n;
     float c[FILTER_MAXQ];
 #pragma unroll
@@ -53,6 +54,7 @@ filter_rows_kernel(const float *__restrict__ in, float *__restrict__ out, const 
         for (int w = 0; w < FROW_THREADS / 32; ++w) a += part[w][d];        // fixed order
         c[d] = a;
     }
+    pdl_trigger();
     float *o_row = out + (size_t)blockIdx.x * n;
     for (int s = threadIdx.x; s < n; s += FROW_THREADS) {
         const float4 qa = __ldg(reinterpret_cast<const float4 *>(q + (size_t)s * FILTER_MAXQ));
@@ -72,6 +74,7 @@ filter_cols_kernel(const float *__restrict__ in, float *__restrict__ out, const 
                    int n_cols, int n_rows, int hi)
 {
     __shared__ float part[FCOL_PARTS][FILTER_MAXQ][FCOL_COLS + 1];
+    pdl_prologue();
     const int lc = threadIdx.x % FCOL_COLS, pr = threadIdx.x / FCOL_COLS;
     const int col = blockIdx.x * FCOL_COLS + lc;
     const bool live = col < n_cols;
@@ -103,6 +106,7 @@ filter_cols_kernel(const float *__restrict__ in, float *__restrict__ out, const 
         for (int p = 0; p < FCOL_PARTS; ++p) s += part[p][d][lc];     // fixed order
         c[d] = s;
     }
+    pdl_trigger();
     if (!live) return;
     for (int a = pr; a < n_rows; a += FCOL_PARTS) {
         const float4 qa = __ldg(reinterpret_cast<const float4 *>(q + (size_t)a * FILTER_MAXQ));
@@ -117,9 +121,9 @@ filter_cols_kernel(const float *__restrict__ in, float *__restrict__ out, const 
 int launch_filter(const DevicePlan &p, int axis, const float *q, int order, const float *in, float *out, cudaStream_t st)
 {
     if (axis == 0)
-        filter_rows_kernel<<<p.n_angles, FROW_THREADS, 0, st>>>(in, out, q, p.n_det, order > 3 ? 1 : 0);
+        launch_pdl(p.pdl, filter_rows_kernel, p.n_angles, FROW_THREADS, 0, st, in, out, q, p.n_det, order > 3 ? 1 : 0);
     else
-        filter_cols_kernel<<<(p.n_det + FCOL_COLS - 1) / FCOL_COLS, FCOL_COLS * FCOL_PARTS, 0, st>>>(in, out, q, p.n_det, p.n_angles, order > 3 ? 1 : 0);
+        launch_pdl(p.pdl, filter_cols_kernel, (p.n_det + FCOL_COLS - 1) / FCOL_COLS, FCOL_COLS * FCOL_PARTS, 0, st, in, out, q, p.n_det, p.n_angles, order > 3 ? 1 : 0);
     count_launch();
     return 0;
 }

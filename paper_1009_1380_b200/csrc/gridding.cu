@@ -11,12 +11,20 @@
 #include "taps.cuh"
 
 #include <atomic>
+#include <cstdlib>
 
 namespace radon {
 
 static std::atomic<long long> g_launches{0};
 long long launch_count() { return g_launches.load(); }
 void count_launch(long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+static thread_local bool g_pdl_suppressed = false;
+void pdl_suppress(bool on) { g_pdl_suppressed = on; }
+bool pdl_enabled()
+{
+    static const bool on = [] { const char *e = std::getenv("RADON_PDL"); return !(e && e[0] == '0'); }();
+    return on && !g_pdl_suppressed;
+}
 
 // =====================================================================================
 // F3: inverse gridding (gather)
@@ -60,6 +68,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full[GATHER_STAGES], empty[GATHER_STAGES];
+    pdl_prologue();
 
     const int it_begin = worker_begin[blockIdx.x], it_end = worker_begin[blockIdx.x + 1];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -177,6 +186,7 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             p2 = norm(Pos{p2.it, p2.r + GATHER_WARPS});
             sl = nx; nx = nn; d = dn;
         }
+        if (it + 1 == it_end) pdl_trigger();            // the CTA's last item is done
         // generic-proxy reads of the tile must be ordered before the async-proxy refill
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();                       // every lane has read its taps of this tile
@@ -493,6 +503,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *acc = reinterpret_cast<float2 *>(smem_raw);
     __shared__ int s_flag;
+    pdl_prologue();
     if (blockIdx.x == 0) {
         // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
         // footprint of the sum is added by the merge of the centre rectangles (DESIGN.md R-tie)
@@ -580,6 +591,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         v0 = v1; v1 = v2; d0 = d1; d1 = d2;
     }
 
+    pdl_trigger();
     // flush: the rectangle is written exactly once, by the copy engine
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> async proxy
     __syncthreads();
@@ -613,7 +625,7 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     if (q.n_gather_ctas == 0) return 0;
-    gather_kernel<<<q.n_gather_workers, GATHER_THREADS, GATHER_SMEM, st>>>(
+    launch_pdl(p.pdl, gather_kernel, q.n_gather_workers, GATHER_THREADS, GATHER_SMEM, st,
         grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.kb, p.G, p.n_det);
     count_launch();
     return 0;
@@ -628,7 +640,7 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
     dcj.n = q.n_dc_jobs;
     for (int i = 0; i < MAX_DC_JOBS; ++i) dcj.job[i] = q.dc_jobs[i];
     // CTA 0 sums the j = 0 samples; CTA b > 0 grids scatter_ctas[b - 1] (heaviest first)
-    scatter_kernel<<<q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st>>>(
+    launch_pdl(p.pdl, scatter_kernel, q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st,
         polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.kb, p.G, p.n_det, nyq,
         dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);
     count_launch();

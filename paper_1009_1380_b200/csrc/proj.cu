@@ -104,6 +104,7 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
 {
     extern __shared__ __align__(16) float2 s_fft[];
     __shared__ float s_red[FILT ? PROJ_RED_FLOATS : 1];
+    pdl_prologue();
     using C = ProjCfg<L>;
     constexpr int TF = C::TF;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -154,6 +155,7 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
         __syncthreads();
         fft_reg<L, +1>(v, s, tw, t);
     }
+    pdl_trigger();
     if constexpr (INV) {
         float z[1][16];
 #pragma unroll
@@ -209,6 +211,7 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
 {
     extern __shared__ __align__(16) float2 s_fft[];
     __shared__ float s_red[FILT ? PROJ_RED_FLOATS : 1];
+    pdl_prologue();
     using C = ProjCfg<L>;
     constexpr int TF = C::TF, n = L, c = L / 2;
     const int f = threadIdx.x / TF, t = threadIdx.x - f * TF;
@@ -255,6 +258,7 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
         }
     }
     fft_reg<L, -1>(v, s, tw, t);
+    pdl_trigger();
     if (INV) {
         float z[2][16];
 #pragma unroll
@@ -311,14 +315,14 @@ static int proj_launch(bool inv, bool half, const DevicePlan &p, const float *in
 #define RADON_PROJ(INV_, BLUE_, FILT_)                                                                   \
     {                                                                                                    \
         if (set_smem(proj_kernel<L, INV_, BLUE_, FILT_>, C::SMEM)) return -1;                            \
-        proj_kernel<L, INV_, BLUE_, FILT_><<<blocks, C::THREADS, C::SMEM, st>>>(                         \
+        launch_pdl(p.pdl, proj_kernel<L, INV_, BLUE_, FILT_>, blocks, C::THREADS, C::SMEM, st,                  \
             in, out, p.chirp_a, p.chirp_b, p.chirp_hf, p.tw_P, p.n_det, p.n_angles, half ? 1 : 0, dens,  \
             ex.sub, ex.q);                                                                               \
     }
 #define RADON_PROJ_PAIR(INV_, FILT_)                                                                     \
     {                                                                                                    \
         if (set_smem(proj_pair_kernel<L, INV_, FILT_>, C::SMEM)) return -1;                              \
-        proj_pair_kernel<L, INV_, FILT_><<<pair_blocks, C::THREADS, C::SMEM, st>>>(                      \
+        launch_pdl(p.pdl, proj_pair_kernel<L, INV_, FILT_>, pair_blocks, C::THREADS, C::SMEM, st,               \
             in, out, p.chirp_a, p.chirp_b, p.tw_P, p.n_angles, dens, ex.sub, ex.q);                      \
     }
     const bool blue = p.chirp_hf != nullptr;
