@@ -470,11 +470,12 @@ def main():
     del p3
     # filter(Radon{x}) against Radon{x} at config 4 (the filter runs in the epilogue of the F4 kernel)
     xf, sf = x[0], sino[0]
+    sf_out = torch.empty_like(sf)
     ft = {}
     for label, fn in (("radon_forward", lambda: plan.radon_forward(xf, sf)),
                       ("radon_forward_filtered", lambda: plan.radon_forward_filtered(xf, sf)),
-                      ("radon_filter_axis0", lambda: plan.radon_filter(sf, out=sino[1], axis=0)),
-                      ("radon_filter_axis1", lambda: plan.radon_filter(sf, out=sino[1], axis=1))):
+                      ("radon_filter_axis0", lambda: plan.radon_filter(sf, out=sf_out, axis=0)),
+                      ("radon_filter_axis1", lambda: plan.radon_filter(sf, out=sf_out, axis=1))):
         for _ in range(3):
             fn()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -139,7 +139,7 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
 
 // ---- second half of F2: rows ky = 0..L/2 of T -> centred grid rows ky and -ky ----------------
 template <int L, bool S2>
-__global__ void __launch_bounds__(FftCfg<L>::THREADS)
+__global__ void __launch_bounds__(FftCfg<L>::THREADS, (FftCfg<L>::THREADS <= 256) ? 1024 / FftCfg<L>::THREADS : 1)   // 64 registers: four CTAs of 256
 rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
                    const float2 *__restrict__ tw, int N, int mirror)
 {
