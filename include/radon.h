@@ -172,10 +172,14 @@ int radon_plan_info(const radon_plan *p, int *N, int *G, int *n_angles, int *n_d
  * eq. :89 (sum over all polar samples, K the Kaiser-Bessel kernel on the oversampled grid),
  * followed by the 2-D inverse FFT, crop and de-apodisation.  scale = n_det phihat(0)^2 / G^2
  * turns D into an area element of the Fourier plane.  D is a plan
- * constant, derived in fp64 on the host at the first call (a second or two at 2048^2).
+ * constant, derived in fp64 by a CUDA kernel (one thread per sample) at the first call, which blocks
+ * for it (tens of ms at 2048^2); radon_plan_prepare_inverse does that ahead of time.
  * d_sino: n_angles*n_det fp32 (device), d_x: N*N fp32 (device, written).  Asynchronous on
- * `stream` after the first call.  Returns RADON_OK or a negative code as radon_adjoint. */
+ * `stream` after the first call (from the first one after radon_plan_prepare_inverse, which also makes
+ * it capturable in a CUDA graph).  Returns RADON_OK or a negative code as radon_adjoint. */
 int radon_inverse(radon_plan *p, const float *d_sino, float *d_x, void *cuda_stream);
+/* Builds the density table of radon_inverse now (blocking; no-op when it exists). */
+int radon_plan_prepare_inverse(radon_plan *p);
 
 /* D * scale as the plan uses it (M = n_angles*n_det floats, HOST pointer, may be NULL) and
  * scale (may be NULL).  Builds D if the plan has not done so yet. */

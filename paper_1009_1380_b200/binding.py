@@ -38,6 +38,7 @@ _SIGNATURES = {
     "radon_schedule_host_stats": (c_int, [c_int, c_int, c_int, c_float, c_int, c_int, P(c_ll)]),
     "radon_kb_weights_host": (c_int, [c_int, c_float, c_float, P(c_float)]),
     "radon_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_plan_prepare_inverse": (c_int, [c_void_p]),
     "radon_plan_density": (c_int, [c_void_p, c_void_p, P(ctypes.c_double)]),
     "radon_density_host": (c_int, [c_int, c_int, c_int, c_float, c_int, c_void_p, P(ctypes.c_double)]),
     "radon_plan_set_filter": (c_int, [c_void_p, c_int]),
@@ -295,6 +296,9 @@ class RadonPlan:
         _check(lib().radon_solver_run(self._h, _ptr(x), _ptr(b), float(alpha), float(tau), int(filtered), int(n_iter),
                                       self._stream()), "radon_solver_run")
         return x
+
+    def prepare_inverse(self):
+        _check(lib().radon_plan_prepare_inverse(self._h), "radon_plan_prepare_inverse")
 
     def density(self):
         """(D * scale as a CPU float32 tensor of shape (n_angles, n_det), scale)."""

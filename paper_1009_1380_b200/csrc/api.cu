@@ -3,6 +3,7 @@
 #include "../../include/radon.h"
 
 #include <chrono>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -430,10 +431,25 @@ extern "C" int radon_adjoint(radon_plan *p, const float *d_sino, float *d_x, voi
 static int density_setup(radon_plan *p)
 {
     if (p->dev_density) return RADON_OK;
-    std::vector<float> D;
+    // D of eq. :89 on the device (plan_device.cu: one thread per sample, neighbours from the geometry,
+    // fp64), downloaded once for radon_plan_density; RADON_PLAN_BUILDER=host builds it on the host.
+    const int n = p->dev.n_det, na = p->dev.n_angles, W = p->geo.W;
+    const double beta = kb_beta(W, p->geo.sigma), inv = 1.0 / kb_i0(beta);
+    const double ph0 = (double)W * inv * std::sinh(beta) / beta;           // phihat(0): the integral of the kernel
+    const double scale = (double)n * ph0 * ph0 / ((double)p->dev.G * (double)p->dev.G);
+    const char *builder_env = std::getenv("RADON_PLAN_BUILDER");
+    int rc;
     try {
-        build_density(p->geo, p->host_density, &p->density_scale);
-        D = p->host_density;
+        if (builder_env && std::strcmp(builder_env, "host") == 0) {
+            build_density(p->geo, p->host_density, &p->density_scale);
+            if ((rc = dev_upload(p, &p->dev_density, p->host_density))) return rc;
+        } else {
+            if ((rc = dev_alloc(p, &p->dev_density, (size_t)p->M))) return rc;
+            if (launch_density(p->dev.cs, na, n, beta, inv, scale, p->dev_density, 0)) return RADON_ECUDA;
+            p->host_density.resize((size_t)p->M);
+            CUDA_TRY(cudaMemcpy(p->host_density.data(), p->dev_density, (size_t)p->M * sizeof(float), cudaMemcpyDeviceToHost));
+            p->density_scale = scale;
+        }
     } catch (const std::bad_alloc &) {
         return RADON_ENOMEM;
     }
@@ -442,16 +458,17 @@ static int density_setup(radon_plan *p)
     // carry the same weight.  For odd n_det the sample set is point symmetric and D_j == D_-j;
     // for even n_det j = -n/2 has no partner and D_j != D_-j near the band edge.  The real part
     // only ever sees the pair sum (D_j + D_-j) Re{Yh_j e}, so giving both the mean is exact.
-    const int n = p->dev.n_det;
-    if ((n & 1) == 0)
-        for (int a = 0; a < p->dev.n_angles; ++a) {
-            float *row = D.data() + (size_t)a * n;
-            for (int k = 1; k < n / 2; ++k) {
-                const float m = 0.5f * (row[k] + row[n - k]);
-                row[k] = m; row[n - k] = m;
-            }
-        }
-    return dev_upload(p, &p->dev_density, D);
+    if (launch_density_pair_mean(p->dev_density, na, n, 0)) return RADON_ECUDA;
+    CUDA_TRY(cudaDeviceSynchronize());
+    return RADON_OK;
+}
+
+// The blocking part of radon_inverse (the density table) done ahead of time, so that radon_inverse
+// is asynchronous -- and capturable in a CUDA graph -- from its first call.
+extern "C" int radon_plan_prepare_inverse(radon_plan *p)
+{
+    if (!p) return RADON_EINVAL;
+    return density_setup(p);
 }
 
 extern "C" int radon_inverse(radon_plan *p, const float *d_sino, float *d_x, void *stream)

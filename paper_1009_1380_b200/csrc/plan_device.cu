@@ -536,3 +536,98 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
 }
 
 }  // namespace radon
+
+// ---- density compensation of the inverse Radon transform on the device ---------------
+// D(x_i, y_i) = scale / sum_j K(x_i - x_j, y_i - y_j), the sum over ALL polar samples, K = phi(dx) phi(dy).
+// One thread per sample i.  Its neighbours are found from the geometry: only radial lines that pass
+// within W/2 sqrt 2 of the sample can hold one (all lines near the centre, a window of angles
+// further out), and on a line the samples inside the W x W box are an interval of j (as in
+// for_candidates).  phi is evaluated in fp64 from the series of I0; the terms are added in a fixed
+// order.  Checked against the host table (build_density) to fp32 round-off.
+namespace radon {
+
+__device__ __forceinline__ double i0_series(double z)
+{
+    const double q = 0.25 * z * z;
+    double term = 1.0, sum = 1.0;
+    for (int m = 1; m < 200; ++m) {
+        term *= q / ((double)m * (double)m);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+
+__device__ __forceinline__ double kb_phi_dev(double u, double beta, double inv_i0b)
+{
+    const double t = 2.0 * u / (double)KW, arg = 1.0 - t * t;
+    if (arg < 0.0) return (arg > -1e-12) ? inv_i0b : 0.0;       // |u| == W/2 up to rounding
+    return i0_series(beta * sqrt(arg)) * inv_i0b;
+}
+
+__global__ void __launch_bounds__(128)
+density_kernel(float *__restrict__ D, const double2 *__restrict__ cs, int n_angles, int n_det, double beta,
+               double inv_i0b, double scale)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_angles * n_det) return;
+    const int a = (int)(i / n_det), k = (int)(i - (long long)a * n_det), cd = n_det / 2;
+    const double2 d = cs[a];
+    const double kx = (double)(k - cd) * d.x, ky = (double)(k - cd) * d.y, hw = 0.5 * KW;
+    const double r = sqrt(kx * kx + ky * ky);
+    // lines that can come within hw * sqrt(2) of the sample: |sin(theta' - theta)| <= hw sqrt 2 / r
+    int win = n_angles;                                         // offsets -win .. +win (all lines when >= n_angles / 2)
+    const double reach = hw * 1.4142135623730951 + 1e-6;
+    if (r > reach) win = (int)ceil(asin(reach / r) / (3.14159265358979323846 / (double)n_angles)) + 1;
+    const bool all = 2 * win + 1 >= n_angles;
+    const int o_lo = all ? 0 : -win, o_hi = all ? n_angles - 1 : win;
+    double sum = 0.0;
+    for (int o = o_lo; o <= o_hi; ++o) {
+        int a2 = all ? o : (a + o) % n_angles;
+        if (a2 < 0) a2 += n_angles;
+        const double2 e = cs[a2];
+        // j e in [kappa - hw, kappa + hw] on both axes: an interval of j
+        double lo = -(double)cd - 0.5, hi = (double)(n_det - 1 - cd) + 0.5;
+        if (fabs(e.x) > 1e-12) { const double u = (kx - hw) / e.x, v = (kx + hw) / e.x; lo = fmax(lo, fmin(u, v) - 1e-6); hi = fmin(hi, fmax(u, v) + 1e-6); }
+        else if (fabs(kx) > hw + 1e-9) continue;
+        if (fabs(e.y) > 1e-12) { const double u = (ky - hw) / e.y, v = (ky + hw) / e.y; lo = fmax(lo, fmin(u, v) - 1e-6); hi = fmin(hi, fmax(u, v) + 1e-6); }
+        else if (fabs(ky) > hw + 1e-9) continue;
+        for (int j = (int)ceil(lo); j <= (int)floor(hi); ++j) {
+            const double px = kb_phi_dev(kx - (double)j * e.x, beta, inv_i0b);
+            if (px != 0.0) sum += px * kb_phi_dev(ky - (double)j * e.y, beta, inv_i0b);
+        }
+    }
+    D[i] = (float)(scale / sum);
+}
+
+// even n_det: the Hermitian-half scatter needs the mean weight of every +-j pair
+__global__ void density_pair_mean_kernel(float *__restrict__ D, int n_angles, int n_det)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int half = n_det / 2 - 1;                             // pairs k = 1 .. n/2 - 1 with n - k
+    if (half <= 0 || i >= (long long)n_angles * half) return;
+    const int a = (int)(i / half), k = 1 + (int)(i - (long long)a * half);
+    float *row = D + (size_t)a * n_det;
+    const float m = 0.5f * (row[k] + row[n_det - k]);
+    row[k] = m; row[n_det - k] = m;
+}
+
+int launch_density(const double2 *d_cs, int n_angles, int n_det, double beta, double inv_i0b, double scale,
+                   float *d_D, cudaStream_t st)
+{
+    const long long M = (long long)n_angles * n_det;
+    density_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(d_D, d_cs, n_angles, n_det, beta, inv_i0b, scale);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int launch_density_pair_mean(float *d_D, int n_angles, int n_det, cudaStream_t st)
+{
+    const long long n = (long long)n_angles * (n_det / 2 - 1);
+    if ((n_det & 1) || n <= 0) return 0;
+    density_pair_mean_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_D, n_angles, n_det);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace radon

@@ -51,4 +51,10 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
                            Slot **d_gather_slots, long long *n_gather_rounds,
                            Slot **d_scatter_slots, long long *n_scatter_rounds);
 
+// Density compensation D of PAPER.md:89 times `scale`, one thread per sample (plan_device.cu); and the
+// pair mean the Hermitian-half scatter needs for even n_det (in place).
+int launch_density(const double2 *d_cs, int n_angles, int n_det, double beta, double inv_i0b, double scale,
+                   float *d_D, cudaStream_t st);
+int launch_density_pair_mean(float *d_D, int n_angles, int n_det, cudaStream_t st);
+
 }  // namespace radon

@@ -396,3 +396,33 @@ def test_forward_adjoint_host_pair_call_equals_the_separate_host_calls(rb):
     plan.radon_adjoint_host(hs2, hxt2)
     assert torch.equal(hs, hs2) and torch.equal(hxt, hxt2)
     plan.close()
+
+
+def test_error_paths_on_a_live_plan(rb):
+    """Every entry point refuses null pointers and out-of-range arguments with RADON_EINVAL (-1)
+    and leaves the plan usable (include/radon.h, "Errors")."""
+    import ctypes
+
+    L = rb.lib()
+    cfg = workloads.get_config(1)
+    plan = rb.RadonPlan(cfg.N, cfg.n_angles, cfg.n_det)
+    x = torch.zeros((cfg.N, cfg.N), device="cuda"); s = torch.zeros((cfg.n_angles, cfg.n_det), device="cuda")
+    px, ps, nul = ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(s.data_ptr()), None
+    h = plan._h
+    for name, a, b in (("radon_forward", px, ps), ("radon_adjoint", ps, px), ("radon_inverse", ps, px),
+                       ("radon_forward_filtered", px, ps), ("radon_adjoint_filtered", ps, px)):
+        assert getattr(L, name)(h, nul, b, nul) == -1 and getattr(L, name)(h, a, nul, nul) == -1, name
+    assert L.radon_forward_batch(h, px, ps, -1, nul) == -1 and L.radon_forward_batch(h, nul, ps, 1, nul) == -1
+    assert L.radon_forward_host(h, nul, nul, 1) == -1 and L.radon_forward_adjoint_host(h, nul, nul, nul, 1) == -1
+    assert L.radon_filter(h, ps, ps, 2, nul) == -1 and L.radon_filter(h, nul, ps, 0, nul) == -1
+    assert L.radon_plan_set_filter(h, 8) == -1 and L.radon_plan_set_filter(h, -1) == -1
+    assert L.radon_solver_step(h, px, ps, ctypes.c_float(0.1), ctypes.c_float(-1.0), 0, nul) == -1
+    assert L.radon_solver_run(h, px, nul, ctypes.c_float(0.1), ctypes.c_float(0.0), 0, 3, nul) == -1
+    assert L.radon_solver_run(h, px, ps, ctypes.c_float(0.1), ctypes.c_float(0.0), 0, -3, nul) == -1
+    assert L.radon_paper_bins_stats(h, None, None, None, None) == -1        # before the first paper-bins call
+    assert L.radon_grid_only_paper_bins(h, ps, ps, 0, nul) == -1
+    assert L.radon_plan_stage_times(None, None, None) == -1 and L.radon_plan_info(None, *([None] * 6)) == -1
+    # the plan still works
+    S = plan.radon_forward(torch.from_numpy(workloads.make_image(1)).cuda())
+    assert torch.isfinite(S).all() and float(S.abs().sum()) > 0
+    plan.close()

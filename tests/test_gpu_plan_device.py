@@ -63,3 +63,17 @@ def test_device_and_host_built_plans_agree_and_match_the_oracle(rb):
     assert np.array_equal(again.radon_adjoint(Sd).cpu().numpy(), Ad)
     for p in (dev_plan, host_plan, again):
         p.close()
+
+
+@pytest.mark.parametrize("shape", [(64, 90, 91), (64, 30, 92), (32, 17, 48), (128, 37, 200), (512, 360, 725)])
+def test_device_built_density_table_matches_the_host_table(rb, shape):
+    """D of PAPER.md:89 for radon_inverse: the CUDA kernel (one thread per sample, neighbours from the
+    geometry, fp64 series of I0) against the host fp64 table (itself checked against the oracle's
+    O(M^2) double sum in tests/test_host_logic.py) to fp32 round-off."""
+    plan = rb.RadonPlan(*shape)
+    plan.prepare_inverse()
+    D, scale = plan.density()
+    ref, scale_ref = rb.density_host(*shape)
+    assert abs(scale / scale_ref - 1) < 1e-12
+    assert np.max(np.abs(D.numpy() / ref - 1)) < 2e-7
+    plan.close()

@@ -150,3 +150,41 @@ def test_filter_basis_of_the_library_spans_the_oracle_projector(n, order):
     got = z - (z @ q) @ q.T
     ref = oracle.polyfilter(z, min(order, n - 1))
     assert np.linalg.norm(got - ref) / np.linalg.norm(z) < 5e-7
+
+
+def test_plan_create_rejects_bad_and_unbuilt_requests_without_touching_a_gpu():
+    """Error behaviour of the boundary (include/radon.h): argument checks come before any CUDA call,
+    so they can be exercised on a CPU box.  EINVAL = -1, EUNSUPPORTED = -5."""
+    import ctypes
+
+    L = rb.lib()
+    h = ctypes.c_void_p(123)
+
+    def create(N, na, nd, sigma=2.0, W=6):
+        return L.radon_plan_create(ctypes.byref(h), N, na, nd, ctypes.c_float(sigma), W), h.value
+
+    assert L.radon_plan_create(None, 64, 90, 91, ctypes.c_float(2.0), 6) == -1
+    for args in [(4, 90, 91), (64, 0, 91), (64, 90, 1), (64, 70000, 91), (64, 90, 65534)]:
+        assert create(*args) == (-1, None), args                          # and *out is set to NULL
+    assert create(64, 90, 91, sigma=1.0)[0] == -1 and create(64, 90, 91, sigma=9.0)[0] == -1
+    assert create(63, 90, 91, sigma=1.5)[0] == -1                          # sigma N not an even integer
+    assert create(64, 90, 91, W=1)[0] == -1 and create(64, 90, 91, W=13)[0] == -1
+    assert create(64, 90, 91, W=8)[0] == -5 and create(64, 90, 91, W=4)[0] == -5      # valid, not built
+    assert create(1536, 1025, 2048)[0] == -5                               # sigma N = 3072 is not a power of two
+    assert create(64, 90, 5000)[0] == -5                                   # Bluestein length > 8192
+    assert b"power of two" in L.radon_strerror(-5)
+    # host-only entry points
+    q = (ctypes.c_float * 64)()
+    assert L.radon_filter_basis_host(0, 3, q) == -1 and L.radon_filter_basis_host(8, 8, q) == -1
+    assert L.radon_filter_basis_host(8, 3, None) == -1 and L.radon_filter_basis_host(8, 3, q) == 0
+    w = (ctypes.c_float * 6)()
+    assert L.radon_kb_weights_host(6, ctypes.c_float(2.0), ctypes.c_float(1.5), w) == -1
+    assert L.radon_kb_weights_host(8, ctypes.c_float(2.0), ctypes.c_float(0.5), w) == -5
+    bad = ctypes.c_longlong()
+    assert L.radon_schedule_selfcheck(64, 90, 91, ctypes.c_float(2.0), 8, 0, ctypes.byref(bad)) == -5
+    assert L.radon_density_host(64, 90, 91, ctypes.c_float(2.0), 6, None, None) == -1
+    # a NULL plan is an argument error everywhere, never a crash
+    for name in ("radon_forward", "radon_adjoint", "radon_inverse", "radon_nufft2", "radon_nufft1", "radon_interp_only",
+                 "radon_grid_only", "radon_proj_ifft", "radon_proj_fft", "radon_forward_filtered", "radon_adjoint_filtered"):
+        assert getattr(L, name)(None, None, None, None) == -1, name
+    assert L.radon_plan_destroy(None) == 0
