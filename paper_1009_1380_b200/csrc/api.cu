@@ -126,7 +126,7 @@ static int validate(int N, int n_angles, int n_det, float sigma, int W, int *G_o
     const double g = (double)sigma * N;
     const long long G = llround(g);
     if (fabs(g - (double)G) > 1e-6 || (G & 1)) return RADON_EINVAL;
-    if (W != KW) return RADON_EUNSUPPORTED;
+    if (!kw_supported(W)) return RADON_EUNSUPPORTED;
     if (!fft_length_supported((int)G)) return RADON_EUNSUPPORTED;
     {   // projection DFT: one FFT of length n_det when that is a power of two >= 16, else Bluestein (L >= 2n - 1)
         const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
@@ -171,7 +171,7 @@ static int workspace_alloc(radon_plan *p, Workspace &w)
     if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
     if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
     if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
-    if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW + 1) * (KW + 1)))) return rc;
+    if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW_MAX + 1) * (KW_MAX + 1)))) return rc;
     if (!w.tickets) {
         const size_t n = (size_t)std::max(p->n_jobs, 1) * MERGE_COUNTERS_PER_JOB;
         if ((rc = dev_alloc(p, &w.tickets, n))) return rc;
@@ -192,7 +192,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     p->geo.init(N, n_angles, n_det, (double)sigma, W);
     p->M = (long long)n_angles * n_det;
     DevicePlan &d = p->dev;
-    d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det;
+    d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det; d.W = W;
     d.n_sm = prop.multiProcessorCount;
     d.pdl = G <= 2048;
     const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
@@ -445,7 +445,7 @@ static int density_setup(radon_plan *p)
             if ((rc = dev_upload(p, &p->dev_density, p->host_density))) return rc;
         } else {
             if ((rc = dev_alloc(p, &p->dev_density, (size_t)p->M))) return rc;
-            if (launch_density(p->dev.cs, na, n, beta, inv, scale, p->dev_density, 0)) return RADON_ECUDA;
+            if (launch_density(p->dev.cs, na, n, W, beta, inv, scale, p->dev_density, 0)) return RADON_ECUDA;
             p->host_density.resize((size_t)p->M);
             CUDA_TRY(cudaMemcpy(p->host_density.data(), p->dev_density, (size_t)p->M * sizeof(float), cudaMemcpyDeviceToHost));
             p->density_scale = scale;
@@ -992,12 +992,14 @@ extern "C" int radon_schedule_host_stats(int N, int n_angles, int n_det, float s
 extern "C" int radon_kb_weights_host(int W, float sigma, float delta, float *w)
 {
     if (!w || W < 2 || W > 12 || !(sigma > 1.0f) || !(delta >= 0.f && delta <= 1.f)) return RADON_EINVAL;
-    if (W != KW) return RADON_EUNSUPPORTED;
+    if (!kw_supported(W)) return RADON_EUNSUPPORTED;
     KbPoly kp;
     build_kb_poly(W, sigma, kp);
-    float tmp[KW];
-    kb_poly_weights(kp, delta, tmp);
-    for (int l = 0; l < KW; ++l) w[l] = tmp[l];
+    RADON_FOR_W(W, {
+        float tmp[WW];
+        kb_poly_weights<WW>(kp, delta, tmp);
+        for (int l = 0; l < WW; ++l) w[l] = tmp[l];
+    })
     return RADON_OK;
 }
 
@@ -1011,7 +1013,7 @@ extern "C" const char *radon_strerror(int code)
     case RADON_ENOMEM: return "out of memory";
     case RADON_ECUDA: return "CUDA runtime error (see radon_last_cuda_error)";
     case RADON_EARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
-    case RADON_EUNSUPPORTED: return "valid request outside this build (W != 6, or sigma*N not a power of two in [16, 8192], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
+    case RADON_EUNSUPPORTED: return "valid request outside this build (W not 4, 6 or 8, or sigma*N not a power of two in [16, 8192], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
     default: return "unknown error";
     }
 }

@@ -141,7 +141,7 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
 template <int L, bool S2>
 __global__ void __launch_bounds__(FftCfg<L>::THREADS, (FftCfg<L>::THREADS <= 256) ? 1024 / FftCfg<L>::THREADS : 1)   // 64 registers: four CTAs of 256
 rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
-                   const float2 *__restrict__ tw, int N, int mirror)
+                   const float2 *__restrict__ tw, int N, int mirror, int KW)
 {
     extern __shared__ __align__(16) float2 s_fft[];
     pdl_prologue();
@@ -399,10 +399,10 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
     case 1:
         if (s2) {
             if (set_smem(rowpass_fwd_kernel<L, true>, C::SMEM)) return -1;
-            launch_pdl(p.pdl, rowpass_fwd_kernel<L, true>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag);
+            launch_pdl(p.pdl, rowpass_fwd_kernel<L, true>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag, p.W);
         } else {
             if (set_smem(rowpass_fwd_kernel<L, false>, C::SMEM)) return -1;
-            launch_pdl(p.pdl, rowpass_fwd_kernel<L, false>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag);
+            launch_pdl(p.pdl, rowpass_fwd_kernel<L, false>, row_blocks, C::THREADS, C::SMEM, st, (const float2 *)in, (float2 *)out, tw, N, flag, p.W);
         }
         break;
     case 2:

@@ -39,10 +39,10 @@ bool pdl_enabled()
 // "empty" mbarrier.  The 36 taps of a sample are 64-bit shared-memory loads that the
 // plan-time schedule made conflict free; slots are fetched two rounds ahead, ray directions one.
 constexpr int GATHER_THREADS = (GATHER_WARPS + 1) * 32;
-constexpr size_t GATHER_TILE_BYTES = (size_t)GT_ROWS * GT_PITCH * sizeof(float2);
-constexpr size_t GATHER_SMEM = GATHER_STAGES * GATHER_TILE_BYTES;
-static_assert((GT_PITCH * sizeof(float2)) % 16 == 0 && GT_X % 2 == 0, "bulk copies need 16-byte rows");
-static_assert(GATHER_TILE_BYTES % 16 == 0, "stage buffers stay 16-byte aligned");
+constexpr size_t gather_tile_bytes(int W) { return (size_t)gt_rows(W) * gt_pitch(W) * sizeof(float2); }
+constexpr size_t gather_smem(int W) { return GATHER_STAGES * gather_tile_bytes(W); }
+static_assert(GT_X % 2 == 0, "bulk copies need 16-byte rows (the pitch GT_X + W is even for the even widths built)");
+static_assert(gather_smem(KW_MAX) <= 227 * 1024, "the stages of the widest kernel must fit one CTA");
 
 #ifndef RADON_GATHER_PACKED
 #define RADON_GATHER_PACKED 1
@@ -59,6 +59,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+template <int KW>
 __global__ void __launch_bounds__(GATHER_THREADS, 1)
 gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
               const GatherCta *__restrict__ items, const int *__restrict__ worker_begin,
@@ -68,6 +69,8 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full[GATHER_STAGES], empty[GATHER_STAGES];
+    constexpr int GT_PITCH = GT_X + KW, GT_ROWS = GT_Y + KW - 1;          // gt_pitch(KW), gt_rows(KW)
+    constexpr size_t GATHER_TILE_BYTES = (size_t)GT_ROWS * GT_PITCH * sizeof(float2);
     pdl_prologue();
 
     const int it_begin = worker_begin[blockIdx.x], it_end = worker_begin[blockIdx.x + 1];
@@ -140,8 +143,8 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
             const double2 dn = load_dir(nx);
             const bool act = sl.ak != SLOT_EMPTY;
             const int a = act ? (int)(sl.ak >> 16) : 0, k = act ? (int)(sl.ak & 0xffff) : 0;
-            Taps tp;
-            sample_taps_dir(d, kp, k, cd, halfG, tp);
+            Taps<KW> tp;
+            sample_taps_dir<KW>(d, kp, k, cd, halfG, tp);
             if (act) {
                 const float2 *base = tile + (sl.lxy >> 16) * GT_PITCH + (sl.lxy & 0xffff);
 #if RADON_GATHER_PACKED
@@ -217,12 +220,33 @@ __device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t by
                  ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
 
-// One footprint row of one sample: cell[lx] += (vr, vi) * wx[lx] for the taps whose bit is set
-// in `mask`.  Written as one PTX block on a 32-bit shared-window address with immediate
-// offsets: W predicated 64-bit loads, 2 W FMAs, W predicated stores, nothing else.
+// One footprint row of one sample: cell[lx] += (vr, vi) * wx[lx] for the taps whose bit is set in
+// `mask` (all loads, then the FMAs, then the stores: the row step of the schedule's disjointness rule).
+template <int KW>
 __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float vr, float vi, const float (&wx)[KW])
 {
-    static_assert(KW == 6, "row step is written for W = 6");
+    uint64_t c[KW];
+#pragma unroll
+    for (int lx = 0; lx < KW; ++lx) {
+        c[lx] = 0ull;
+        if (mask & (1u << lx)) asm volatile("ld.shared.b64 %0, [%1];" : "=l"(c[lx]) : "r"(addr + 8u * lx) : "memory");
+    }
+    const uint64_t v2 = pack2(vr, vi);
+#pragma unroll
+    for (int lx = 0; lx < KW; ++lx) {
+        const uint64_t w2 = pack2(wx[lx], wx[lx]);
+        asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c[lx]) : "l"(v2), "l"(w2));
+    }
+#pragma unroll
+    for (int lx = 0; lx < KW; ++lx)
+        if (mask & (1u << lx)) asm volatile("st.shared.b64 [%0], %1;" ::"r"(addr + 8u * lx), "l"(c[lx]) : "memory");
+}
+
+// W = 6: one PTX block on a 32-bit shared-window address with immediate offsets: W predicated 64-bit
+// loads, 2 W FMAs, W predicated stores, nothing else.
+template <>
+__device__ __forceinline__ void scatter_row<6>(uint32_t addr, uint32_t mask, float vr, float vi, const float (&wx)[6])
+{
     asm volatile(
         "{\n"
         ".reg .pred p0, p1, p2, p3, p4, p5;\n"
@@ -295,9 +319,23 @@ __device__ __forceinline__ void scatter_row(uint32_t addr, uint32_t mask, float 
 #else
 #error "add the row offsets of this accumulator pitch"
 #endif
-__device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, float vr, float vi, const Taps &tp)
+// widths other than 6: the same row steps from the generic row routine (no tap predicates needed:
+// the mask is all ones for an active lane)
+template <int KW>
+__device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, float vr, float vi, const Taps<KW> &tp)
 {
-    static_assert(KW == 6 && ACC_PITCH * sizeof(float2) == RADON_RO1, "row offsets are written for W = 6 and this pitch");
+#pragma unroll
+    for (int ly = 0; ly < KW; ++ly) {
+        scatter_row<KW>(addr + (uint32_t)(ly * ACC_PITCH * (int)sizeof(float2)), act ? ((1u << KW) - 1u) : 0u,
+                        vr * tp.wy[ly], vi * tp.wy[ly], tp.wx);
+        __syncwarp();
+    }
+}
+template <>
+__device__ __forceinline__ void scatter_footprint_fast<6>(uint32_t addr, int act, float vr, float vi, const Taps<6> &tp)
+{
+    constexpr int KW = 6;
+    static_assert(ACC_PITCH * sizeof(float2) == RADON_RO1, "row offsets are written for this pitch");
     uint64_t v[KW], w[KW];
 #pragma unroll
     for (int l = 0; l < KW; ++l) {
@@ -324,11 +362,11 @@ __device__ __forceinline__ void scatter_footprint_fast(uint32_t addr, int act, f
         "l"(w[0]), "l"(w[1]), "l"(w[2]), "l"(w[3]), "l"(w[4]), "l"(w[5]) : "memory");
 }
 
-constexpr int DC_CELLS = (KW + 1) * (KW + 1);
+constexpr int DC_CELLS_MAX = (KW_MAX + 1) * (KW_MAX + 1);
 // NT threads of one CTA: sum the j = 0 samples of all angles (fixed order) and write the value
 // to add to each cell of the (W+1)^2 centre window to dcbuf (cell c: offset ux = c % (W+1) - W/2,
 // uy = c / (W+1) - W/2 from DC; zero where nothing is to be added).  part: NT float2 of shared memory.
-template <int NT>
+template <int NT, int KW>
 __device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, const KbPoly &kp, int n_det, int n_angles, int half,
                                            float2 *part, float2 *__restrict__ dcbuf)
 {
@@ -351,9 +389,10 @@ __device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, con
         __syncthreads();
     }
     const float2 V = part[0];
+    constexpr int DC_CELLS = (KW + 1) * (KW + 1);
     float wa[KW], wb[KW];
-    kb_poly_weights(kp, 0.f, wa);
-    kb_poly_weights(kp, 1.f, wb);
+    kb_poly_weights<KW>(kp, 0.f, wa);
+    kb_poly_weights<KW>(kp, 1.f, wb);
     auto tap = [](const float (&w)[KW], int l) {
         float r = 0.f;
 #pragma unroll
@@ -381,7 +420,7 @@ __device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, con
 // (W+1)^2 centre window (DESIGN.md R-tie).
 template <int NT>
 __device__ __forceinline__ void merge_rows(const MergeJob &j, int y_begin, int y_end, const float2 *__restrict__ scratch,
-                                           float2 *__restrict__ grid, int G, const float2 *__restrict__ dcbuf)
+                                           float2 *__restrict__ grid, int G, const float2 *__restrict__ dcbuf, int KW)
 {
     const int ppr = j.rw >> 1, p_begin = ppr * y_begin, p_end = ppr * y_end;        // rw is even (check_schedules)
     const float4 *src = reinterpret_cast<const float4 *>(scratch + (size_t)j.first_slot * (SR_X * SR_Y));
@@ -450,7 +489,7 @@ constexpr int MERGE_COUNTERS = MERGE_COUNTERS_PER_JOB;   // ints per job: arriva
 template <int NT>
 __device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *__restrict__ jobs, int *__restrict__ tickets,
                                            const float2 *__restrict__ scratch, float2 *__restrict__ grid, int G,
-                                           const float2 *__restrict__ dcbuf, int *s_flag)
+                                           const float2 *__restrict__ dcbuf, int *s_flag, int KW)
 {
     int *cnt = tickets + job * MERGE_COUNTERS;
     const MergeJob j = jobs[job];
@@ -482,7 +521,7 @@ __device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *_
             __syncthreads();
             const int c = *s_flag;
             if (c >= n_chunks) break;
-            merge_rows<NT>(j, c * rows, min(j.rh, (c + 1) * rows), scratch, grid, G, dcbuf);
+            merge_rows<NT>(j, c * rows, min(j.rh, (c + 1) * rows), scratch, grid, G, dcbuf, KW);
         }
     }
     __syncthreads();
@@ -493,6 +532,7 @@ __device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *_
 
 struct DcJobs { int n; int job[MAX_DC_JOBS]; };
 
+template <int KW>
 __global__ void __launch_bounds__(SCATTER_THREADS, SCATTER_CTAS_PER_SM)
 scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, float2 *__restrict__ scratch,
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
@@ -507,10 +547,10 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     if (blockIdx.x == 0) {
         // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
         // footprint of the sum is added by the merge of the centre rectangles (DESIGN.md R-tie)
-        dc_compute<SCATTER_THREADS>(polar, kp, n_det, n_angles, half, acc, dcbuf);
+        dc_compute<SCATTER_THREADS, KW>(polar, kp, n_det, n_angles, half, acc, dcbuf);
         __threadfence();
         for (int q = 0; q < dcj.n; ++q)
-            join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
+            join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW);
         return;
     }
     __shared__ ScatterCta cta;
@@ -555,6 +595,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     __syncthreads();
 
     // shared-window address of slot (0,0); never dereferenced outside the quadrant
+    constexpr int KH = KW - 1;
     const uint32_t origin = smem_u32(acc) + (uint32_t)(((item.sy0 - KH) * ACC_PITCH + (item.sx0 - KH)) * (int)sizeof(float2));
     for (int r = 0; r < nr; ++r) {
         const Slot s4 = load_slot(r + 4);
@@ -567,12 +608,12 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         // ghost k = n (j = +n/2) carry half the value each, the ghost conjugated.  Applied here,
         // at the point of use, so that the prefetched load stays off the critical path.
         if (nyq_split && (k0 == 0 || k0 == n_det)) v0 = make_float2(0.5f * v0.x, k0 == 0 ? 0.5f * v0.y : -0.5f * v0.y);
-        Taps tp;
-        sample_taps_dir(d0, kp, k0, cd, halfG, tp);
+        Taps<KW> tp;
+        sample_taps_dir<KW>(d0, kp, k0, cd, halfG, tp);
         const int bx = (int)(s0.lxy & 0xffff), by = (int)(s0.lxy >> 16);   // biased by KH
         const uint32_t base = origin + (uint32_t)((by * ACC_PITCH + bx) * (int)sizeof(float2));
         if (RADON_SC_FAST && r < item.fast_count) {   // warp-uniform: footprints wholly inside the quadrant
-            scatter_footprint_fast(base, act ? 1 : 0, v0.x, v0.y, tp);
+            scatter_footprint_fast<KW>(base, act ? 1 : 0, v0.x, v0.y, tp);
         } else {
         // taps inside the quadrant: KH <= bx + lx < KH + sw, likewise rows -> bit masks
         const int xlo = min(max(KH - bx, 0), KW), xhi = min(max(KH + item.sw - bx, 0), KW);
@@ -582,7 +623,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
 #pragma unroll
         for (int ly = 0; ly < KW; ++ly) {
             const uint32_t m = (ymask & (1u << ly)) ? xmask : 0u;
-            scatter_row(base + (uint32_t)(ly * ACC_PITCH * (int)sizeof(float2)), m,
+            scatter_row<KW>(base + (uint32_t)(ly * ACC_PITCH * (int)sizeof(float2)), m,
                         v0.x * tp.wy[ly], v0.y * tp.wy[ly], tp.wx);
             __syncwarp();   // row steps of different lanes may touch the same cells
         }
@@ -610,7 +651,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
     __threadfence();
-    join_merge<SCATTER_THREADS>(cta.job, true, jobs, tickets, scratch, grid, G, dcbuf, &s_flag);
+    join_merge<SCATTER_THREADS>(cta.job, true, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW);
 }
 
 // The j = 0 samples (k = n/2) of all angles sit at kappa = (0,0) and share one footprint, so
@@ -625,8 +666,8 @@ int launch_gather(const DevicePlan &p, bool half, const float2 *grid, float2 *po
 {
     const DevicePlan::Sched &q = p.sched[half ? 1 : 0];
     if (q.n_gather_ctas == 0) return 0;
-    launch_pdl(p.pdl, gather_kernel, q.n_gather_workers, GATHER_THREADS, GATHER_SMEM, st,
-        grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.kb, p.G, p.n_det);
+    RADON_FOR_W(p.W, launch_pdl(p.pdl, gather_kernel<WW>, q.n_gather_workers, GATHER_THREADS, gather_smem(WW), st,
+        grid, polar, q.gather_ctas, q.gather_worker_begin, q.gather_slots, p.cs, p.kb, p.G, p.n_det);)
     count_launch();
     return 0;
 }
@@ -640,17 +681,19 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
     dcj.n = q.n_dc_jobs;
     for (int i = 0; i < MAX_DC_JOBS; ++i) dcj.job[i] = q.dc_jobs[i];
     // CTA 0 sums the j = 0 samples; CTA b > 0 grids scatter_ctas[b - 1] (heaviest first)
-    launch_pdl(p.pdl, scatter_kernel, q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st,
+    RADON_FOR_W(p.W, launch_pdl(p.pdl, scatter_kernel<WW>, q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st,
         polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.kb, p.G, p.n_det, nyq,
-        dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);
+        dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);)
     count_launch();
     return 0;
 }
 
 int init_kernel_attributes()
 {
-    if (set_smem(gather_kernel, GATHER_SMEM)) return -1;
-    if (set_smem(scatter_kernel, SCATTER_SMEM)) return -1;
+    if (set_smem(gather_kernel<4>, gather_smem(4)) || set_smem(gather_kernel<6>, gather_smem(6)) ||
+        set_smem(gather_kernel<8>, gather_smem(8))) return -1;
+    if (set_smem(scatter_kernel<4>, SCATTER_SMEM) || set_smem(scatter_kernel<6>, SCATTER_SMEM) ||
+        set_smem(scatter_kernel<8>, SCATTER_SMEM)) return -1;
     return 0;
 }
 

@@ -11,6 +11,7 @@ namespace radon {
 
 struct DevicePlan {
     int N = 0, G = 0, n_angles = 0, n_det = 0, LP = 0;   // LP: FFT length of the projection DFT
+    int W = 6;                    // Kaiser-Bessel width (4, 6 or 8)
     int n_sm = 148;               // multiprocessors of the device (persistent grids)
     bool pdl = false;             // programmatic dependent launch between the kernels of a call (small grids)
     // tables
@@ -46,7 +47,7 @@ void count_launch(long long n = 1);
 template <typename F>
 static inline int set_smem(F kernel, size_t bytes)
 {
-    if (bytes <= 48 * 1024) return 0;
+    if (bytes <= 40 * 1024) return 0;        // static shared memory counts towards the 48 KB default too
     static std::mutex mu;
     static std::set<std::pair<int, const void *>> done;
     int dev = 0;

@@ -22,22 +22,24 @@ namespace radon {
 
 constexpr int PB_THREADS = 256;
 constexpr int PB_STAGE = 1024;                  // samples that "fit in shared memory" (64 bytes each)
+template <int KW>
 struct __align__(16) StagedSample {
     float wx[KW], wy[KW];                       // tap weights along x and y
     float vr, vi;                               // sample value
     int bx, by;                                 // base cell of the footprint (may lie outside [0, G))
 };
-static_assert(sizeof(StagedSample) == 64 && KW == 6, "one staged sample = 64 bytes");
+static_assert(sizeof(StagedSample<6>) == 64 && sizeof(StagedSample<8>) == 80 && sizeof(StagedSample<4>) == 48, "staged sample layout");
 
+template <int KW>
 __device__ __forceinline__ void stage_sample(const PaperBinEntry en, const float2 *__restrict__ polar,
                                              const double2 *__restrict__ cs, const KbPoly &kp, int G, int n_det,
-                                             StagedSample &s)
+                                             StagedSample<KW> &s)
 {
     const int a = (int)(en.ak >> 16), k = (int)(en.ak & 0xffff);
     const double2 d = __ldg(&cs[a]);
     const double halfG = 0.5 * (double)G, jj = (double)(k - n_det / 2);
-    Taps tp;
-    sample_taps_dir(d, kp, k, n_det / 2, halfG, tp);
+    Taps<KW> tp;
+    sample_taps_dir<KW>(d, kp, k, n_det / 2, halfG, tp);
 #pragma unroll
     for (int l = 0; l < KW; ++l) { s.wx[l] = tp.wx[l]; s.wy[l] = tp.wy[l]; }
     const float2 v = __ldg(&polar[(size_t)a * n_det + k]);
@@ -47,13 +49,14 @@ __device__ __forceinline__ void stage_sample(const PaperBinEntry en, const float
 }
 
 // one thread block per bin
+template <int KW>
 __global__ void __launch_bounds__(PB_THREADS)
 paper_bins_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, const PaperBin *__restrict__ bins,
                   const PaperBinEntry *__restrict__ entries, const double2 *__restrict__ cs, const KbPoly kp,
                   int G, int n_det)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    StagedSample *st = reinterpret_cast<StagedSample *>(smem_raw);
+    StagedSample<KW> *st = reinterpret_cast<StagedSample<KW> *>(smem_raw);
     __shared__ float2 red[PB_THREADS / 32];
     const PaperBin bin = bins[blockIdx.x];
     const PaperBinEntry *list = entries + bin.first;
@@ -61,7 +64,7 @@ paper_bins_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, c
 
     if (bin.count <= PB_STAGE) {
         // "it does fit in shared memory": one thread per grid point, loop through the staged samples
-        for (int i = threadIdx.x; i < bin.count; i += PB_THREADS) stage_sample(list[i], polar, cs, kp, G, n_det, st[i]);
+        for (int i = threadIdx.x; i < bin.count; i += PB_THREADS) stage_sample<KW>(list[i], polar, cs, kp, G, n_det, st[i]);
         __syncthreads();
         for (int c = threadIdx.x; c < n_cells; c += PB_THREADS) {
             const int X = bin.x0 + c % bin.w, Y = bin.y0 + c / bin.w;
@@ -84,7 +87,7 @@ paper_bins_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, c
         const int X = bin.x0 + c % bin.w, Y = bin.y0 + c / bin.w;
         float ar = 0.f, ai = 0.f;
         for (int i = threadIdx.x; i < bin.count; i += PB_THREADS) {
-            StagedSample s;
+            StagedSample<KW> s;
             const PaperBinEntry en = list[i];
             // cheap reject before the weights: base cell from the fp64 coordinates
             const int a = (int)(en.ak >> 16), k = (int)(en.ak & 0xffff);
@@ -94,7 +97,7 @@ paper_bins_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, c
             const int by = (int)ceil(fma(jj, d.y, halfG) - 0.5 * KW) + (((en.shift >> 2) & 3) - 1) * G;
             const unsigned lx = (unsigned)(X - bx), ly = (unsigned)(Y - by);
             if (lx < (unsigned)KW && ly < (unsigned)KW) {
-                stage_sample(en, polar, cs, kp, G, n_det, s);
+                stage_sample<KW>(en, polar, cs, kp, G, n_det, s);
                 float wx = 0.f, wy = 0.f;
 #pragma unroll
                 for (int l = 0; l < KW; ++l) { wx = (l == (int)lx) ? s.wx[l] : wx; wy = (l == (int)ly) ? s.wy[l] : wy; }
@@ -121,9 +124,11 @@ paper_bins_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, c
 int launch_paper_bins(const DevicePlan &p, const PaperBin *bins, int n_bins, const PaperBinEntry *entries,
                       const float2 *polar, float2 *grid, cudaStream_t st)
 {
-    const size_t smem = (size_t)PB_STAGE * sizeof(StagedSample);
-    if (set_smem(paper_bins_kernel, smem)) return -1;
-    paper_bins_kernel<<<n_bins, PB_THREADS, smem, st>>>(polar, grid, bins, entries, p.cs, p.kb, p.G, p.n_det);
+    RADON_FOR_W(p.W, {
+        const size_t smem = (size_t)PB_STAGE * sizeof(StagedSample<WW>);
+        if (set_smem(paper_bins_kernel<WW>, smem)) return -1;
+        launch_pdl(false, paper_bins_kernel<WW>, n_bins, PB_THREADS, smem, st, polar, grid, bins, entries, p.cs, p.kb, p.G, p.n_det);
+    })
     count_launch();
     return 0;
 }

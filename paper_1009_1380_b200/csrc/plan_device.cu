@@ -34,9 +34,10 @@ struct SampleSet {              // which (a, k) a schedule covers
     int n_angles, n_det, G;
     int k0, k1;                 // k in [k0, k1); k == n_det is the Nyquist ghost (j = +n/2)
     int skip_k;                 // left out (scatter: j = 0), or -1
+    int W;                      // kernel width
 };
 
-__device__ __forceinline__ void base_cell(const double2 d, int j, double halfG, int &x0, int &y0)
+__device__ __forceinline__ void base_cell(const double2 d, int j, double halfG, int KW, int &x0, int &y0)
 {
     // the same fp64 expressions as Geometry::base and sample_taps_dir: bit-identical tap selection
     x0 = (int)ceil(fma((double)j, d.x, halfG) - 0.5 * KW);
@@ -61,7 +62,7 @@ template <typename F>
 __device__ __forceinline__ void for_candidates(const PackRegion &r, const SampleSet &s, const double2 d, int a,
                                                int sx, int sy, F f)
 {
-    const int cd = s.n_det / 2;
+    const int cd = s.n_det / 2, KW = s.W;
     const double halfG = 0.5 * (double)s.G;
     int jlo = s.k0 - cd, jhi = s.k1 - 1 - cd;
     j_interval(d.x, halfG - 0.5 * KW + (double)sx * s.G, r.rx0 - r.lo, r.rx0 + r.rw - 1, jlo, jhi);
@@ -70,7 +71,7 @@ __device__ __forceinline__ void for_candidates(const PackRegion &r, const Sample
         const int k = j + cd;
         if (k == s.skip_k) continue;
         int x0, y0;
-        base_cell(d, j, halfG, x0, y0);
+        base_cell(d, j, halfG, KW, x0, y0);
         const int bx = x0 + sx * s.G, by = y0 + sy * s.G - r.oy;
         if (bx < r.rx0 - r.lo || bx >= r.rx0 + r.rw || by < r.ry0 - r.lo || by >= r.ry0 + r.rh) continue;
         if (r.lo == 0 && (bx < 0 || bx >= s.G || by < 0 || by >= s.G)) continue;     // gather: one image per sample
@@ -80,7 +81,7 @@ __device__ __forceinline__ void for_candidates(const PackRegion &r, const Sample
 
 __device__ __forceinline__ bool cand_inside(const PackRegion &r, int lx, int ly)
 {
-    return r.lo == 0 || (lx >= KH && lx <= r.rw - 1 && ly >= KH && ly <= r.rh - 1);
+    return r.lo == 0 || (lx >= r.lo && lx <= r.rw - 1 && ly >= r.lo && ly <= r.rh - 1);     // scatter: lo = W - 1
 }
 
 // ---- pass 1: count the candidates of every region ---------------------------------------------
@@ -88,12 +89,12 @@ constexpr int PLAN_WARPS = 4;
 __global__ void __launch_bounds__(PLAN_WARPS * 32)
 count_regions_kernel(PackRegion *__restrict__ regions, int n_regions, const double2 *__restrict__ cs, const SampleSet s)
 {
-    __shared__ int rowcnt[PLAN_WARPS][ST_Y + KH > GT_ROWS ? ST_Y + KH : GT_ROWS];
+    __shared__ int rowcnt[PLAN_WARPS][SB_H_MAX > GT_ROWS_MAX ? SB_H_MAX : GT_ROWS_MAX];
     const int ri = blockIdx.x * PLAN_WARPS + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (ri >= n_regions) return;
     const PackRegion r = regions[ri];
     int *rc = rowcnt[threadIdx.x >> 5];
-    constexpr int NROW = ST_Y + KH > GT_ROWS ? ST_Y + KH : GT_ROWS;
+    constexpr int NROW = SB_H_MAX > GT_ROWS_MAX ? SB_H_MAX : GT_ROWS_MAX;
     for (int i = lane; i < NROW; i += 32) rc[i] = 0;
     __syncwarp();
     int n_in = 0, n_cl = 0;
@@ -123,13 +124,13 @@ struct RoundState {
 };
 
 // occupancy of the round: one 128-bit row per base row (bit = base column no other lane may take)
-struct OccRows { unsigned long long w[(ST_Y + KH > GT_ROWS ? ST_Y + KH : GT_ROWS)][2]; };
+struct OccRows { unsigned long long w[(SB_H_MAX > GT_ROWS_MAX ? SB_H_MAX : GT_ROWS_MAX)][2]; };
 
 __device__ __forceinline__ bool occ_overlaps(const OccRows &o, int lx, int ly)
 {
     return (o.w[ly][lx >> 6] >> (lx & 63)) & 1ull;
 }
-__device__ __forceinline__ void occ_mark(OccRows &o, int lx, int ly)       // one lane
+__device__ __forceinline__ void occ_mark(OccRows &o, int lx, int ly, int KH)       // one lane
 {
     const int lo = max(lx - KH, 0), hi = min(lx + KH, 127);
     for (int x = lo; x <= hi; ++x) o.w[ly][x >> 6] |= 1ull << (x & 63);
@@ -236,7 +237,7 @@ fill_pack_kernel(PackList *__restrict__ lists, const PackRegion *__restrict__ re
                     if (lane == win) {
                         row[wh * 16 + st.cnt[wh]] = c;
                         cand[i].ak = SLOT_EMPTY;
-                        if (disjoint) occ_mark(occ, lx, ly);
+                        if (disjoint) occ_mark(occ, lx, ly, s.W - 1);
                         pending = false;
                     }
                     all_in = all_in && __shfl_sync(0xffffffffu, (int)cand_inside(r, lx, ly), win);
@@ -300,7 +301,7 @@ int device_pack(const double2 *d_cs, const DevicePackParams &prm, std::vector<Pa
 {
     int rc = 0;
     SampleSet s;
-    s.n_angles = prm.n_angles; s.n_det = prm.n_det; s.G = prm.G; s.k0 = prm.k0; s.k1 = prm.k1; s.skip_k = prm.skip_k;
+    s.n_angles = prm.n_angles; s.n_det = prm.n_det; s.G = prm.G; s.k0 = prm.k0; s.k1 = prm.k1; s.skip_k = prm.skip_k; s.W = prm.W;
     PackRegion *d_regions = nullptr;
     PackList *d_lists = nullptr;
     Slot *d_slots = nullptr;
@@ -432,11 +433,11 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
     out = Schedules();
     out.half = half;
     *d_gather_slots = *d_scatter_slots = nullptr;
-    const int G = g.G;
+    const int G = g.G, KW = g.W, KH = KW - 1;
     int gk0, gk1, sk1;
     sample_ranges(g, half, gk0, gk1, sk1);
     DevicePackParams prm;
-    prm.n_angles = g.n_angles; prm.n_det = g.n_det; prm.G = G;
+    prm.n_angles = g.n_angles; prm.n_det = g.n_det; prm.G = G; prm.W = KW;
     std::vector<PackRegion> regions;
     std::vector<PackList> lists;
 
@@ -451,7 +452,7 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
                 r.lo = 0; r.oy = yorg; r.K = 1;
                 regions.push_back(r);
             }
-        prm.k0 = gk0; prm.k1 = gk1; prm.skip_k = -1; prm.pitch = GT_PITCH; prm.disjoint = false;
+        prm.k0 = gk0; prm.k1 = gk1; prm.skip_k = -1; prm.pitch = gt_pitch(KW); prm.disjoint = false;
         prm.split = no_split; prm.redo = nullptr; prm.split_arg = nullptr;
         int rc = device_pack(d_cs, prm, regions, lists, d_gather_slots, n_gather_rounds);
         if (rc) return rc;
@@ -558,7 +559,7 @@ __device__ __forceinline__ double i0_series(double z)
     return sum;
 }
 
-__device__ __forceinline__ double kb_phi_dev(double u, double beta, double inv_i0b)
+__device__ __forceinline__ double kb_phi_dev(double u, double beta, double inv_i0b, int KW)
 {
     const double t = 2.0 * u / (double)KW, arg = 1.0 - t * t;
     if (arg < 0.0) return (arg > -1e-12) ? inv_i0b : 0.0;       // |u| == W/2 up to rounding
@@ -566,7 +567,7 @@ __device__ __forceinline__ double kb_phi_dev(double u, double beta, double inv_i
 }
 
 __global__ void __launch_bounds__(128)
-density_kernel(float *__restrict__ D, const double2 *__restrict__ cs, int n_angles, int n_det, double beta,
+density_kernel(float *__restrict__ D, const double2 *__restrict__ cs, int n_angles, int n_det, int KW, double beta,
                double inv_i0b, double scale)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -593,8 +594,8 @@ density_kernel(float *__restrict__ D, const double2 *__restrict__ cs, int n_angl
         if (fabs(e.y) > 1e-12) { const double u = (ky - hw) / e.y, v = (ky + hw) / e.y; lo = fmax(lo, fmin(u, v) - 1e-6); hi = fmin(hi, fmax(u, v) + 1e-6); }
         else if (fabs(ky) > hw + 1e-9) continue;
         for (int j = (int)ceil(lo); j <= (int)floor(hi); ++j) {
-            const double px = kb_phi_dev(kx - (double)j * e.x, beta, inv_i0b);
-            if (px != 0.0) sum += px * kb_phi_dev(ky - (double)j * e.y, beta, inv_i0b);
+            const double px = kb_phi_dev(kx - (double)j * e.x, beta, inv_i0b, KW);
+            if (px != 0.0) sum += px * kb_phi_dev(ky - (double)j * e.y, beta, inv_i0b, KW);
         }
     }
     D[i] = (float)(scale / sum);
@@ -612,11 +613,11 @@ __global__ void density_pair_mean_kernel(float *__restrict__ D, int n_angles, in
     row[k] = m; row[n_det - k] = m;
 }
 
-int launch_density(const double2 *d_cs, int n_angles, int n_det, double beta, double inv_i0b, double scale,
+int launch_density(const double2 *d_cs, int n_angles, int n_det, int W, double beta, double inv_i0b, double scale,
                    float *d_D, cudaStream_t st)
 {
     const long long M = (long long)n_angles * n_det;
-    density_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(d_D, d_cs, n_angles, n_det, beta, inv_i0b, scale);
+    density_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(d_D, d_cs, n_angles, n_det, W, beta, inv_i0b, scale);
     count_launch();
     return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }

@@ -9,7 +9,7 @@ namespace radon {
 
 struct PackRegion {             // a grid tile whose candidate samples are enumerated
     int rx0, ry0, rw, rh;       // cells (scatter: absolute; gather: after the row shift `oy`)
-    int lo;                     // KH: every footprint that touches the tile (scatter); 0: base cell inside (gather)
+    int lo;                     // W - 1: every footprint that touches the tile (scatter); 0: base cell inside (gather)
     int oy;                     // row shift of the gather's tile grid (Hermitian half), else 0
     int n_in, n_cl;             // device: candidates wholly inside / clipped by the tile
     int K;                      // host: lists the tile's candidates are dealt to
@@ -28,7 +28,7 @@ struct PackList {               // one gather tile, or one of the K shares of a 
 };
 
 struct DevicePackParams {
-    int n_angles, n_det, G;
+    int n_angles, n_det, G, W;
     int k0, k1, skip_k;         // samples k in [k0, k1) except skip_k
     int pitch;                  // shared-memory row pitch (complex) the bank pairs are computed for
     bool disjoint;              // scatter: footprints of a round must not meet within a row step
@@ -53,7 +53,7 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
 
 // Density compensation D of PAPER.md:89 times `scale`, one thread per sample (plan_device.cu); and the
 // pair mean the Hermitian-half scatter needs for even n_det (in place).
-int launch_density(const double2 *d_cs, int n_angles, int n_det, double beta, double inv_i0b, double scale,
+int launch_density(const double2 *d_cs, int n_angles, int n_det, int W, double beta, double inv_i0b, double scale,
                    float *d_D, cudaStream_t st);
 int launch_density_pair_mean(float *d_D, int n_angles, int n_det, cudaStream_t st);
 

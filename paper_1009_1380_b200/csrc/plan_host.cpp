@@ -325,7 +325,8 @@ struct Cand {
 // columns closer than W.  (Footprints of a round may overlap otherwise: lane i's row step l
 // and lane j's row step l' != l are separated by a barrier.)
 struct Occupancy {          // one bitmap row per base row, up to 128 base columns
-    uint64_t rows[SB_H > GT_ROWS ? SB_H : GT_ROWS][2];
+    uint64_t rows[SB_H_MAX > GT_ROWS_MAX ? SB_H_MAX : GT_ROWS_MAX][2];
+    int kh = 5;                // W - 1
     void clear() { std::memset(rows, 0, sizeof(rows)); }
     bool overlaps(int lx, int ly) const
     {
@@ -333,7 +334,7 @@ struct Occupancy {          // one bitmap row per base row, up to 128 base colum
     }
     void mark(int lx, int ly)
     {
-        const int lo = std::max(lx - KH, 0), hi = std::min(lx + KH, 127);
+        const int lo = std::max(lx - kh, 0), hi = std::min(lx + kh, 127);
         unsigned __int128 m = ((((unsigned __int128)1) << (hi - lo + 1)) - 1) << lo;
         constexpr int NR = (int)(sizeof(rows) / sizeof(rows[0]));
         // a step covers SC_STEP_ROWS rows from each lane's own base row: base rows closer than
@@ -346,11 +347,12 @@ struct Occupancy {          // one bitmap row per base row, up to 128 base colum
 
 // Greedy packing of `cands` (in order) into rounds of 32 lanes.  Appends 32 slots per
 // round to `out`; returns the number of rounds.
-static int build_rounds(std::vector<Cand> &cands, bool disjoint, int pitch,
+static int build_rounds(std::vector<Cand> &cands, bool disjoint, int pitch, int W,
                         std::vector<Slot> &out, long long &filled)
 {
     int rounds = 0;
     Occupancy occ;
+    occ.kh = W - 1;
     std::vector<Cand> next;
     next.reserve(cands.size());
     while (!cands.empty()) {
@@ -456,7 +458,7 @@ void finish_gather(Schedules &out, int n_workers)
 
 static void build_gather(const Geometry &g, Schedules &out, int n_workers)
 {
-    const int G = g.G;
+    const int G = g.G, KW = g.W;
     const bool half = out.half;
     const int k0 = half ? half_k_begin(g) : 0, k1 = half ? half_k_end(g) : g.n_det, nk = k1 - k0;
     // half: bases of the j >= 0 samples lie in rows [G/2 - W/2, G - W/2]; tiles start there
@@ -491,7 +493,7 @@ static void build_gather(const Geometry &g, Schedules &out, int n_workers)
         cands.clear();
         for (uint32_t q = count[t]; q < count[t + 1]; ++q) cands.push_back(all[order[q]]);
         const int rb = (int)(out.gather_slots.size() / 32);
-        const int nr = build_rounds(cands, false, GT_PITCH, out.gather_slots, out.gather_filled);
+        const int nr = build_rounds(cands, false, gt_pitch(KW), KW, out.gather_slots, out.gather_filled);
         for (int r = 0; r < nr; r += GATHER_ROUND_CAP) {
             GatherCta c;
             c.tx0 = (t % ntx) * GT_X; c.ty0 = (int)posmod(yorg + (t / ntx) * GT_Y, G);
@@ -531,7 +533,7 @@ static void scatter_rects(const Geometry &g, bool half, std::vector<RowSeg> &seg
 
 static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
 {
-    const int G = g.G;
+    const int G = g.G, KW = g.W, KH = KW - 1;
     const bool half = out.half;
     const int k_end = scatter_k_end(g, half);
     int round_max = SCATTER_ROUND_MAX;       // set below, once the incidences are counted
@@ -649,7 +651,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
                     // one greedy packing over "inside first, clipped after": the leading rounds
                     // come out all-inside, one round mixes, the rest is clipped
                     part.insert(part.end(), part_clip.begin(), part_clip.end());
-                    const int nr = build_rounds(part, true, ACC_PITCH, tmp_slots, f);
+                    const int nr = build_rounds(part, true, ACC_PITCH, KW, tmp_slots, f);
                     rc[kk * SCATTER_ITEMS + it] = nr;
                     int nf = 0;
                     for (; nf < nr; ++nf) {
@@ -715,7 +717,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
 // ---------------------------------------------------------------- paper's bins ----
 void build_paper_bins(const Geometry &g, int n_bins_target, PaperBins &out)
 {
-    const int G = g.G;
+    const int G = g.G, KH = g.W - 1;
     struct Node { int x0, y0, w, h; std::vector<PaperBinEntry> e; };
     auto cost = [](const Node &n) { return (long long)n.e.size() * n.w * n.h; };
     auto base_of = [&](const PaperBinEntry &en, int &bx, int &by) {
@@ -806,7 +808,7 @@ void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers
 // ---------------------------------------------------------------- self check -----
 static inline uint64_t tap_hash(uint32_t ak, int tx, int ty)
 {
-    uint64_t h = (uint64_t)ak * 0x9E3779B97F4A7C15ull + (uint64_t)(ty * KW + tx + 1) * 0xC2B2AE3D27D4EB4Full;
+    uint64_t h = (uint64_t)ak * 0x9E3779B97F4A7C15ull + (uint64_t)(ty * KW_MAX + tx + 1) * 0xC2B2AE3D27D4EB4Full;
     h ^= h >> 29;
     return h | 1ull;
 }
@@ -814,7 +816,7 @@ static inline uint64_t tap_hash(uint32_t ak, int tx, int ty)
 long long check_schedules(const Geometry &g, const Schedules &s)
 {
     long long bad = 0;
-    const int G = g.G;
+    const int G = g.G, KW = g.W, KH = KW - 1;
     const bool half = s.half;
     const int kg0 = half ? half_k_begin(g) : 0, kg1 = half ? half_k_end(g) : g.n_det;   // gather samples
     const int ks1 = scatter_k_end(g, half);                                              // scatter samples
@@ -830,7 +832,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         for (int i = 0; i < 32; ++i) {
             if (lanes[i].ak == SLOT_EMPTY) continue;
             const int xi = lanes[i].lxy & 0xffff, yi = lanes[i].lxy >> 16;
-            if (disjoint && (xi >= SB_W || yi >= SB_H)) ++bad;
+            if (disjoint && (xi >= ST_X + KH || yi >= ST_Y + KH)) ++bad;
             int same_bank = 0;      // lanes of this half-warp in the same bank pair: at most 2-way
             for (int j = 0; j < 32; ++j)
                 if (j != i && lanes[j].ak != SLOT_EMPTY && (i >> 4) == (j >> 4) &&
@@ -856,7 +858,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         if (c.round_count < 1 || c.round_count > GATHER_ROUND_CAP) ++bad;
         for (int r = 0; r < c.round_count; ++r) {
             const Slot *lanes = &s.gather_slots[(size_t)(c.round_begin + r) * 32];
-            check_round(lanes, GT_PITCH, false);
+            check_round(lanes, gt_pitch(KW), false);
             for (int l = 0; l < 32; ++l) {
                 if (lanes[l].ak == SLOT_EMPTY) continue;
                 const int a = lanes[l].ak >> 16, k = lanes[l].ak & 0xffff;

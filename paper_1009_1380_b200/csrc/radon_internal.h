@@ -7,8 +7,18 @@
 namespace radon {
 
 // ---- compile-time configuration -------------------------------------------------
-constexpr int KW = 6;                 // Kaiser-Bessel width this build is specialised for
-constexpr int KH = KW - 1;            // halo: a footprint reaches base .. base+KH
+// Kaiser-Bessel widths this build carries: the gridding kernels are instantiated for each (even
+// widths: the polynomial pieces pair up), the host code takes W at run time.  A footprint reaches
+// base .. base + W - 1 ("halo" W - 1).
+constexpr int KW_MAX = 8;
+inline bool kw_supported(int W) { return W == 4 || W == 6 || W == 8; }
+#define RADON_FOR_W(Wrt, BODY)                        \
+    switch (Wrt) {                                    \
+    case 4: { constexpr int WW = 4; BODY } break;     \
+    case 6: { constexpr int WW = 6; BODY } break;     \
+    case 8: { constexpr int WW = 8; BODY } break;     \
+    default: break;                                   \
+    }
 // Kaiser-Bessel weights: ONE polynomial piece per tap (degree KB_DEG in z = 2*delta - 1, fitted
 // in fp64 at plan time, max error ~7e-8), passed to the kernels in the constant bank -- a lookup
 // table whose rows are polynomial pieces, read as broadcast operands, so it costs neither
@@ -18,25 +28,26 @@ constexpr int KH = KW - 1;            // halo: a footprint reaches base .. base+
 // the gather 56 % slower); the polynomial pieces are what the library ships.
 constexpr int KB_DEG = 7;
 constexpr int KB_HALF = (KB_DEG + 1) / 2;   // coefficients of the even / odd part
-struct KbPoly {                       // tap l: E_l(z^2) + z O_l(z^2); tap KW-1-l: E_l - z O_l
-    float e[KW / 2][KB_HALF];
-    float o[KW / 2][KB_HALF];
+struct KbPoly {                       // tap l: E_l(z^2) + z O_l(z^2); tap W-1-l: E_l - z O_l
+    float e[KW_MAX / 2][KB_HALF];
+    float o[KW_MAX / 2][KB_HALF];
 };
 #ifdef __CUDACC__
 #define RADON_HD __host__ __device__ __forceinline__
 #else
 #define RADON_HD inline
 #endif
-// w[l] = phi(delta - W/2 + l), l = 0..KW-1, delta in [0,1]: Horner in z^2 on the even and odd
+// w[l] = phi(delta - W/2 + l), l = 0..W-1, delta in [0,1]: Horner in z^2 on the even and odd
 // parts.  In the kernels kp sits in the parameter constant bank, so its entries are FFMA
 // operands, not loads.  Host-callable for the CPU-side unit test.
-RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
+template <int W>
+RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[W])
 {
     const float z = 2.f * delta - 1.f, z2 = z * z;
 #ifdef __CUDACC__
 #pragma unroll
 #endif
-    for (int l = 0; l < KW / 2; ++l) {
+    for (int l = 0; l < W / 2; ++l) {
         float e = kp.e[l][KB_HALF - 1], o = kp.o[l][KB_HALF - 1];
 #ifdef __CUDACC__
 #pragma unroll
@@ -46,7 +57,7 @@ RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
             o = o * z2 + kp.o[l][h];
         }
         w[l] = e + z * o;
-        w[KW - 1 - l] = e - z * o;
+        w[W - 1 - l] = e - z * o;
     }
 }
 // Gather (inverse gridding): a work item is a GT_X x GT_Y tile of the grid (+halo), staged by
@@ -60,13 +71,14 @@ RADON_HD void kb_poly_weights(const KbPoly &kp, float delta, float (&w)[KW])
 #define RADON_GSTAGES 3
 #endif
 constexpr int GT_X = RADON_GT_X, GT_Y = RADON_GT_Y;
-constexpr int GT_PITCH = GT_X + KH + 1;   // complex per smem row: 16-byte multiple for the bulk copies
-constexpr int GT_ROWS = GT_Y + KH;    // 21 rows staged per tile
+constexpr int gt_pitch(int W) { return GT_X + W; }       // complex per smem row (tile + halo W - 1, + 1): 16-byte multiple for the bulk copies
+constexpr int gt_rows(int W) { return GT_Y + W - 1; }    // rows staged per tile (21 at W = 6)
+constexpr int GT_ROWS_MAX = gt_rows(KW_MAX);
 #ifndef RADON_GWARPS
 #define RADON_GWARPS 24
 #endif
 constexpr int GATHER_WARPS = RADON_GWARPS;      // consumer warps of the persistent gather CTA (+1 producer warp)
-constexpr int GATHER_STAGES = RADON_GSTAGES;   // tiles in flight per CTA (GT_ROWS x GT_PITCH x 8 B = 65.5 KB each)
+constexpr int GATHER_STAGES = RADON_GSTAGES;   // tiles in flight per CTA (gt_rows x gt_pitch x 8 B = 65.5 KB each at W = 6)
 #ifndef RADON_GCOST
 #define RADON_GCOST 16
 #endif
@@ -105,7 +117,7 @@ constexpr int SQ_X = RADON_SQ_X, SQ_Y = RADON_SQ_Y;   // quadrants per rectangle
 constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
 constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
-constexpr int SB_W = ST_X + KH, SB_H = ST_Y + KH;   // range of biased base coordinates in a quadrant
+constexpr int SB_W_MAX = ST_X + KW_MAX - 1, SB_H_MAX = ST_Y + KW_MAX - 1;   // range of biased base coordinates in a tile (ST + W - 1)
 constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples are split over CTAs: upper and
 #ifndef RADON_SC_RMIN
 #define RADON_SC_RMIN 12
@@ -128,7 +140,7 @@ struct GatherCta {              // one work item of the gather: a staged tile an
 };
 
 struct ScatterItem {            // one warp: quadrant (relative to the rectangle) and its rounds
-    int sx0, sy0, sw, sh;       // slot coordinates are relative to (sx0 - KH, sy0 - KH)
+    int sx0, sy0, sw, sh;       // slot coordinates are relative to (sx0 - (W-1), sy0 - (W-1))
     int round_begin, round_count;
     int fast_count;             // the first fast_count rounds hold only footprints wholly inside the quadrant
     int pad;
@@ -156,7 +168,7 @@ constexpr int MAX_DC_JOBS = 4;  // the (W+1)^2 centre window touches at most 2 x
 
 // ---- host-side geometry + schedules ----------------------------------------------
 struct Geometry {
-    int N = 0, G = 0, n_angles = 0, n_det = 0, W = KW;
+    int N = 0, G = 0, n_angles = 0, n_det = 0, W = 6;
     double sigma = 2.0;
     std::vector<double> cs;     // per angle: (G/n) cos(theta_a), (G/n) sin(theta_a)
 

@@ -41,7 +41,7 @@ def test_strerror_and_validation_without_gpu():
     assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 13) == -1
     assert L.radon_plan_create(ctypes.byref(h), 65, 90, 91, 1.5, 6) == -1                   # odd sigma*N
     assert L.radon_plan_create(None, 64, 90, 91, 2.0, 6) == -1
-    assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 4) == -5                   # W != 6: not built
+    assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 10) == -5                  # W not in {4, 6, 8}: not built
     assert L.radon_plan_create(ctypes.byref(h), 96, 90, 91, 2.0, 6) == -5                   # G not a power of two
     assert L.radon_plan_destroy(None) == 0
     assert L.radon_forward(None, None, None, None) == -1
@@ -169,7 +169,7 @@ def test_plan_create_rejects_bad_and_unbuilt_requests_without_touching_a_gpu():
     assert create(64, 90, 91, sigma=1.0)[0] == -1 and create(64, 90, 91, sigma=9.0)[0] == -1
     assert create(63, 90, 91, sigma=1.5)[0] == -1                          # sigma N not an even integer
     assert create(64, 90, 91, W=1)[0] == -1 and create(64, 90, 91, W=13)[0] == -1
-    assert create(64, 90, 91, W=8)[0] == -5 and create(64, 90, 91, W=4)[0] == -5      # valid, not built
+    assert create(64, 90, 91, W=10)[0] == -5 and create(64, 90, 91, W=5)[0] == -5     # valid, not built (4, 6, 8 are)
     assert create(1536, 1025, 2048)[0] == -5                               # sigma N = 3072 is not a power of two
     assert create(64, 90, 5000)[0] == -5                                   # Bluestein length > 8192
     assert b"power of two" in L.radon_strerror(-5)
@@ -179,12 +179,29 @@ def test_plan_create_rejects_bad_and_unbuilt_requests_without_touching_a_gpu():
     assert L.radon_filter_basis_host(8, 3, None) == -1 and L.radon_filter_basis_host(8, 3, q) == 0
     w = (ctypes.c_float * 6)()
     assert L.radon_kb_weights_host(6, ctypes.c_float(2.0), ctypes.c_float(1.5), w) == -1
-    assert L.radon_kb_weights_host(8, ctypes.c_float(2.0), ctypes.c_float(0.5), w) == -5
+    assert L.radon_kb_weights_host(10, ctypes.c_float(2.0), ctypes.c_float(0.5), w) == -5
     bad = ctypes.c_longlong()
-    assert L.radon_schedule_selfcheck(64, 90, 91, ctypes.c_float(2.0), 8, 0, ctypes.byref(bad)) == -5
+    assert L.radon_schedule_selfcheck(64, 90, 91, ctypes.c_float(2.0), 10, 0, ctypes.byref(bad)) == -5
     assert L.radon_density_host(64, 90, 91, ctypes.c_float(2.0), 6, None, None) == -1
     # a NULL plan is an argument error everywhere, never a crash
     for name in ("radon_forward", "radon_adjoint", "radon_inverse", "radon_nufft2", "radon_nufft1", "radon_interp_only",
                  "radon_grid_only", "radon_proj_ifft", "radon_proj_fft", "radon_forward_filtered", "radon_adjoint_filtered"):
         assert getattr(L, name)(None, None, None, None) == -1, name
     assert L.radon_plan_destroy(None) == 0
+
+
+@pytest.mark.parametrize("W", [4, 8])
+def test_other_kernel_widths_weights_and_schedules(W):
+    """radon_plan_create(..., W) for the other widths the library is instantiated for: the tap
+    weights against the oracle's directly evaluated Kaiser-Bessel kernel, and the host schedule
+    builder's invariants with footprints of W x W cells."""
+    import oracle
+
+    beta = oracle.kb_beta(W, 2.0)
+    for delta in (0.0, 0.123, 0.5, 0.77, 1.0):
+        w = rb.kb_weights_host(delta, W=W)
+        ref = oracle.kb_phi(delta - W / 2 + np.arange(W), W, beta)
+        assert np.max(np.abs(np.array(w) - ref)) < 5e-7, (W, delta)
+    for shape in [(16, 7, 12), (64, 90, 91), (128, 64, 181)]:
+        for half in (False, True):
+            assert rb.schedule_selfcheck(*shape, W=W, half=half) == (0, 0), (W, shape, half)
