@@ -64,14 +64,16 @@ extern "C" {
 #define RADON_ENOMEM       -2   /* host or device allocation failed */
 #define RADON_ECUDA        -3   /* a CUDA runtime call failed (radon_last_cuda_error) */
 #define RADON_EARCH        -4   /* current device is not compute capability 10.x */
-#define RADON_EUNSUPPORTED -5   /* valid but not built: W not 4, 6 or 8, sigma*N not a power of two in [16, 8192],
+#define RADON_EUNSUPPORTED -5   /* valid but not built: W not 4, 6 or 8; sigma*N neither a power of two in [16, 8192]
+                                   nor 3 or 5 times a power of two in [16, 2048];
                                    n_det > 8192 (power of two) or 2*n_det - 1 > 8192 (otherwise) */
 
 typedef struct radon_plan radon_plan;   /* opaque, owned by the library */
 
 /* Plan for images N x N, n_angles uniform angles in [0, pi), n_det detector bins,
- * oversampling sigma (G = sigma*N must be an even integer; this build needs a
- * power of two, 16 <= G <= 8192) and Kaiser-Bessel width W (this build: 4, 6 or 8; the gridding
+ * oversampling sigma (G = sigma*N must be an even integer; this build takes a power of two,
+ * 16 <= G <= 8192 -- the tuned FFT passes -- or 3 or 5 times a power of two in [16, 2048], e.g. N = 1536
+ * or 2560 at sigma = 2 -- plainer passes, about 1.6 times the time per grid cell) and Kaiser-Bessel width W (this build: 4, 6 or 8; the gridding
  * kernels are instantiated for each; 6 is north_star's and the one the benchmarks run).
  * Builds, for the current CUDA device: per-angle fp64 direction table (Fourier
  * slice geometry), Kaiser-Bessel weight table (polynomial pieces) and de-apodisation vectors,

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libradon_b200.so")
-SOURCES = ["api.cu", "gridding.cu", "fft2d.cu", "proj.cu", "filter.cu", "paper_bins.cu", "plan_device.cu", "plan_host.cpp"]
+SOURCES = ["api.cu", "gridding.cu", "fft2d.cu", "fft2d_composite.cu", "proj.cu", "filter.cu", "paper_bins.cu", "plan_device.cu", "plan_host.cpp"]
 HEADERS = ["kernels.h", "radon_internal.h", "fft_device.cuh", "async_copy.cuh", "taps.cuh", "plan_device.h", os.path.join("..", "..", "include", "radon.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",

@@ -141,7 +141,7 @@ extern "C" int radon_plan_destroy(radon_plan *p)
     if (!p) return RADON_OK;
     cudaDeviceSynchronize();
     DevicePlan &d = p->dev;
-    cudaFree(d.cs); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_P);
+    cudaFree(d.cs); cudaFree(d.deapod); cudaFree(d.tw_G); cudaFree(d.tw_sub); cudaFree(d.tw_P);
     cudaFree(d.chirp_a); cudaFree(d.chirp_b); cudaFree(d.chirp_hf);
     for (auto &q : d.sched) {
         cudaFree(q.gather_ctas); cudaFree(q.gather_worker_begin); cudaFree(q.gather_slots); cudaFree(q.scatter_ctas); cudaFree(q.scatter_slots);
@@ -208,6 +208,13 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     if ((rc = dev_upload(p, &d.deapod, deapod))) return rc;
     build_twiddles(G, tw);
     if ((rc = dev_upload(p, &d.tw_G, tw))) return rc;
+    {
+        int P = 0, PR = 0;
+        if ((G & (G - 1)) != 0 && fft_composite_split(G, &P, &PR)) {
+            build_twiddles(P, tw);
+            if ((rc = dev_upload(p, &d.tw_sub, tw))) return rc;
+        }
+    }
     build_twiddles(d.LP, tw);
     if ((rc = dev_upload(p, &d.tw_P, tw))) return rc;
     build_chirp(n_det, d.LP, ca, cb, hf);
@@ -1013,7 +1020,7 @@ extern "C" const char *radon_strerror(int code)
     case RADON_ENOMEM: return "out of memory";
     case RADON_ECUDA: return "CUDA runtime error (see radon_last_cuda_error)";
     case RADON_EARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
-    case RADON_EUNSUPPORTED: return "valid request outside this build (W not 4, 6 or 8, or sigma*N not a power of two in [16, 8192], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
+    case RADON_EUNSUPPORTED: return "valid request outside this build (W not 4, 6 or 8, or sigma*N neither a power of two in [16, 8192] nor 3 or 5 times a power of two in [16, 2048], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
     default: return "unknown error";
     }
 }

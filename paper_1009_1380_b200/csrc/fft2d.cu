@@ -374,7 +374,11 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
 }
 
 // ---- dispatch on the FFT length -----------------------------------------------------------
-bool fft_length_supported(int L) { return L >= 16 && L <= 8192 && (L & (L - 1)) == 0; }
+bool fft_length_supported(int L)
+{
+    if (L >= 16 && L <= 8192 && (L & (L - 1)) == 0) return true;
+    return fft_composite_split(L, nullptr, nullptr);
+}
 
 template <int L>
 static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
@@ -443,6 +447,7 @@ static int fft2d_launch(int which, const DevicePlan &p, const void *in, void *ou
 int launch_fft2d_pass(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
                       const IstaUpdate *upd)
 {
+    if ((p.G & (p.G - 1)) != 0) return launch_fft2d_composite(which, p, in, out, flag, st, upd);
     RADON_FOR_L(p.G, return fft2d_launch<LL>(which, p, in, out, flag, st, upd);)
     return -1;
 }

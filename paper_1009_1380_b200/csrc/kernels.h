@@ -19,6 +19,7 @@ struct DevicePlan {
     KbPoly kb;                    // polynomial pieces of the Kaiser-Bessel kernel
     float *deapod = nullptr;      // N
     float2 *tw_G = nullptr;       // twiddles for length G
+    float2 *tw_sub = nullptr;     // G = 3 or 5 times a power of two P: twiddles for length P (fft2d_composite.cu)
     float2 *tw_P = nullptr;       // twiddles for length LP
     float2 *chirp_a = nullptr, *chirp_b = nullptr, *chirp_hf = nullptr;   // hf == nullptr: direct FFT
     // schedules: [0] every sample / whole grid (arbitrary complex data: the test hooks),
@@ -37,7 +38,10 @@ struct DevicePlan {
 // A4 epilogue of a solver iteration: x <- S_tau(x - alpha * g) in place, g the freshly computed adjoint
 struct IstaUpdate { float alpha = 0.f, tau = 0.f; };
 
-bool fft_length_supported(int L);
+bool fft_length_supported(int L);            // power of two in [16, 8192], or 3 / 5 times a power of two in [16, 2048]
+bool fft_composite_split(int L, int *P_out, int *PR_out);
+int launch_fft2d_composite(int which, const DevicePlan &p, const void *in, void *out, int flag, cudaStream_t st,
+                           const IstaUpdate *upd);
 int init_kernel_attributes();
 long long launch_count();
 void count_launch(long long n = 1);

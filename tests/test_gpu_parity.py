@@ -217,7 +217,7 @@ def test_invalid_arguments_are_refused_with_error_codes(rb):
     assert L.radon_plan_create(ctypes.byref(h), 64, 0, 8, ctypes.c_float(2.0), 6) == -1       # no angles
     assert L.radon_plan_create(ctypes.byref(h), 64, 4, 1, ctypes.c_float(2.0), 6) == -1       # n_det < 2
     assert L.radon_plan_create(ctypes.byref(h), 64, 4, 8, ctypes.c_float(2.0), 10) == -5      # W not 4, 6, 8: unsupported build
-    assert L.radon_plan_create(ctypes.byref(h), 96, 4, 8, ctypes.c_float(2.0), 6) != 0        # sigma*N not a power of two
+    assert L.radon_plan_create(ctypes.byref(h), 56, 4, 8, ctypes.c_float(2.0), 6) == -5       # sigma*N = 7 * 16: not built
     assert not h.value
     plan = rb.RadonPlan(16, 3, 9)
     assert L.radon_forward(plan._h, None, None, None) == -1
@@ -479,3 +479,39 @@ def test_other_kernel_widths_match_the_oracle(rb, W):
     got = p1.radon_inverse(torch.from_numpy(y1.astype(np.float32)).cuda()).cpu().numpy()
     assert rel(got, oracle.inverse(y1, c1.N, W=W, brute=True)) < (1e-5 if W == 8 else 1e-3)
     p1.close()
+
+
+@pytest.mark.parametrize("shape", [(96, 60, 131), (80, 45, 100), (24, 9, 32), (1536, 1025, 2048)])
+def test_grid_sides_three_or_five_times_a_power_of_two(rb, shape):
+    """sigma N = 3 * 2^m or 5 * 2^m (a 1536^2 or 2560^2 slice at sigma = 2): the composite FFT passes
+    (one decimation step in front of the power-of-two FFT, fft2d_composite.cu).  Forward / adjoint
+    against O-alg on full arrays, against O-direct (full at the small shapes, a stratified-random
+    subset at 1536^2), the adjoint identity, the bare NUFFT pair and the solver step."""
+    N, na, nd = shape
+    plan = rb.RadonPlan(N, na, nd)
+    assert plan.G == 2 * N and (plan.G & (plan.G - 1)) != 0
+    rng = np.random.default_rng(N)
+    x = workloads.make_batch_slice(7, N) if N >= 64 else rng.standard_normal((N, N)).astype(np.float32)
+    S = plan.radon_forward(torch.from_numpy(x).cuda()).cpu().numpy()
+    y = rng.standard_normal((na, nd)).astype(np.float32)
+    A = plan.radon_adjoint(torch.from_numpy(y).cuda()).cpu().numpy()
+    # (24, 9, 32): one of nine rays is an exact-tie ray (reading R-tie, boundary tap 9e-6): a larger share than at real sizes
+    tol = 2e-6 if N >= 64 else 5e-6
+    assert rel(S, oracle.fast_forward(x, na, nd)) < tol
+    assert rel(A, oracle.fast_adjoint(y.astype(np.float64), N)) < tol
+    if N <= 96:
+        assert rel(S, oracle.forward(x, na, nd)) < 2e-5 if N < 64 else rel(S, oracle.forward(x, na, nd)) < G1
+        P = plan.radon_nufft2(torch.from_numpy(x).cuda()).cpu().numpy()
+        assert rel(P, oracle.ndft2(x, na, nd)) < G2
+    else:
+        idx = rng.choice(na * nd, 256, replace=False)
+        assert rel(S.ravel()[idx], oracle.dirichlet_forward_subset(x, na, nd, idx)) < G1
+    lhs = float(np.vdot(S.astype(np.float64), y)); rhs = float(np.vdot(x.astype(np.float64), A))
+    assert abs(lhs - rhs) <= 5e-6 * np.linalg.norm(S) * np.linalg.norm(y)
+    # the solver step's fused epilogues exist on this path too
+    xs = torch.zeros((N, N), device="cuda"); b = torch.from_numpy(S).cuda()
+    plan.radon_solver_step(xs, b, 1e-3 / max(float(np.abs(A).max()), 1e-6), 0.0)
+    ref = oracle.ista_step(np.zeros((N, N)), S, 1e-3 / max(float(np.abs(A).max()), 1e-6), 0.0,
+                           lambda u: oracle.fast_forward(u, na, nd), lambda v: oracle.fast_adjoint(v, N))
+    assert rel(xs.cpu().numpy(), ref) < 1e-5
+    plan.close()

@@ -42,7 +42,7 @@ def test_strerror_and_validation_without_gpu():
     assert L.radon_plan_create(ctypes.byref(h), 65, 90, 91, 1.5, 6) == -1                   # odd sigma*N
     assert L.radon_plan_create(None, 64, 90, 91, 2.0, 6) == -1
     assert L.radon_plan_create(ctypes.byref(h), 64, 90, 91, 2.0, 10) == -5                  # W not in {4, 6, 8}: not built
-    assert L.radon_plan_create(ctypes.byref(h), 96, 90, 91, 2.0, 6) == -5                   # G not a power of two
+    assert L.radon_plan_create(ctypes.byref(h), 56, 90, 91, 2.0, 6) == -5                   # G = 112 = 7 * 16: not built
     assert L.radon_plan_destroy(None) == 0
     assert L.radon_forward(None, None, None, None) == -1
 
@@ -170,7 +170,7 @@ def test_plan_create_rejects_bad_and_unbuilt_requests_without_touching_a_gpu():
     assert create(63, 90, 91, sigma=1.5)[0] == -1                          # sigma N not an even integer
     assert create(64, 90, 91, W=1)[0] == -1 and create(64, 90, 91, W=13)[0] == -1
     assert create(64, 90, 91, W=10)[0] == -5 and create(64, 90, 91, W=5)[0] == -5     # valid, not built (4, 6, 8 are)
-    assert create(1536, 1025, 2048)[0] == -5                               # sigma N = 3072 is not a power of two
+    assert create(56, 90, 91)[0] == -5 and create(6144, 90, 91)[0] == -5   # sigma N = 7 * 16; 3 * 4096 (sub-length > 2048)
     assert create(64, 90, 5000)[0] == -5                                   # Bluestein length > 8192
     assert b"power of two" in L.radon_strerror(-5)
     # host-only entry points
