@@ -249,16 +249,6 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
         }
         p->gather_filled[h] = sch.gather_filled;
         p->scatter_filled[h] = sch.scatter_filled;
-        if (std::getenv("RADON_PLAN_DEBUG")) {
-            long long rounds = 0, fast = 0, mx = 0, heavy = 0;
-            for (const ScatterCta &c : sch.scatter_ctas) {
-                rounds += c.items[0].round_count; fast += c.items[0].fast_count;
-                mx = std::max<long long>(mx, c.items[0].round_count);
-                heavy += c.partial_slot >= 0 ? 1 : 0;
-            }
-            fprintf(stderr, "schedule half=%d device=%d: scatter ctas %zu rounds %lld fast %lld max %lld partial ctas %lld jobs %zu\n",
-                    h, p->device_built[h], sch.scatter_ctas.size(), rounds, fast, mx, heavy, sch.merge_jobs.size());
-        }
         q.n_gather_ctas = (int)sch.gather_ctas.size();
         q.n_scatter_ctas = (int)sch.scatter_ctas.size();
         q.n_merge_jobs = (int)sch.merge_jobs.size();
