@@ -9,7 +9,8 @@ C-ABI calls (pinned host memory, copies inside the timed region).  Beside the co
 line carries `stages` (per-stage CUDA events of a second, untimed pass), `roofline` (the dominant
 stage against the measured HBM peak), `gridding_kernels` (the bare interpolation / gridding kernels
 on complex data, SURVEY 8(d)'s 151 MB, north_star's 50 % target), `paper_shape` (PAPER.md:59's own
-180 x 1024 shape, context), `next_rows` (radon_inverse) and `cpu_baseline` (the oracle, sampled).
+180 x 1024 shape, context), `next_rows` (radon_inverse, solver loop, filter), `library_context` (cuFFT timed beside the FFT passes:
+a yardstick, never on the product path) and `cpu_baseline` (the oracle, sampled).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--slices B] [--impl reference]
   torchrun ... bench.py --gpus N ...      one rank per GPU; slice-parallel replicas (weak scaling)
@@ -203,6 +204,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=512)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-library-context", action="store_true", help="skip the cuFFT yardstick (context only)")
     ap.add_argument("--no-clock-load", action="store_true",
                     help="skip the 0.5 s of untimed identical steps that give nvidia-smi time to sample "
                          "(profiling runs: keeps the kernel launch list short and deterministic)")
@@ -489,6 +491,33 @@ def main():
 
     if rank != 0:
         return 0
+    # ---- context only, never on the product path: the vendor FFT library (cuFFT through torch.fft)
+    #      on the transforms F1-F2 and A3-A4 stand for, same sizes, inputs cycling through HBM ----
+    library_context = None
+    if not args.no_library_context and per_stage:
+        G = cfg.G
+        imgs = [torch.randn(cfg.N, cfg.N, device=dev) for _ in range(4)]
+        spec = [torch.fft.rfft2(im, s=(G, G)) for im in imgs]
+        rows_c = [torch.randn(1024, G, device=dev, dtype=torch.complex64) for _ in range(8)]
+        lc = {}
+        for label, fn in (("rfft2_zero_padded_N_to_G", lambda i: torch.fft.rfft2(imgs[i % 4], s=(G, G))),
+                          ("irfft2_G", lambda i: torch.fft.irfft2(spec[i % 4], s=(G, G))),
+                          ("fft_1024_contiguous_rows_of_G", lambda i: torch.fft.fft(rows_c[i % 8], dim=1))):
+            for i in range(3):
+                fn(i)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(20):
+                fn(i)
+            e1.record()
+            torch.cuda.synchronize()
+            lc[label] = round(e0.elapsed_time(e1) / 20 * 1e3, 1)
+        lc["this_library_us"] = {"F1+F2 (de-apodise, pad, 2-D FFT, Hermitian half)": round(per_stage["F1_colfft"]["us_per_launch"] + per_stage["F2_rowfft"]["us_per_launch"], 1),
+                                 "A3+A4 (2-D inverse FFT, crop, de-apodise)": round(per_stage["A3_rowifft"]["us_per_launch"] + per_stage["A4_colifft"]["us_per_launch"], 1),
+                                 "one column pass = 1024 FFTs of length G on column pairs": per_stage["F1_colfft"]["us_per_launch"]}
+        lc["note"] = "cuFFT via torch.fft, us per call; a yardstick for the FFT passes, not used by the library"
+        library_context = lc
+        del imgs, spec, rows_c
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         v, cores, dt = cpu_oracle_pairs_per_s(cfg, args.ref_sample)
@@ -510,7 +539,7 @@ def main():
                  "note": "radon_plan_create: tables + schedules (CUDA kernels, plan_device.cu) + first workspace; the batched calls "
                          "add three more workspaces on first use"},
         "roofline": roofline, "stages": per_stage, "gridding_kernels": gk, "paper_shape": paper_shape, "next_rows": next_rows,
-        "cpu_baseline": cpu_baseline,
+        "library_context": library_context, "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line))
     return 0
