@@ -112,9 +112,10 @@ colpass_fwd_kernel(const float *__restrict__ x, const float *__restrict__ deapod
         if (S2) v[i] = (i < 4 || i >= 12) ? (live ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f)) : make_float2(0.f, 0.f);
         else v[i] = (live && iy < N) ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
     }
-    __syncthreads();
-    fft_reg<L, -1>(v, s, tw, t);
-    __syncthreads();
+    // from here to the cooperative store the four FFTs of the CTA only meet their own threads
+    fft_sync<TF, true>(f);
+    fft_reg<L, -1, true>(v, s, tw, t, f);
+    fft_sync<TF, true>(f);
 #pragma unroll
     for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
     pdl_trigger();
@@ -160,7 +161,7 @@ rowpass_fwd_kernel(const float2 *__restrict__ T, float2 *__restrict__ grid,
         if (S2) v[i] = (i < 4 || i >= 12) ? (live ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f)) : make_float2(0.f, 0.f);
         else v[i] = (live && ix < N) ? __ldg(&T[(size_t)ky * N + ix]) : make_float2(0.f, 0.f);
     }
-    fft_reg<L, -1>(v, s, tw, t);
+    fft_reg<L, -1, true>(v, s, tw, t, f);
     pdl_trigger();
     if (!live) return;
     const int cy = (ky + L / 2) & (L - 1);
@@ -211,7 +212,7 @@ rowpass_inv_kernel(const float2 *__restrict__ grid, float2 *__restrict__ T,
             }
         }
     }
-    fft_reg<L, +1>(v, s, tw, t);
+    fft_reg<L, +1, true>(v, s, tw, t, f);
     pdl_trigger();
     if (!live) return;
 #pragma unroll
@@ -281,7 +282,7 @@ rowpass_inv_staged_kernel(const float2 *__restrict__ grid, float2 *__restrict__ 
         __syncthreads();                                    // stage is free; s is free (previous FFT done)
         if (threadIdx.x == 0 && g + (int)gridDim.x < n_groups) fetch(g + gridDim.x);
         if (g + (int)gridDim.x >= n_groups) pdl_trigger();      // this CTA's last group
-        fft_reg<L, +1>(v, s, tw, t);
+        fft_reg<L, +1, true>(v, s, tw, t, f);
         if (live) {
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
@@ -341,9 +342,9 @@ colpass_inv_kernel(const float2 *__restrict__ T, const float *__restrict__ deapo
     float2 v[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = live ? s[FFT_PAD(t + i * TF)] : make_float2(0.f, 0.f);
-    __syncthreads();
-    fft_reg<L, +1>(v, s, tw, t);
-    __syncthreads();
+    fft_sync<TF, true>(f);
+    fft_reg<L, +1, true>(v, s, tw, t, f);
+    fft_sync<TF, true>(f);
 #pragma unroll
     for (int i = 0; i < 16; ++i)
         if (!S2 || i < 4 || i >= 12) s[FFT_PAD(t + i * TF)] = v[i];       // S2: the other rows are cropped

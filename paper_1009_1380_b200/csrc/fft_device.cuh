@@ -119,12 +119,24 @@ __device__ __forceinline__ void dft_reg(float2 (&v)[R])
     }
 }
 
+// Barrier between the passes of one FFT.  GROUP == false: the whole CTA (__syncthreads).  GROUP ==
+// true: only the TF threads of this FFT (group grp of the CTA, threads grp*TF .. grp*TF + TF - 1):
+// a warp-level barrier when the group sits inside one warp, else the named barrier grp + 1, so that
+// the FFTs of a CTA drift apart and one group's exchange overlaps another's butterflies.
+template <int TF, bool GROUP>
+__device__ __forceinline__ void fft_sync(int grp)
+{
+    if constexpr (!GROUP) __syncthreads();
+    else if constexpr (TF <= 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(TF) : "memory");
+}
+
 // One Stockham pass of radix R; NS = product of the radices already applied.  Register slot
 // b + q*NB (NB = 16/R) holds input q of the thread's butterfly b (butterfly index j = b*TF + t).
 //   FIRST: inputs are already in v (slot i = element t + i*TF);   otherwise read from s.
 //   LAST (R == 16): outputs stay in v (slot u = element t + u*TF); otherwise written to s.
-template <int L, int R, int NS, int SIGN, bool FIRST, bool LAST>
-__device__ __forceinline__ void fft_pass(float2 (&v)[16], float2 *s, const float2 *__restrict__ tw, int t)
+template <int L, int R, int NS, int SIGN, bool FIRST, bool LAST, bool GROUP>
+__device__ __forceinline__ void fft_pass(float2 (&v)[16], float2 *s, const float2 *__restrict__ tw, int t, int grp)
 {
     constexpr int TF = L / 16, NB = 16 / R, STRIDE = L / R;
     if constexpr (!FIRST) {
@@ -132,7 +144,7 @@ __device__ __forceinline__ void fft_pass(float2 (&v)[16], float2 *s, const float
         for (int b = 0; b < NB; ++b)
 #pragma unroll
             for (int q = 0; q < R; ++q) v[b + q * NB] = s[FFT_PAD(b * TF + t + q * STRIDE)];
-        if constexpr (!LAST) __syncthreads();     // everybody has read before anybody overwrites
+        if constexpr (!LAST) fft_sync<TF, GROUP>(grp);     // everybody has read before anybody overwrites
     }
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
@@ -170,7 +182,7 @@ __device__ __forceinline__ void fft_pass(float2 (&v)[16], float2 *s, const float
             for (int u = 0; u < R; ++u) s[FFT_PAD(base + u * NS)] = x[u];
         }
     }
-    if constexpr (!LAST) __syncthreads();
+    if constexpr (!LAST) fft_sync<TF, GROUP>(grp);
 }
 
 // Length-L FFT (SIGN < 0: forward exp(-i..), SIGN > 0: unnormalised inverse).
@@ -178,35 +190,36 @@ __device__ __forceinline__ void fft_pass(float2 (&v)[16], float2 *s, const float
 // s: this FFT's private shared-memory scratch of fft_padded_len(L) float2, free on entry.
 // Every thread of the CTA must call it (it contains __syncthreads).  On return other threads
 // may still be reading s: the caller synchronises before writing s again.
-template <int L, int SIGN>
-__device__ __forceinline__ void fft_reg(float2 (&v)[16], float2 *s, const float2 *__restrict__ tw, int t)
+// GROUP: see fft_sync (then only the TF threads of group grp need to call it together).
+template <int L, int SIGN, bool GROUP = false>
+__device__ __forceinline__ void fft_reg(float2 (&v)[16], float2 *s, const float2 *__restrict__ tw, int t, int grp = 0)
 {
     constexpr int LOG = ilog2_c(L);
     constexpr int R0 = 1 << (LOG % 4);          // first pass: radix 1 (none), 2, 4 or 8
     constexpr int NQ = LOG / 4;                 // then NQ radix-16 passes
     static_assert(NQ >= 1 && NQ <= 3 && L >= 16, "length");
     if constexpr (R0 > 1) {
-        fft_pass<L, R0, 1, SIGN, true, false>(v, s, tw, t);
-        if constexpr (NQ == 1) fft_pass<L, 16, R0, SIGN, false, true>(v, s, tw, t);
+        fft_pass<L, R0, 1, SIGN, true, false, GROUP>(v, s, tw, t, grp);
+        if constexpr (NQ == 1) fft_pass<L, 16, R0, SIGN, false, true, GROUP>(v, s, tw, t, grp);
         if constexpr (NQ == 2) {
-            fft_pass<L, 16, R0, SIGN, false, false>(v, s, tw, t);
-            fft_pass<L, 16, R0 * 16, SIGN, false, true>(v, s, tw, t);
+            fft_pass<L, 16, R0, SIGN, false, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, R0 * 16, SIGN, false, true, GROUP>(v, s, tw, t, grp);
         }
         if constexpr (NQ == 3) {
-            fft_pass<L, 16, R0, SIGN, false, false>(v, s, tw, t);
-            fft_pass<L, 16, R0 * 16, SIGN, false, false>(v, s, tw, t);
-            fft_pass<L, 16, R0 * 256, SIGN, false, true>(v, s, tw, t);
+            fft_pass<L, 16, R0, SIGN, false, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, R0 * 16, SIGN, false, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, R0 * 256, SIGN, false, true, GROUP>(v, s, tw, t, grp);
         }
     } else {
-        if constexpr (NQ == 1) fft_pass<L, 16, 1, SIGN, true, true>(v, s, tw, t);
+        if constexpr (NQ == 1) fft_pass<L, 16, 1, SIGN, true, true, GROUP>(v, s, tw, t, grp);
         if constexpr (NQ == 2) {
-            fft_pass<L, 16, 1, SIGN, true, false>(v, s, tw, t);
-            fft_pass<L, 16, 16, SIGN, false, true>(v, s, tw, t);
+            fft_pass<L, 16, 1, SIGN, true, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, 16, SIGN, false, true, GROUP>(v, s, tw, t, grp);
         }
         if constexpr (NQ == 3) {
-            fft_pass<L, 16, 1, SIGN, true, false>(v, s, tw, t);
-            fft_pass<L, 16, 16, SIGN, false, false>(v, s, tw, t);
-            fft_pass<L, 16, 256, SIGN, false, true>(v, s, tw, t);
+            fft_pass<L, 16, 1, SIGN, true, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, 16, SIGN, false, false, GROUP>(v, s, tw, t, grp);
+            fft_pass<L, 16, 256, SIGN, false, true, GROUP>(v, s, tw, t, grp);
         }
     }
 }

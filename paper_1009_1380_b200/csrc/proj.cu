@@ -148,12 +148,12 @@ proj_kernel(const float *__restrict__ in, float *__restrict__ out,
             }
         }
     }
-    fft_reg<L, -1>(v, s, tw, t);
+    fft_reg<L, -1, true>(v, s, tw, t, f);          // the FFTs of a CTA only meet their own threads
     if constexpr (BLUE) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], __ldg(&hf[t + i * TF]));
-        __syncthreads();
-        fft_reg<L, +1>(v, s, tw, t);
+        fft_sync<TF, true>(f);
+        fft_reg<L, +1, true>(v, s, tw, t, f);
     }
     pdl_trigger();
     if constexpr (INV) {
@@ -257,7 +257,7 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
             }
         }
     }
-    fft_reg<L, -1>(v, s, tw, t);
+    fft_reg<L, -1, true>(v, s, tw, t, f);
     pdl_trigger();
     if (INV) {
         float z[2][16];
@@ -283,10 +283,10 @@ proj_pair_kernel(const float *__restrict__ in, float *__restrict__ out,
             if (live1) out[(size_t)r1 * n + k] = z[1][i];
         }
     } else {
-        __syncthreads();
+        fft_sync<TF, true>(f);
 #pragma unroll
         for (int i = 0; i < 16; ++i) s[FFT_PAD(t + i * TF)] = v[i];
-        __syncthreads();
+        fft_sync<TF, true>(f);
         float2 *Y = reinterpret_cast<float2 *>(out);
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
