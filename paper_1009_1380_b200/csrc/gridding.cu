@@ -109,30 +109,39 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
     // ---- consumers ----
     const int cd = n_det / 2;
     const double halfG = 0.5 * (double)G;
-    // position in the concatenated round sequence of this CTA's items
+    // position in the concatenated round sequence of this CTA's items.  Positions only move forward
+    // and a slot is loaded right after its position was normalised, so the descriptor of the item a
+    // position sits in (round count, first round) is kept in registers and re-read only when the
+    // position enters the next item (it was two dependent loads per round).
     struct Pos { int it, r; };
+    int c_it = -1, c_rc = 0, c_rb = 0;
     auto norm = [&](Pos p) {
         while (p.it < it_end) {
-            const int rc = __ldg(&items[p.it].round_count);
-            if (p.r < rc) break;
-            p.r -= rc;
+            if (p.it != c_it) {
+                c_it = p.it;
+                c_rc = __ldg(&items[p.it].round_count);
+                c_rb = __ldg(&items[p.it].round_begin);
+            }
+            if (p.r < c_rc) break;
+            p.r -= c_rc;
             ++p.it;
         }
         return p;
     };
-    auto load_slot = [&](const Pos &p) {
+    auto load_slot = [&](const Pos &p) {      // p: the position normalised last
         Slot s;
         s.ak = SLOT_EMPTY; s.lxy = 0;
-        if (p.it < it_end) s = slots[((size_t)__ldg(&items[p.it].round_begin) + p.r) * 32 + lane];
+        if (p.it < it_end) s = slots[((size_t)c_rb + p.r) * 32 + lane];
         return s;
     };
     auto load_dir = [&](const Slot &s) {
         return s.ak != SLOT_EMPTY ? __ldg(&cs[s.ak >> 16]) : make_double2(0.0, 0.0);
     };
     Pos cur = norm(Pos{it_begin, warp});
+    Slot sl = load_slot(cur);
     Pos p1 = norm(Pos{cur.it, cur.r + GATHER_WARPS});
+    Slot nx = load_slot(p1);
     Pos p2 = norm(Pos{p1.it, p1.r + GATHER_WARPS});
-    Slot sl = load_slot(cur), nx = load_slot(p1);
     double2 d = load_dir(sl);
     for (int it = it_begin; it < it_end; ++it) {
         const int q = it - it_begin, st = q % GATHER_STAGES;
