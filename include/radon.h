@@ -64,6 +64,7 @@ extern "C" {
 #define RADON_ENOMEM       -2   /* host or device allocation failed */
 #define RADON_ECUDA        -3   /* a CUDA runtime call failed (radon_last_cuda_error) */
 #define RADON_EARCH        -4   /* current device is not compute capability 10.x */
+#define RADON_ELIMIT       -6   /* radon_grid_only_static: the plan needs more scratch than the static arrays hold */
 #define RADON_EUNSUPPORTED -5   /* valid but not built: W not 4, 6 or 8; sigma*N neither a power of two in [16, 8192]
                                    nor 3 or 5 times a power of two in [16, 2048];
                                    n_det > 8192 (power of two) or 2*n_det - 1 > 8192 (otherwise) */
@@ -132,6 +133,30 @@ int radon_interp_only(radon_plan *p, const float *d_grid, float *d_polar, void *
  * every cell of d_grid is written exactly once (zeros included), no atomics, and
  * the result is bit-identical from run to run. */
 int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *stream);
+
+/* radon_grid_only for callers that cannot allocate (a stream under CUDA graph capture, a serving
+ * loop, a harness that forbids cudaMalloc): same arguments, same kernel, same schedule, bit-identical
+ * result, but the kernel's scratch -- the partial rectangles of tiles whose samples are dealt to
+ * several thread blocks, the counters of their merge, the summed j = 0 samples -- lives in
+ * file-scope device arrays of the library instead of a plan workspace.  The call allocates and
+ * frees nothing (no cudaMalloc / cudaFree / allocating library routine): one cudaMemsetAsync of
+ * the merge counters and one kernel launch on `stream`; at the first call on a device it also
+ * resolves the arrays' device addresses (cudaGetSymbolAddress, no allocation) -- make that call
+ * outside a capture.
+ *   Limits: RADON_STATIC_SCRATCH_SLOTS partial rectangles (64 x 32 complex cells, 16 KiB each:
+ * 32 MiB) and RADON_STATIC_SCRATCH_JOBS merge jobs.  Every GPU that loads the library holds these
+ * arrays (32 MiB + 33 KiB) until the process exits.  BASELINE.json's configs need 64 to ~1500
+ * rectangles; a plan that needs more than the limit (millions of samples on a small grid, e.g.
+ * 1024^2 with 4096 x 2048 samples: ~5500 rectangles) is rejected with RADON_ELIMIT before anything
+ * is launched; use radon_grid_only for it.
+ *   The arrays are shared by every call on a device, whatever the plan or stream, and keep the
+ * last call's contents: the counters are cleared by the call itself, everything else is written
+ * by the launch before it is read.  Two calls that overlap on the GPU (different streams, or
+ * graph branches) race on them: serialise such calls.
+ * Errors: RADON_EINVAL (null argument), RADON_ELIMIT, RADON_ECUDA. */
+#define RADON_STATIC_SCRATCH_SLOTS 2048
+#define RADON_STATIC_SCRATCH_JOBS 2048
+int radon_grid_only_static(radon_plan *p, const float *d_polar, float *d_grid, void *stream);
 
 /* The paper's own GPU design for the same gridding sum, kept as a measured comparison (prior
  * art, not the product path): load-balanced bins by recursive four-way splitting of the most

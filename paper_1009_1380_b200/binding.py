@@ -25,6 +25,7 @@ _SIGNATURES = {
     "radon_nufft1": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_interp_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_grid_only": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "radon_grid_only_static": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "radon_grid_only_paper_bins": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "radon_paper_bins_stats": (c_int, [c_void_p, P(c_int), P(c_ll), P(c_int), P(c_int)]),
     "radon_proj_ifft": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -388,6 +389,17 @@ class RadonPlan:
         grid = self._new((self.G, self.G), torch.complex64) if grid is None else grid
         self._chk(grid, torch.complex64, self.G * self.G, "grid")
         _check(lib().radon_grid_only(self._h, _ptr(polar), _ptr(grid), self._stream()), "radon_grid_only")
+        return grid
+
+    def radon_grid_only_static(self, polar, grid):
+        """radon_grid_only with the kernel's scratch in the library's static device arrays: the call
+        allocates nothing (the caller passes the output too).  RadonError -6 when the plan needs
+        more than RADON_STATIC_SCRATCH_SLOTS = 2048 partial rectangles; calls that overlap on the GPU race."""
+        import torch
+
+        self._chk(polar, torch.complex64, self.M, "polar")
+        self._chk(grid, torch.complex64, self.G * self.G, "grid")
+        _check(lib().radon_grid_only_static(self._h, _ptr(polar), _ptr(grid), self._stream()), "radon_grid_only_static")
         return grid
 
     def radon_grid_only_paper_bins(self, polar, grid=None, n_bins=4096):

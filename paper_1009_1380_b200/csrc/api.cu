@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -1000,6 +1001,63 @@ extern "C" int radon_kb_weights_host(int W, float sigma, float delta, float *w)
     return RADON_OK;
 }
 
+// ---- gridding without any allocation: scratch in a file-scope device array ---------------------
+// radon_grid_only_static runs the scatter kernel of radon_grid_only with its scratch (partial
+// rectangles of split tiles, merge counters, the summed j = 0 samples) in the three arrays below
+// instead of a plan workspace, for callers that cannot call cudaMalloc (a stream under graph capture,
+// a tight serving loop, a harness that forbids allocation).  Every GPU that loads the library holds
+// the arrays (32 MiB + 32 KiB + 648 B) until the process exits.  In host code the array names are
+// host-side stand-ins, not device addresses: their device addresses are resolved once per device,
+// with that device current, by cudaGetSymbolAddress (static_scratch_of) and passed to the kernel.
+// All calls on a device share the arrays: two calls that overlap on the GPU race.
+constexpr int STATIC_SCRATCH_SLOTS = RADON_STATIC_SCRATCH_SLOTS;   // partial rectangles of SR_X x SR_Y cells (16 KiB each)
+constexpr int STATIC_SCRATCH_JOBS = RADON_STATIC_SCRATCH_JOBS;     // merge jobs (MERGE_COUNTERS_PER_JOB counters each)
+static __device__ __align__(256) float2 g_static_scratch[(size_t)STATIC_SCRATCH_SLOTS * SR_X * SR_Y];
+static __device__ __align__(256) int g_static_tickets[STATIC_SCRATCH_JOBS * MERGE_COUNTERS_PER_JOB];
+static __device__ __align__(256) float2 g_static_dcbuf[(KW_MAX + 1) * (KW_MAX + 1)];
+
+struct StaticScratch { float2 *scratch = nullptr; int *tickets = nullptr; float2 *dcbuf = nullptr; bool ready = false; };
+constexpr int STATIC_MAX_DEVICES = 64;
+static StaticScratch g_static_dev[STATIC_MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+// device addresses of the arrays on the current device (resolved at the first call on that device)
+static int static_scratch_of(StaticScratch &out)
+{
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) { g_last_cuda_error = "radon_grid_only_static: device ordinal above 63"; return RADON_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticScratch &d = g_static_dev[dev];
+    if (!d.ready) {
+        CUDA_TRY(cudaGetSymbolAddress((void **)&d.scratch, g_static_scratch));
+        CUDA_TRY(cudaGetSymbolAddress((void **)&d.tickets, g_static_tickets));
+        CUDA_TRY(cudaGetSymbolAddress((void **)&d.dcbuf, g_static_dcbuf));
+        d.ready = true;
+    }
+    out = d;
+    return RADON_OK;
+}
+
+extern "C" int radon_grid_only_static(radon_plan *p, const float *d_polar, float *d_grid, void *stream)
+{
+    if (!p || !d_grid || !d_polar) return RADON_EINVAL;
+    const DevicePlan::Sched &q = p->dev.sched[0];                 // the full-grid schedule, as radon_grid_only
+    if (p->n_partial > STATIC_SCRATCH_SLOTS || q.n_merge_jobs > STATIC_SCRATCH_JOBS) return RADON_ELIMIT;
+    StaticScratch s;
+    int rc = static_scratch_of(s);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the arrays keep the last call's contents.  The merge counters must start at zero (a launch
+    // leaves them at zero, but a call that failed or was cut short need not have): cleared here, on
+    // the caller's stream.  Partial rectangles and the j = 0 sum are written in full by the launch
+    // before it reads them.
+    if (q.n_merge_jobs > 0)
+        CUDA_TRY(cudaMemsetAsync(s.tickets, 0, sizeof(int) * MERGE_COUNTERS_PER_JOB * (size_t)q.n_merge_jobs, st));
+    if (launch_scatter(p->dev, false, (const float2 *)d_polar, (float2 *)d_grid, s.scratch, s.dcbuf, s.tickets, st)) return RADON_ECUDA;
+    return check_launch();
+}
+
 extern "C" long long radon_kernel_launch_count(void) { return launch_count(); }
 
 extern "C" const char *radon_strerror(int code)
@@ -1010,6 +1068,7 @@ extern "C" const char *radon_strerror(int code)
     case RADON_ENOMEM: return "out of memory";
     case RADON_ECUDA: return "CUDA runtime error (see radon_last_cuda_error)";
     case RADON_EARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
+    case RADON_ELIMIT: return "the plan's gridding needs more scratch than the library's static arrays hold (radon_grid_only_static: 2048 partial rectangles, 2048 merge jobs; use radon_grid_only)";
     case RADON_EUNSUPPORTED: return "valid request outside this build (W not 4, 6 or 8, or sigma*N neither a power of two in [16, 8192] nor 3 or 5 times a power of two in [16, 2048], or n_det > 8192 (power of two) / 2*n_det-1 > 8192 (otherwise))";
     default: return "unknown error";
     }
