@@ -649,8 +649,8 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     int dpitch;
     if (cta.partial_slot >= 0) { dst = scratch + (size_t)cta.partial_slot * (SR_X * SR_Y); dpitch = SR_X; }
     else { dst = grid + (size_t)cta.ry0 * G + cta.rx0; dpitch = G; }
-    if (threadIdx.x < cta.rh)
-        bulk_s2g(dst + (size_t)threadIdx.x * dpitch, acc + threadIdx.x * ACC_PITCH, (uint32_t)(cta.rw * sizeof(float2)));
+    for (int y = threadIdx.x; y < cta.rh; y += SCATTER_THREADS)          // one bulk store per row
+        bulk_s2g(dst + (size_t)y * dpitch, acc + y * ACC_PITCH, (uint32_t)(cta.rw * sizeof(float2)));
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     if (cta.job < 0) {
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the reads

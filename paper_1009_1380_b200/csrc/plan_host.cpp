@@ -793,7 +793,7 @@ void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1,
 int scatter_round_limit(long long est_rounds, int n_workers)
 {
     const double slots = (double)std::max(1, n_workers) * SCATTER_CTAS_PER_SM * SCATTER_ITEMS;
-    const int r = (int)std::lround(1.8 * (double)est_rounds / slots);
+    const int r = (int)std::lround(RADON_SC_RFAC * (double)est_rounds / slots);
     return std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, r));
 }
 

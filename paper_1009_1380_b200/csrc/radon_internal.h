@@ -122,6 +122,9 @@ constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples
 #ifndef RADON_SC_RMIN
 #define RADON_SC_RMIN 12
 #endif
+#ifndef RADON_SC_RFAC
+#define RADON_SC_RFAC 1.8                // split limit = RFAC x the mean rounds per resident warp (0.7-1.8 measured)
+#endif
 constexpr int SCATTER_ROUND_MIN = RADON_SC_RMIN;  // lower limit (12: best over configs 1-3 and the paper's shape, 8..24 measured); the builder
                                       // picks 1.8 x the mean rounds per resident warp
 constexpr int SCATTER_CTAS_PER_SM = RADON_SC_CTAS;
