@@ -171,7 +171,7 @@ static int workspace_alloc(radon_plan *p, Workspace &w)
     if (!w.T && (rc = dev_alloc(p, &w.T, (size_t)(G / 2 + 1) * N))) return rc;
     if (!w.grid && (rc = dev_alloc(p, &w.grid, (size_t)G * G))) return rc;
     if (!w.polar && (rc = dev_alloc(p, &w.polar, (size_t)p->M))) return rc;
-    if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * SR_Y))) return rc;
+    if (!w.scratch && (rc = dev_alloc(p, &w.scratch, (size_t)std::max(p->n_partial, 1) * SR_X * p->geo.sr_y()))) return rc;
     if (!w.dcbuf && (rc = dev_alloc(p, &w.dcbuf, (size_t)(KW_MAX + 1) * (KW_MAX + 1)))) return rc;
     if (!w.tickets) {
         const size_t n = (size_t)std::max(p->n_jobs, 1) * MERGE_COUNTERS_PER_JOB;
@@ -193,7 +193,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     p->geo.init(N, n_angles, n_det, (double)sigma, W);
     p->M = (long long)n_angles * n_det;
     DevicePlan &d = p->dev;
-    d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det; d.W = W;
+    d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det; d.W = W; d.st_y = p->geo.st_y;
     d.n_sm = prop.multiProcessorCount;
     d.pdl = G <= 2048;
     const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
@@ -1043,7 +1043,9 @@ extern "C" int radon_grid_only_static(radon_plan *p, const float *d_polar, float
 {
     if (!p || !d_grid || !d_polar) return RADON_EINVAL;
     const DevicePlan::Sched &q = p->dev.sched[0];                 // the full-grid schedule, as radon_grid_only
-    if (p->n_partial > STATIC_SCRATCH_SLOTS || q.n_merge_jobs > STATIC_SCRATCH_JOBS) return RADON_ELIMIT;
+    // a partial rectangle of a plan with tall tiles (Geometry::st_y) takes more than one 64 x 32 slot of the array
+    if ((size_t)p->n_partial * SR_X * p->geo.sr_y() > (size_t)STATIC_SCRATCH_SLOTS * SR_X * SR_Y ||
+        q.n_merge_jobs > STATIC_SCRATCH_JOBS) return RADON_ELIMIT;
     StaticScratch s;
     int rc = static_scratch_of(s);
     if (rc) return rc;

@@ -219,8 +219,9 @@ gather_kernel(const float2 *__restrict__ grid, float2 *__restrict__ polar,
 // bank-conflict free.  Slots and sample values are prefetched ahead of use.  The finished
 // rectangle leaves through the copy engine (bulk shared -> global stores, one per row).
 constexpr int SCATTER_THREADS = SCATTER_ITEMS * 32;
-constexpr size_t SCATTER_ACC_BYTES = (size_t)SR_Y * ACC_PITCH * sizeof(float2);
-constexpr size_t SCATTER_SMEM = SCATTER_ACC_BYTES;
+// the accumulator of a CTA whose tiles are st_y rows high (a property of the plan: ST_Y or ST_Y_TALL)
+constexpr size_t scatter_acc_bytes(int st_y) { return (size_t)(SQ_Y * st_y) * ACC_PITCH * sizeof(float2); }
+constexpr size_t SCATTER_SMEM_MAX = scatter_acc_bytes(ST_Y_TALL);
 static_assert((ACC_PITCH * sizeof(float2)) % 16 == 0, "bulk stores need 16-byte rows");
 
 __device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes)
@@ -429,11 +430,12 @@ __device__ __forceinline__ void dc_compute(const float2 *__restrict__ polar, con
 // (W+1)^2 centre window (DESIGN.md R-tie).
 template <int NT>
 __device__ __forceinline__ void merge_rows(const MergeJob &j, int y_begin, int y_end, const float2 *__restrict__ scratch,
-                                           float2 *__restrict__ grid, int G, const float2 *__restrict__ dcbuf, int KW)
+                                           float2 *__restrict__ grid, int G, const float2 *__restrict__ dcbuf, int KW, int slot_cells)
 {
     const int ppr = j.rw >> 1, p_begin = ppr * y_begin, p_end = ppr * y_end;        // rw is even (check_schedules)
-    const float4 *src = reinterpret_cast<const float4 *>(scratch + (size_t)j.first_slot * (SR_X * SR_Y));
-    constexpr int SLOT4 = SR_X * SR_Y / 2, ROW4 = SR_X / 2;
+    const float4 *src = reinterpret_cast<const float4 *>(scratch + (size_t)j.first_slot * slot_cells);
+    const int SLOT4 = slot_cells / 2;
+    constexpr int ROW4 = SR_X / 2;
     const bool has_dc = j.expected > j.n_slots;
     for (int i0 = p_begin + threadIdx.x; i0 < p_end; i0 += 4 * NT) {
         float4 sum[4];
@@ -498,7 +500,7 @@ constexpr int MERGE_COUNTERS = MERGE_COUNTERS_PER_JOB;   // ints per job: arriva
 template <int NT>
 __device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *__restrict__ jobs, int *__restrict__ tickets,
                                            const float2 *__restrict__ scratch, float2 *__restrict__ grid, int G,
-                                           const float2 *__restrict__ dcbuf, int *s_flag, int KW)
+                                           const float2 *__restrict__ dcbuf, int *s_flag, int KW, int slot_cells)
 {
     int *cnt = tickets + job * MERGE_COUNTERS;
     const MergeJob j = jobs[job];
@@ -530,7 +532,7 @@ __device__ __forceinline__ void join_merge(int job, bool wait, const MergeJob *_
             __syncthreads();
             const int c = *s_flag;
             if (c >= n_chunks) break;
-            merge_rows<NT>(j, c * rows, min(j.rh, (c + 1) * rows), scratch, grid, G, dcbuf, KW);
+            merge_rows<NT>(j, c * rows, min(j.rh, (c + 1) * rows), scratch, grid, G, dcbuf, KW, slot_cells);
         }
     }
     __syncthreads();
@@ -547,11 +549,12 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
                const ScatterCta *__restrict__ ctas, const Slot *__restrict__ slots,
                const double2 *__restrict__ cs, const KbPoly kp,
                int G, int n_det, int nyq_split, float2 *__restrict__ dcbuf, int n_angles, int half,
-               const MergeJob *__restrict__ jobs, int *__restrict__ tickets, const DcJobs dcj)
+               const MergeJob *__restrict__ jobs, int *__restrict__ tickets, const DcJobs dcj, int st_y)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *acc = reinterpret_cast<float2 *>(smem_raw);
     __shared__ int s_flag;
+    const int slot_cells = SR_X * SQ_Y * st_y;      // cells of a partial rectangle in scratch
     pdl_prologue();
     if (blockIdx.x == 0) {
         // CTA 0: the j = 0 samples of all angles, summed (fixed order) while the others grid; the
@@ -559,7 +562,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
         dc_compute<SCATTER_THREADS, KW>(polar, kp, n_det, n_angles, half, acc, dcbuf);
         __threadfence();
         for (int q = 0; q < dcj.n; ++q)
-            join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW);
+            join_merge<SCATTER_THREADS>(dcj.job[q], false, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW, slot_cells);
         return;
     }
     __shared__ ScatterCta cta;
@@ -594,7 +597,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     Slot s0 = load_slot(0), s1 = load_slot(1), s2 = load_slot(2), s3 = load_slot(3);
     {   // zero the accumulator while those loads are in flight
         float4 *z = reinterpret_cast<float4 *>(acc);
-        for (int i = threadIdx.x; i < (int)(SCATTER_ACC_BYTES / 16); i += SCATTER_THREADS)
+        for (int i = threadIdx.x; i < SQ_Y * st_y * ACC_PITCH / 2; i += SCATTER_THREADS)
             z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     float2 v0, v1;
@@ -647,7 +650,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     __syncthreads();
     float2 *dst;
     int dpitch;
-    if (cta.partial_slot >= 0) { dst = scratch + (size_t)cta.partial_slot * (SR_X * SR_Y); dpitch = SR_X; }
+    if (cta.partial_slot >= 0) { dst = scratch + (size_t)cta.partial_slot * slot_cells; dpitch = SR_X; }
     else { dst = grid + (size_t)cta.ry0 * G + cta.rx0; dpitch = G; }
     for (int y = threadIdx.x; y < cta.rh; y += SCATTER_THREADS)          // one bulk store per row
         bulk_s2g(dst + (size_t)y * dpitch, acc + y * ACC_PITCH, (uint32_t)(cta.rw * sizeof(float2)));
@@ -660,7 +663,7 @@ scatter_kernel(const float2 *__restrict__ polar, float2 *__restrict__ grid, floa
     asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
     __threadfence();
-    join_merge<SCATTER_THREADS>(cta.job, true, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW);
+    join_merge<SCATTER_THREADS>(cta.job, true, jobs, tickets, scratch, grid, G, dcbuf, &s_flag, KW, slot_cells);
 }
 
 // The j = 0 samples (k = n/2) of all angles sit at kappa = (0,0) and share one footprint, so
@@ -690,9 +693,9 @@ int launch_scatter(const DevicePlan &p, bool half, const float2 *polar, float2 *
     dcj.n = q.n_dc_jobs;
     for (int i = 0; i < MAX_DC_JOBS; ++i) dcj.job[i] = q.dc_jobs[i];
     // CTA 0 sums the j = 0 samples; CTA b > 0 grids scatter_ctas[b - 1] (heaviest first)
-    RADON_FOR_W(p.W, launch_pdl(p.pdl, scatter_kernel<WW>, q.n_scatter_ctas + 1, SCATTER_THREADS, SCATTER_SMEM, st,
+    RADON_FOR_W(p.W, launch_pdl(p.pdl, scatter_kernel<WW>, q.n_scatter_ctas + 1, SCATTER_THREADS, scatter_acc_bytes(p.st_y), st,
         polar, grid, scratch, q.scatter_ctas, q.scatter_slots, p.cs, p.kb, p.G, p.n_det, nyq,
-        dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj);)
+        dcbuf, p.n_angles, half ? 1 : 0, q.merge_jobs, tickets, dcj, p.st_y);)
     count_launch();
     return 0;
 }
@@ -701,8 +704,8 @@ int init_kernel_attributes()
 {
     if (set_smem(gather_kernel<4>, gather_smem(4)) || set_smem(gather_kernel<6>, gather_smem(6)) ||
         set_smem(gather_kernel<8>, gather_smem(8))) return -1;
-    if (set_smem(scatter_kernel<4>, SCATTER_SMEM) || set_smem(scatter_kernel<6>, SCATTER_SMEM) ||
-        set_smem(scatter_kernel<8>, SCATTER_SMEM)) return -1;
+    if (set_smem(scatter_kernel<4>, SCATTER_SMEM_MAX) || set_smem(scatter_kernel<6>, SCATTER_SMEM_MAX) ||
+        set_smem(scatter_kernel<8>, SCATTER_SMEM_MAX)) return -1;
     return 0;
 }
 

@@ -12,6 +12,7 @@ namespace radon {
 struct DevicePlan {
     int N = 0, G = 0, n_angles = 0, n_det = 0, LP = 0;   // LP: FFT length of the projection DFT
     int W = 6;                    // Kaiser-Bessel width (4, 6 or 8)
+    int st_y = ST_Y;              // rows of a scatter tile (Geometry::st_y)
     int n_sm = 148;               // multiprocessors of the device (persistent grids)
     bool pdl = false;             // programmatic dependent launch between the kernels of a call (small grids)
     // tables

@@ -44,6 +44,7 @@ void Geometry::init(int N_, int n_angles_, int n_det_, double sigma_, int W_)
 {
     N = N_; n_angles = n_angles_; n_det = n_det_; sigma = sigma_; W = W_;
     G = (int)std::llround(sigma * N);
+    st_y = (G >= ST_Y_TALL_MIN_G) ? ST_Y_TALL : ST_Y;
     cs.resize(2 * (size_t)n_angles);
     const double scale = (double)G / (double)n_det;
     for (int a = 0; a < n_angles; ++a) {
@@ -525,9 +526,9 @@ static void scatter_rects(const Geometry &g, bool half, std::vector<RowSeg> &seg
     else segs.push_back(RowSeg{0, G});
     for (const RowSeg &sg : segs) {
         seg_first.push_back((int)rects.size());
-        for (int ry0 = sg.y0; ry0 < sg.y1; ry0 += SR_Y)
+        for (int ry0 = sg.y0; ry0 < sg.y1; ry0 += g.sr_y())
             for (int rx0 = 0; rx0 < G; rx0 += SR_X)
-                rects.push_back(RectGeom{rx0, ry0, std::min(SR_X, G - rx0), std::min(SR_Y, sg.y1 - ry0)});
+                rects.push_back(RectGeom{rx0, ry0, std::min(SR_X, G - rx0), std::min(g.sr_y(), sg.y1 - ry0)});
     }
 }
 
@@ -568,7 +569,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
                         for (size_t sg = 0; sg < segs.size(); ++sg) {
                             const int ylo = std::max(by, segs[sg].y0), yhi = std::min(by + KH, segs[sg].y1 - 1);
                             if (ylo > yhi) continue;
-                            const int ry_lo = (ylo - segs[sg].y0) / SR_Y, ry_hi = (yhi - segs[sg].y0) / SR_Y;
+                            const int ry_lo = (ylo - segs[sg].y0) / g.sr_y(), ry_hi = (yhi - segs[sg].y0) / g.sr_y();
                             for (int ry = ry_lo; ry <= ry_hi; ++ry)
                                 for (int rx = rx_lo; rx <= rx_hi; ++rx) {
                                     const int r = seg_first[sg] + ry * nrx + rx;
@@ -590,7 +591,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
     {
         long long est_rounds = 0;
         for (int r = 0; r < nrect; ++r) est_rounds += (count[r + 1] - count[r] + 27) / 28;
-        round_max = scatter_round_limit(est_rounds, n_workers);
+        round_max = scatter_round_limit(g, est_rounds, n_workers);
     }
     struct Pending { ScatterCta cta; long long work; };
     std::vector<Pending> ctas;
@@ -599,7 +600,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
 
     for (int r = 0; r < nrect; ++r) {
         const int rx0 = rects[r].rx0, ry0 = rects[r].ry0, rw = rects[r].rw, rh = rects[r].rh;
-        const int nsx = (rw + ST_X - 1) / ST_X, nsy = (rh + ST_Y - 1) / ST_Y;
+        const int nsx = (rw + ST_X - 1) / ST_X, nsy = (rh + g.st_y - 1) / g.st_y;
         const uint32_t lo = count[r], hi = count[r + 1];
 
         // quadrants of the rectangle and, for each, every sample image whose footprint
@@ -611,8 +612,8 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
         for (int iy = 0; iy < nsy; ++iy)
             for (int ix = 0; ix < nsx; ++ix) {
                 ScatterItem &I = geom[iy * SQ_X + ix];
-                I.sx0 = ix * ST_X; I.sy0 = iy * ST_Y;
-                I.sw = std::min(ST_X, rw - I.sx0); I.sh = std::min(ST_Y, rh - I.sy0);
+                I.sx0 = ix * ST_X; I.sy0 = iy * g.st_y;
+                I.sw = std::min(ST_X, rw - I.sx0); I.sh = std::min(g.st_y, rh - I.sy0);
                 const int ax0 = rx0 + I.sx0, ay0 = ry0 + I.sy0;          // absolute origin
                 for (uint32_t q = lo; q < hi; ++q) {
                     const Image &im = inc[q];
@@ -790,10 +791,10 @@ void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1,
     scatter_k1 = scatter_k_end(g, half);
 }
 
-int scatter_round_limit(long long est_rounds, int n_workers)
+int scatter_round_limit(const Geometry &g, long long est_rounds, int n_workers)
 {
-    const double slots = (double)std::max(1, n_workers) * SCATTER_CTAS_PER_SM * SCATTER_ITEMS;
-    const int r = (int)std::lround(RADON_SC_RFAC * (double)est_rounds / slots);
+    const double slots = (double)std::max(1, n_workers) * g.scatter_ctas_per_sm() * SCATTER_ITEMS;
+    const int r = (int)std::lround(g.scatter_rfac() * (double)est_rounds / slots);
     return std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, r));
 }
 
@@ -832,7 +833,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
         for (int i = 0; i < 32; ++i) {
             if (lanes[i].ak == SLOT_EMPTY) continue;
             const int xi = lanes[i].lxy & 0xffff, yi = lanes[i].lxy >> 16;
-            if (disjoint && (xi >= ST_X + KH || yi >= ST_Y + KH)) ++bad;
+            if (disjoint && (xi >= ST_X + KH || yi >= g.st_y + KH)) ++bad;
             int same_bank = 0;      // lanes of this half-warp in the same bank pair: at most 2-way
             for (int j = 0; j < 32; ++j)
                 if (j != i && lanes[j].ak != SLOT_EMPTY && (i >> 4) == (j >> 4) &&
@@ -892,7 +893,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
     std::vector<int> slot_owner(s.n_partial_slots, 0);
     for (const ScatterCta &c : s.scatter_ctas) {
         if (c.rx0 < 0 || c.ry0 < 0 || c.rx0 + c.rw > G || c.ry0 + c.rh > G || c.rw < 1 || c.rh < 1 ||
-            c.rw > SR_X || c.rh > SR_Y || (c.rw & 1) || (c.rx0 & 1)) { ++bad; continue; }
+            c.rw > SR_X || c.rh > g.sr_y() || (c.rw & 1) || (c.rx0 & 1)) { ++bad; continue; }
         if (c.partial_slot >= 0) {
             if (c.partial_slot >= s.n_partial_slots) { ++bad; continue; }
             ++slot_owner[c.partial_slot];
@@ -905,7 +906,7 @@ long long check_schedules(const Geometry &g, const Schedules &s)
             const ScatterItem &A = c.items[i];
             if (A.round_count == 0) continue;
             if (A.sx0 < 0 || A.sy0 < 0 || A.sw < 1 || A.sh < 1 || A.sx0 + A.sw > c.rw || A.sy0 + A.sh > c.rh ||
-                A.sw > ST_X || A.sh > ST_Y) ++bad;
+                A.sw > ST_X || A.sh > g.st_y) ++bad;
             for (int j = i + 1; j < SCATTER_ITEMS; ++j) {
                 const ScatterItem &B = c.items[j];
                 if (B.round_count == 0) continue;

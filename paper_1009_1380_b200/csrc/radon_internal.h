@@ -96,7 +96,7 @@ constexpr int GATHER_ROUND_CAP = RADON_GCAP;  // rounds (of 32 samples) per CTA;
 // slots, first sample values: three dependent global loads; the flush) overlaps the accumulation
 // of eleven independent warps.  Measured at config 4 against four warps per 128 x 64 rectangle at
 // three CTAs per multiprocessor: bare 92.7 -> 89.0 us, A2 stage 58.1 -> 56.9 us, 32-slice batch
-// 185.6 -> 180.4 us per pair.
+// 185.6 -> 180.4 us per pair.  Grids of ST_Y_TALL_MIN_G and more use tiles of ST_Y_TALL rows (below).
 #ifndef RADON_SC_FAST
 #define RADON_SC_FAST 1               // unclipped footprints first, run without tap predicates
 #endif
@@ -117,10 +117,19 @@ constexpr int SQ_X = RADON_SQ_X, SQ_Y = RADON_SQ_Y;   // quadrants per rectangle
 constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
 constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
-constexpr int SB_W_MAX = ST_X + KW_MAX - 1, SB_H_MAX = ST_Y + KW_MAX - 1;   // range of biased base coordinates in a tile (ST + W - 1)
+// Tile height is a property of the plan: ST_Y rows, or ST_Y_TALL on large grids (Geometry::st_y), where the
+// scatter is bound by shared-memory bandwidth, not latency: eight warps per multiprocessor already fill
+// the pipe, and taller tiles list fewer footprints twice and pay fewer prologues.
+constexpr int ST_Y_TALL = (SCATTER_ITEMS == 1) ? 48 : ST_Y;
+constexpr int ST_Y_TALL_MIN_G = 4096;               // grids at least this wide get the tall tiles
+constexpr int SCATTER_CTAS_PER_SM_TALL = 8;         // 8 x 25 KB of accumulators
+constexpr int SB_W_MAX = ST_X + KW_MAX - 1, SB_H_MAX = ST_Y_TALL + KW_MAX - 1;   // range of biased base coordinates in a tile (ST + W - 1)
 constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples are split over CTAs: upper and
 #ifndef RADON_SC_RMIN
 #define RADON_SC_RMIN 12
+#endif
+#ifndef RADON_SC_RFAC_TALL
+#define RADON_SC_RFAC_TALL 1.4           // the same for the tall tiles (1.0-1.8 measured)
 #endif
 #ifndef RADON_SC_RFAC
 #define RADON_SC_RFAC 1.8                // split limit = RFAC x the mean rounds per resident warp (0.7-1.8 measured)
@@ -173,6 +182,10 @@ constexpr int MAX_DC_JOBS = 4;  // the (W+1)^2 centre window touches at most 2 x
 struct Geometry {
     int N = 0, G = 0, n_angles = 0, n_det = 0, W = 6;
     double sigma = 2.0;
+    int st_y = ST_Y;            // rows of a scatter tile (ST_Y or ST_Y_TALL)
+    int sr_y() const { return SQ_Y * st_y; }                                  // rows of a CTA's rectangle
+    int scatter_ctas_per_sm() const { return st_y == ST_Y ? SCATTER_CTAS_PER_SM : SCATTER_CTAS_PER_SM_TALL; }
+    double scatter_rfac() const { return st_y == ST_Y ? RADON_SC_RFAC : RADON_SC_RFAC_TALL; }
     std::vector<double> cs;     // per angle: (G/n) cos(theta_a), (G/n) sin(theta_a)
 
     void init(int N_, int n_angles_, int n_det_, double sigma_, int W_);
@@ -202,7 +215,7 @@ void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers
 struct TileRect { int rx0, ry0, rw, rh; };
 void scatter_tile_rects(const Geometry &g, bool half, std::vector<TileRect> &tiles);   // tiles the scatter writes
 void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1, int &scatter_k1);
-int scatter_round_limit(long long est_rounds, int n_workers);    // rounds per warp before a tile is split
+int scatter_round_limit(const Geometry &g, long long est_rounds, int n_workers);    // rounds per warp before a tile is split
 void finish_gather(Schedules &out, int n_workers);               // gather items -> persistent CTAs
 // Returns the number of violated invariants (0 = schedules are valid).
 long long check_schedules(const Geometry &g, const Schedules &s);
