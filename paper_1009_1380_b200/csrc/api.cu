@@ -195,7 +195,7 @@ static int plan_create_impl(radon_plan *p, int N, int n_angles, int n_det, float
     DevicePlan &d = p->dev;
     d.N = N; d.G = G; d.n_angles = n_angles; d.n_det = n_det; d.W = W; d.st_y = p->geo.st_y;
     d.n_sm = prop.multiProcessorCount;
-    d.pdl = G <= 2048;
+    d.pdl = true;   // every kernel of a call waits (griddepcontrol.wait) for its predecessor and signals its dependents late
     const bool pow2 = (n_det & (n_det - 1)) == 0 && n_det >= 16;
     d.LP = pow2 ? n_det : std::max(16, next_pow2(2 * n_det - 1));
 

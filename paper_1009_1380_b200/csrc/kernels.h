@@ -14,7 +14,7 @@ struct DevicePlan {
     int W = 6;                    // Kaiser-Bessel width (4, 6 or 8)
     int st_y = ST_Y;              // rows of a scatter tile (Geometry::st_y)
     int n_sm = 148;               // multiprocessors of the device (persistent grids)
-    bool pdl = false;             // programmatic dependent launch between the kernels of a call (small grids)
+    bool pdl = false;             // programmatic dependent launch between the kernels of a call
     // tables
     double2 *cs = nullptr;        // per angle (G/n)(cos, sin), fp64
     KbPoly kb;                    // polynomial pieces of the Kaiser-Bessel kernel
@@ -72,10 +72,10 @@ static inline int set_smem(F kernel, size_t bytes)
 // wait, so the order of the sequence is what stream order would give.  A kernel calls
 // pdl_trigger() when its main work is done: once all its CTAs have, the successor's CTAs are
 // scheduled onto the multiprocessors the tail of this grid leaves idle and run their set-up.
-// Used for G <= 2048 (measured on a B200: config 1 pair 57 -> 43 us, config 2 82 -> 64 us, the paper's
-// 180 x 1024 shape 71 -> 54 us; at G = 4096 the kernels are long and early successors cost 1-2 %).
-// RADON_PDL=0 in the environment launches plainly (A/B).  RADON_PDL=0 in the
-// environment launches plainly (A/B).
+// Measured on a B200: config 1 pair 57 -> 43 us, config 2 82 -> 64 us, the paper's 180 x 1024 shape
+// 71 -> 54 us; at config 4 (G = 4096), with the trigger late in every kernel, one slice at a time
+// 222-230 -> 214 us, bare gridding 83.8 -> 81.9 us, bare interpolation 42.0 -> 40.8 us, the 32-slice batch
+// unchanged.  RADON_PDL=0 in the environment launches plainly (A/B).
 bool pdl_enabled();                  // RADON_PDL != 0 and no graph capture of the library in progress
 void pdl_suppress(bool on);          // the solver's graph capture launches plainly (measured: graph + PDL is slower)
 #ifdef __CUDACC__
