@@ -60,8 +60,8 @@ def stage_bytes(N, G, M, n_angles, W=6):
 # 126 MB L2 when the kernel ended (one-slice capture: the grid written by A2 is read by A3 from L2).
 NCU_TRAFFIC_SOURCE = "profiles/r02_kernels.md (ncu --set full, one slice at a time; copied, not measured by this run)"
 NCU_DRAM_BYTES = {
-    "F1_colfft": 16.91e6, "F2_rowfft": 45.21e6, "F3_gather": 68.57e6, "F4_proj_ifft": 8.59e6,
-    "A1_proj_fft": 8.46e6, "A2_scatter": 39.62e6, "A3_rowifft": 71.86e6, "A4_colifft": 33.68e6,
+    "F1_colfft": 17.06e6, "F2_rowfft": 44.63e6, "F3_gather": 69.30e6, "F4_proj_ifft": 8.59e6,
+    "A1_proj_fft": 8.46e6, "A2_scatter": 40.66e6, "A3_rowifft": 71.60e6, "A4_colifft": 33.74e6,
 }
 
 

@@ -144,7 +144,7 @@ int radon_grid_only(radon_plan *p, const float *d_polar, float *d_grid, void *st
  * resolves the arrays' device addresses (cudaGetSymbolAddress, no allocation) -- make that call
  * outside a capture.
  *   Limits: RADON_STATIC_SCRATCH_SLOTS partial rectangles (64 x 32 complex cells, 16 KiB each:
- * 32 MiB; plans with sigma*N >= 4096 use 64 x 48 tiles and take 1.5 slots per rectangle) and RADON_STATIC_SCRATCH_JOBS merge jobs.  Every GPU that loads the library holds these
+ * 32 MiB; plans with sigma*N >= 4096 use 64 x 40 tiles and take 1.25 slots per rectangle) and RADON_STATIC_SCRATCH_JOBS merge jobs.  Every GPU that loads the library holds these
  * arrays (32 MiB + 33 KiB) until the process exits.  BASELINE.json's configs need 64 to ~1500
  * rectangles; a plan that needs more than the limit (millions of samples on a small grid, e.g.
  * 1024^2 with 4096 x 2048 samples: ~5500 rectangles) is rejected with RADON_ELIMIT before anything

@@ -389,13 +389,13 @@ done:
 // ---- both schedules of one plan half ---------------------------------------------------------------
 static inline long long posmod_ll(long long v, long long m) { const long long r = v % m; return r < 0 ? r + m : r; }
 
-struct ScatterSplitArg { int n_workers; int round_max; const std::vector<int> *k_min; const Geometry *g; };
+struct ScatterSplitArg { int n_workers; int round_max; const std::vector<int> *k_min; const Geometry *g; bool half; };
 static void scatter_split(std::vector<PackRegion> &regions, void *argp)
 {
     ScatterSplitArg *arg = static_cast<ScatterSplitArg *>(argp);
     long long est = 0;
     for (const PackRegion &r : regions) est += (r.n_in + r.n_cl + 27) / 28;
-    arg->round_max = scatter_round_limit(*arg->g, est, arg->n_workers);
+    arg->round_max = scatter_round_limit(*arg->g, arg->half, est, arg->n_workers);
     // host rule (plan_host.cpp): a tile's samples are dealt to K CTAs when one warp would run more
     // than round_max rounds at ~24 samples per round
     for (PackRegion &r : regions) {
@@ -483,7 +483,7 @@ int build_schedules_device(const Geometry &g, const double2 *d_cs, bool half, in
         }
         // Where samples pile up on few base cells (the centre) a share needs more rounds than its
         // sample count suggests: like the host builder, such a tile is dealt to more CTAs and packed again.
-        ScatterSplitArg arg{n_workers, SCATTER_ROUND_MAX, nullptr, &g};
+        ScatterSplitArg arg{n_workers, SCATTER_ROUND_MAX, nullptr, &g, half};
         prm.k0 = 0; prm.k1 = sk1; prm.skip_k = g.n_det / 2; prm.pitch = ACC_PITCH; prm.disjoint = true;
         prm.split = scatter_split; prm.redo = scatter_redo; prm.split_arg = &arg;
         {

@@ -591,7 +591,7 @@ static void build_scatter(const Geometry &g, Schedules &out, int n_workers)
     {
         long long est_rounds = 0;
         for (int r = 0; r < nrect; ++r) est_rounds += (count[r + 1] - count[r] + 27) / 28;
-        round_max = scatter_round_limit(g, est_rounds, n_workers);
+        round_max = scatter_round_limit(g, out.half, est_rounds, n_workers);
     }
     struct Pending { ScatterCta cta; long long work; };
     std::vector<Pending> ctas;
@@ -791,10 +791,10 @@ void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1,
     scatter_k1 = scatter_k_end(g, half);
 }
 
-int scatter_round_limit(const Geometry &g, long long est_rounds, int n_workers)
+int scatter_round_limit(const Geometry &g, bool half, long long est_rounds, int n_workers)
 {
     const double slots = (double)std::max(1, n_workers) * g.scatter_ctas_per_sm() * SCATTER_ITEMS;
-    const int r = (int)std::lround(g.scatter_rfac() * (double)est_rounds / slots);
+    const int r = (int)std::lround(g.scatter_rfac(half) * (double)est_rounds / slots);
     return std::max(SCATTER_ROUND_MIN, std::min(SCATTER_ROUND_MAX, r));
 }
 

@@ -118,18 +118,25 @@ constexpr int SR_X = SQ_X * ST_X, SR_Y = SQ_Y * ST_Y; // CTA output rectangle
 constexpr int SCATTER_ITEMS = SQ_X * SQ_Y;            // warps per CTA
 constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byte multiple, != 0 mod 16)
 // Tile height is a property of the plan: ST_Y rows, or ST_Y_TALL on large grids (Geometry::st_y), where the
-// scatter is bound by shared-memory bandwidth, not latency: eight warps per multiprocessor already fill
+// scatter is bound by shared-memory bandwidth, not latency: eight to ten warps per multiprocessor fill
 // the pipe, and taller tiles list fewer footprints twice and pay fewer prologues.
-constexpr int ST_Y_TALL = (SCATTER_ITEMS == 1) ? 48 : ST_Y;
+#ifndef RADON_ST_Y_TALL
+#define RADON_ST_Y_TALL 40
+#define RADON_SC_CTAS_TALL 10
+#endif
+constexpr int ST_Y_TALL = (SCATTER_ITEMS == 1) ? RADON_ST_Y_TALL : ST_Y;
 constexpr int ST_Y_TALL_MIN_G = 4096;               // grids at least this wide get the tall tiles
-constexpr int SCATTER_CTAS_PER_SM_TALL = 8;         // 8 x 25 KB of accumulators
+constexpr int SCATTER_CTAS_PER_SM_TALL = RADON_SC_CTAS_TALL;   // 10 x 21 KB of accumulators
 constexpr int SB_W_MAX = ST_X + KW_MAX - 1, SB_H_MAX = ST_Y_TALL + KW_MAX - 1;   // range of biased base coordinates in a tile (ST + W - 1)
 constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples are split over CTAs: upper and
 #ifndef RADON_SC_RMIN
 #define RADON_SC_RMIN 12
 #endif
+#ifndef RADON_SC_RFAC_TALL_FULL
+#define RADON_SC_RFAC_TALL_FULL 1.2      // the full-grid schedule of the tall tiles (twice the rounds per warp of the half one)
+#endif
 #ifndef RADON_SC_RFAC_TALL
-#define RADON_SC_RFAC_TALL 1.4           // the same for the tall tiles (1.0-1.8 measured)
+#define RADON_SC_RFAC_TALL 1.5           // the same for the tall tiles, Hermitian-half schedule (1.2-1.8 measured)
 #endif
 #ifndef RADON_SC_RFAC
 #define RADON_SC_RFAC 1.8                // split limit = RFAC x the mean rounds per resident warp (0.7-1.8 measured)
@@ -185,7 +192,7 @@ struct Geometry {
     int st_y = ST_Y;            // rows of a scatter tile (ST_Y or ST_Y_TALL)
     int sr_y() const { return SQ_Y * st_y; }                                  // rows of a CTA's rectangle
     int scatter_ctas_per_sm() const { return st_y == ST_Y ? SCATTER_CTAS_PER_SM : SCATTER_CTAS_PER_SM_TALL; }
-    double scatter_rfac() const { return st_y == ST_Y ? RADON_SC_RFAC : RADON_SC_RFAC_TALL; }
+    double scatter_rfac(bool half) const { return st_y == ST_Y ? RADON_SC_RFAC : (half ? RADON_SC_RFAC_TALL : RADON_SC_RFAC_TALL_FULL); }
     std::vector<double> cs;     // per angle: (G/n) cos(theta_a), (G/n) sin(theta_a)
 
     void init(int N_, int n_angles_, int n_det_, double sigma_, int W_);
@@ -215,7 +222,7 @@ void build_schedules(const Geometry &g, Schedules &out, bool half, int n_workers
 struct TileRect { int rx0, ry0, rw, rh; };
 void scatter_tile_rects(const Geometry &g, bool half, std::vector<TileRect> &tiles);   // tiles the scatter writes
 void sample_ranges(const Geometry &g, bool half, int &gather_k0, int &gather_k1, int &scatter_k1);
-int scatter_round_limit(const Geometry &g, long long est_rounds, int n_workers);    // rounds per warp before a tile is split
+int scatter_round_limit(const Geometry &g, bool half, long long est_rounds, int n_workers);    // rounds per warp before a tile is split
 void finish_gather(Schedules &out, int n_workers);               // gather items -> persistent CTAs
 // Returns the number of violated invariants (0 = schedules are valid).
 long long check_schedules(const Geometry &g, const Schedules &s);

@@ -63,13 +63,13 @@ def test_schedule_invariants(shape, half):
 @pytest.mark.parametrize("half", [False, True])
 @pytest.mark.parametrize("shape", [(2048, 12, 40), (2048, 40, 2048), (1536, 9, 100)])
 def test_schedule_invariants_with_tall_scatter_tiles(shape, half):
-    """Grids of 4096 and more get 64 x 48 scatter tiles (Geometry::st_y; 64 x 32 below): the same
+    """Grids of 4096 and more get 64 x 40 scatter tiles (Geometry::st_y; 64 x 32 below): the same
     invariants, and the tile count says which height the plan took (G = 4096: 64 tiles across,
-    ceil(G / 48) = 86 down on the full grid against 128 with 32 rows; G = 3072 keeps 32 rows)."""
+    ceil(G / 40) = 103 down on the full grid against 128 with 32 rows; G = 3072 keeps 32 rows)."""
     assert rb.schedule_selfcheck(*shape, half=half) == (0, 0)
     st = rb.schedule_host_stats(*shape, half=half)
     G = 2 * shape[0]
-    rows = (1 + -(-(G // 2) // (48 if G >= 4096 else 32))) if half else -(-G // (48 if G >= 4096 else 32))
+    rows = (1 + -(-(G // 2) // (40 if G >= 4096 else 32))) if half else -(-G // (40 if G >= 4096 else 32))
     tiles = (G // 64) * rows
     assert tiles <= st["scatter_ctas"] <= tiles + st["partial_rects"], (st["scatter_ctas"], tiles)
 
