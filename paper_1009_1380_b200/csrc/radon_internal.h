@@ -125,7 +125,10 @@ constexpr int ACC_PITCH = SR_X + 2;   // 130 complex per accumulator row (16-byt
 #define RADON_SC_CTAS_TALL 10
 #endif
 constexpr int ST_Y_TALL = (SCATTER_ITEMS == 1) ? RADON_ST_Y_TALL : ST_Y;
-constexpr int ST_Y_TALL_MIN_G = 4096;               // grids at least this wide get the tall tiles
+#ifndef RADON_ST_Y_TALL_MIN_G
+#define RADON_ST_Y_TALL_MIN_G 4096
+#endif
+constexpr int ST_Y_TALL_MIN_G = RADON_ST_Y_TALL_MIN_G;               // grids at least this wide get the tall tiles
 constexpr int SCATTER_CTAS_PER_SM_TALL = RADON_SC_CTAS_TALL;   // 10 x 21 KB of accumulators
 constexpr int SB_W_MAX = ST_X + KW_MAX - 1, SB_H_MAX = ST_Y_TALL + KW_MAX - 1;   // range of biased base coordinates in a tile (ST + W - 1)
 constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples are split over CTAs: upper and
