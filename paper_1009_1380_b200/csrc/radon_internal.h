@@ -135,6 +135,10 @@ constexpr int SCATTER_ROUND_MAX = 96; // rounds per warp before a tile's samples
 #ifndef RADON_SC_RMIN
 #define RADON_SC_RMIN 12
 #endif
+#define RADON_SC_RFAC_FULL_DEFAULT 1.8
+#ifndef RADON_SC_RFAC_FULL
+#define RADON_SC_RFAC_FULL RADON_SC_RFAC_FULL_DEFAULT
+#endif
 #ifndef RADON_SC_RFAC_TALL_FULL
 #define RADON_SC_RFAC_TALL_FULL 1.2      // the full-grid schedule of the tall tiles (twice the rounds per warp of the half one)
 #endif
@@ -195,7 +199,7 @@ struct Geometry {
     int st_y = ST_Y;            // rows of a scatter tile (ST_Y or ST_Y_TALL)
     int sr_y() const { return SQ_Y * st_y; }                                  // rows of a CTA's rectangle
     int scatter_ctas_per_sm() const { return st_y == ST_Y ? SCATTER_CTAS_PER_SM : SCATTER_CTAS_PER_SM_TALL; }
-    double scatter_rfac(bool half) const { return st_y == ST_Y ? RADON_SC_RFAC : (half ? RADON_SC_RFAC_TALL : RADON_SC_RFAC_TALL_FULL); }
+    double scatter_rfac(bool half) const { return st_y == ST_Y ? (half ? RADON_SC_RFAC : RADON_SC_RFAC_FULL) : (half ? RADON_SC_RFAC_TALL : RADON_SC_RFAC_TALL_FULL); }
     std::vector<double> cs;     // per angle: (G/n) cos(theta_a), (G/n) sin(theta_a)
 
     void init(int N_, int n_angles_, int n_det_, double sigma_, int W_);
